@@ -1,0 +1,123 @@
+/* dgswem.h -- C ABI of the B200-native DG-SWEM hot path (arxiv 2508.21208).
+ *
+ * The library evaluates, on ONE sm_100a GPU in fp64, the per-RK-stage discontinuous Galerkin
+ * right-hand side of the 2-D shallow water equations on an unstructured triangular mesh
+ * (eqs (1)-(5); kernels EDGE / GATHER / AREA = PAPER.md Alg. 2 / 3 / 1) and the
+ * SSP Runge-Kutta stage update followed by slope limiting and wetting/drying.
+ * Readings of everything the paper leaves open: DESIGN.md section 3.
+ *
+ * Conventions
+ *   - every pointer argument is HOST memory owned by the caller; it is copied in or out during
+ *     the call and never retained.  All device memory is owned by the handle.
+ *   - element arrays are [ndof][n_elem] doubles, mode index slow, in the CALLER's element order
+ *     (any internal reordering is invisible); ndof = (p+1)(p+2)/2; mode order 00,01,10,(02,11,20).
+ *   - triangles are counter-clockwise, 0-based; local edge l joins local vertices (l+1)%3 -> (l+2)%3.
+ *   - return value 0 = success; <0 = error (DGSWEM_E_*), text via dgswem_last_error().
+ *   - calls on one handle must not be concurrent.  Work is enqueued on the handle's stream;
+ *     get_* calls synchronise it.
+ */
+#ifndef DGSWEM_H
+#define DGSWEM_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DGSWEM_OK          0
+#define DGSWEM_E_ARG      -1   /* bad argument (NULL, size, parameter range) */
+#define DGSWEM_E_MESH     -2   /* inconsistent mesh tables (orientation, edge/element tables) */
+#define DGSWEM_E_CUDA     -3   /* CUDA runtime error */
+#define DGSWEM_E_NONFINITE -4  /* non-finite state found by dgswem_get_state */
+
+typedef struct dgswem dgswem_t;   /* opaque */
+
+typedef struct {
+  int32_t p;            /* polynomial degree, 1 or 2 (paper runs p=1)              */
+  int32_t rk_order;     /* 2: SSP(2,2), 3: SSP(3,3) (R-2)                */
+  double  g;            /* gravity, e.g. 9.81                                                    */
+  double  cf;           /* quadratic bottom friction coefficient, 0 = off (R-6)        */
+  double  coriolis_f;   /* Coriolis parameter, 0 = off                             */
+  double  h0_dry;       /* dry tolerance H0 > 0; also the depth floor in denominators (R-6, R-8) */
+  int32_t limiter;      /* 0/1: slope limiter after every stage (R-7)              */
+  int32_t wetdry;       /* 0/1: wet/dry pass after every stage (R-8)               */
+  int32_t reorder;      /* 0: keep caller's numbering internally; 1: Hilbert-curve renumbering   */
+  int32_t device;       /* CUDA device ordinal                                                   */
+} dgswem_params;
+
+/* Holland (1980) vortex, R-9: centre (x0+vx t, y0+vy t), radius of max wind rmax [m],
+ * pressure deficit dp [Pa], shape B, densities [kg/m3], Coriolis f used in the gradient wind. */
+typedef struct { double x0, y0, vx, vy, rmax, dp, B, rho_air, rho_water, f; } dgswem_holland;
+
+/* Optional device-memory hooks (the Python binding backs them with torch allocations) and the
+ * CUDA stream (a cudaStream_t cast to void*; NULL = the library creates its own stream). */
+typedef struct {
+  void* (*alloc)(size_t bytes, void* user);   /* returns a device pointer, 256-byte aligned, or NULL */
+  void  (*free)(void* ptr, void* user);
+  void* user;
+  void* stream;
+} dgswem_devhooks;
+
+/* Build a model.  xy[n_nodes][2], bathy[n_nodes] (positive down), tri[n_elem][3],
+ * edge_elem[n_edge][2] = (e+, e-) with e- = -1 on a boundary edge, edge_local[n_edge][2] = local
+ * edge number of e+ / of e- (-1), edge_bc[n_edge] = 0 interior, 1 land/wall, 2 ocean elevation,
+ * elem_edge[n_elem][3] = global edge of local edge l  (the paper's NEDEL / LED / NIEDN tables,
+ * PAPER.md:341-354).  The tables are validated (E_MESH).  hooks may be NULL. */
+int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* hooks,
+                  int64_t n_nodes, const double* xy, const double* bathy,
+                  int64_t n_elem, const int32_t* tri,
+                  int64_t n_edge, const int32_t* edge_elem, const int8_t* edge_local,
+                  const int32_t* edge_bc, const int32_t* elem_edge);
+
+/* Load the modal state at time t.  If wetdry is on, one wet/dry pass is applied (it initialises
+ * the wet mask and may modify the state); otherwise every element is flagged wet. */
+int dgswem_set_state(dgswem_t*, double t, const double* ze, const double* qx, const double* qy);
+
+/* Ocean-boundary elevation zeta_b(t) = amp sin(omega t + phase) on edge_bc == 2 edges (R-4). */
+int dgswem_set_tide(dgswem_t*, double amp, double omega, double phase);
+
+/* Moving Holland vortex wind stress (R-9); NULL switches the wind off. */
+int dgswem_set_wind_holland(dgswem_t*, const dgswem_holland*);
+
+/* Advance nsteps time steps of size dt: per step WIND at the nodes, then per
+ * stage EDGE -> GATHER+AREA+RK update -> limiter -> wet/dry.  Asynchronous on the stream. */
+int dgswem_step(dgswem_t*, int64_t nsteps, double dt);
+
+/* TEST HOOK: L_h(current state) (eq. (5)) at the current time, each [ndof][n_elem]. */
+int dgswem_eval_rhs(dgswem_t*, double* rze, double* rqx, double* rqy);
+
+/* TEST HOOK: per-edge numerical flux buffer [3][nq_e][n_edge] of the last RHS evaluation
+ * (caller's edge order; point j numbered along e+'s local edge). */
+int dgswem_get_flux(dgswem_t*, double* flux);
+
+/* Copy the state (and time, if t != NULL) back; synchronises; E_NONFINITE if any value is not finite. */
+int dgswem_get_state(dgswem_t*, double* t, double* ze, double* qx, double* qy);
+
+/* Wet (1) / dry (0) flag per element, caller's order. */
+int dgswem_get_wetdry(dgswem_t*, uint8_t* wet);
+
+/* Nodal kinematic wind stress tau_s/rho_0 of the last WIND evaluation, [2][n_nodes] (test hook). */
+int dgswem_get_wind(dgswem_t*, double* tau);
+
+/* Number of kernels launched by this handle so far (for bench.py's gpu_launches). */
+int64_t dgswem_launch_count(const dgswem_t*);
+
+/* Per-kernel timing for bench.py's roofline: while enabled, every kernel launch of dgswem_step /
+ * dgswem_eval_rhs is bracketed by CUDA events recorded on the handle's stream (at most 32768
+ * launches are recorded between reads).  dgswem_profile_read synchronises, returns the summed
+ * device time in milliseconds and the launch count per kernel kind
+ * (0 WIND, 1 EDGE, 2 ELEMENT = GATHER+AREA+RK(+wet/dry), 3 LIMITER+WETDRY; arrays of 4) and clears the records. */
+int dgswem_profile(dgswem_t*, int enable);
+int dgswem_profile_read(dgswem_t*, double* ms, int64_t* count);
+
+/* Block until all enqueued work is done. */
+int dgswem_sync(dgswem_t*);
+
+const char* dgswem_last_error(const dgswem_t*);   /* valid until the next call on the handle; NULL handle: creation error */
+void dgswem_destroy(dgswem_t*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,242 @@
+"""ctypes binding of libdgswem.so (include/dgswem.h) -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; this module converts numpy
+arrays to pointers, backs the library's device allocations with torch tensors and hands it torch's
+current CUDA stream.  There is no CPU fallback: a missing library or device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+PKG = Path(__file__).resolve().parent
+LIB_PATH = PKG / "libdgswem.so"
+
+E_NONFINITE = -4
+
+
+class Params(C.Structure):
+    _fields_ = [("p", C.c_int32), ("rk_order", C.c_int32), ("g", C.c_double), ("cf", C.c_double),
+                ("coriolis_f", C.c_double), ("h0_dry", C.c_double), ("limiter", C.c_int32), ("wetdry", C.c_int32),
+                ("reorder", C.c_int32), ("device", C.c_int32)]
+
+
+class Holland(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("x0", "y0", "vx", "vy", "rmax", "dp", "B", "rho_air", "rho_water", "f")]
+
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class DevHooks(C.Structure):
+    _fields_ = [("alloc", ALLOC_FN), ("free", FREE_FN), ("user", C.c_void_p), ("stream", C.c_void_p)]
+
+
+class DgswemError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"dgswem error {code}: {msg}")
+        self.code = code
+
+
+EXPORTS = ["dgswem_create", "dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_step",
+           "dgswem_eval_rhs", "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_wind",
+           "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree library (fails loudly if it has not been built)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2508_21208_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(str(LIB_PATH))
+    D, I64, VP = C.c_double, C.c_int64, C.c_void_p
+    PD, PI32 = C.POINTER(C.c_double), C.POINTER(C.c_int32)
+    L.dgswem_create.argtypes = [C.POINTER(VP), C.POINTER(Params), C.POINTER(DevHooks), I64, PD, PD, I64, PI32, I64, PI32,
+                                C.POINTER(C.c_int8), PI32, PI32]
+    L.dgswem_create.restype = C.c_int
+    L.dgswem_set_state.argtypes = [VP, D, PD, PD, PD]
+    L.dgswem_set_tide.argtypes = [VP, D, D, D]
+    L.dgswem_set_wind_holland.argtypes = [VP, C.POINTER(Holland)]
+    L.dgswem_step.argtypes = [VP, I64, D]
+    L.dgswem_eval_rhs.argtypes = [VP, PD, PD, PD]
+    L.dgswem_get_flux.argtypes = [VP, PD]
+    L.dgswem_get_state.argtypes = [VP, PD, PD, PD, PD]
+    L.dgswem_get_wetdry.argtypes = [VP, C.POINTER(C.c_uint8)]
+    L.dgswem_get_wind.argtypes = [VP, PD]
+    L.dgswem_launch_count.argtypes = [VP]; L.dgswem_launch_count.restype = I64
+    L.dgswem_profile.argtypes = [VP, C.c_int]; L.dgswem_profile.restype = C.c_int
+    L.dgswem_profile_read.argtypes = [VP, PD, C.POINTER(I64)]; L.dgswem_profile_read.restype = C.c_int
+    L.dgswem_sync.argtypes = [VP]
+    L.dgswem_last_error.argtypes = [VP]; L.dgswem_last_error.restype = C.c_char_p
+    L.dgswem_destroy.argtypes = [VP]; L.dgswem_destroy.restype = None
+    for name in ("dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_step", "dgswem_eval_rhs",
+                 "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_wind", "dgswem_sync"):
+        getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+class Dgswem:
+    """One model on one GPU.  Method names mirror the C ABI (dgswem_<name>)."""
+
+    def __init__(self, params: dict, xy, bathy, tri, edge_elem, edge_local, edge_bc, elem_edge, *,
+                 reorder: int = 1, device: int = 0, use_torch_alloc: bool = True):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2508_21208_b200 needs a CUDA device (there is no CPU fallback)")
+        L = load_library()
+        self.L = L
+        self.p = int(params["p"])
+        self.ndof = (self.p + 1) * (self.p + 2) // 2
+        self.nqe = self.p + 1
+        self.n_stage = int(params["rk_order"])
+        xy = np.ascontiguousarray(xy, dtype=np.float64)
+        bathy = np.ascontiguousarray(bathy, dtype=np.float64)
+        tri = np.ascontiguousarray(tri, dtype=np.int32)
+        edge_elem = np.ascontiguousarray(edge_elem, dtype=np.int32)
+        edge_local = np.ascontiguousarray(edge_local, dtype=np.int8)
+        edge_bc = np.ascontiguousarray(edge_bc, dtype=np.int32)
+        elem_edge = np.ascontiguousarray(elem_edge, dtype=np.int32)
+        self.n_nodes, self.n_elem, self.n_edge = xy.shape[0], tri.shape[0], edge_elem.shape[0]
+        assert xy.shape == (self.n_nodes, 2) and bathy.shape == (self.n_nodes,) and tri.shape == (self.n_elem, 3)
+        assert edge_elem.shape == (self.n_edge, 2) and edge_local.shape == (self.n_edge, 2)
+        assert edge_bc.shape == (self.n_edge,) and elem_edge.shape == (self.n_elem, 3)
+        prm = Params(p=self.p, rk_order=self.n_stage, g=params["g"], cf=params["cf"], coriolis_f=params["coriolis_f"],
+                     h0_dry=params["h0_dry"], limiter=int(params["limiter"]), wetdry=int(params["wetdry"]),
+                     reorder=int(reorder), device=int(device))
+        self.device = torch.device("cuda", device)
+        self._tensors = {}
+        hooks = None
+        if use_torch_alloc:
+            def _alloc(nbytes, _user):
+                try:
+                    t = torch.empty(int(nbytes), dtype=torch.uint8, device=self.device)
+                except Exception:
+                    return None
+                self._tensors[t.data_ptr()] = t
+                return t.data_ptr()
+
+            def _free(ptr, _user):
+                self._tensors.pop(ptr, None)
+
+            self._alloc_cb, self._free_cb = ALLOC_FN(_alloc), FREE_FN(_free)   # keep the callbacks alive
+            with torch.cuda.device(self.device):
+                stream = torch.cuda.current_stream().cuda_stream
+            hooks = DevHooks(self._alloc_cb, self._free_cb, None, C.c_void_p(stream))
+        self.h = C.c_void_p()
+        i32 = lambda a: a.ctypes.data_as(C.POINTER(C.c_int32))
+        rc = L.dgswem_create(C.byref(self.h), C.byref(prm), C.byref(hooks) if hooks is not None else None,
+                             self.n_nodes, _dp(xy), _dp(bathy), self.n_elem, i32(tri), self.n_edge, i32(edge_elem),
+                             edge_local.ctypes.data_as(C.POINTER(C.c_int8)), i32(edge_bc), i32(elem_edge))
+        if rc != 0:
+            msg = L.dgswem_last_error(None)
+            self.h = None
+            raise DgswemError(rc, msg.decode() if msg else "?")
+
+    @classmethod
+    def from_workload(cls, w, **kw):
+        m = w.mesh
+        o = cls(w.params, m.xy, w.bathy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, **kw)
+        if w.tide is not None:
+            o.set_tide(*w.tide)
+        if w.holland is not None:
+            o.set_wind_holland(w.holland)
+        o.set_state(0.0, w.ze, w.qx, w.qy)
+        return o
+
+    # ------------------------------------------------------------------
+    def _check(self, rc):
+        if rc != 0:
+            msg = self.L.dgswem_last_error(self.h)
+            raise DgswemError(rc, msg.decode() if msg else "?")
+
+    def _st(self, a):
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        if a.shape != (self.ndof, self.n_elem):
+            raise ValueError(f"state array must be [{self.ndof}, {self.n_elem}], got {a.shape}")
+        return a
+
+    def set_state(self, t, ze, qx, qy):
+        ze, qx, qy = self._st(ze), self._st(qx), self._st(qy)
+        self._check(self.L.dgswem_set_state(self.h, float(t), _dp(ze), _dp(qx), _dp(qy)))
+
+    def set_tide(self, amp, omega, phase):
+        self._check(self.L.dgswem_set_tide(self.h, float(amp), float(omega), float(phase)))
+
+    def set_wind_holland(self, hol: dict | None):
+        if hol is None:
+            self._check(self.L.dgswem_set_wind_holland(self.h, None))
+        else:
+            self._check(self.L.dgswem_set_wind_holland(self.h, C.byref(Holland(**hol))))
+
+    def step(self, nsteps, dt):
+        self._check(self.L.dgswem_step(self.h, int(nsteps), float(dt)))
+
+    def eval_rhs(self):
+        r = [np.empty((self.ndof, self.n_elem)) for _ in range(3)]
+        self._check(self.L.dgswem_eval_rhs(self.h, *[_dp(a) for a in r]))
+        return r
+
+    def get_flux(self):
+        f = np.empty((3, self.nqe, self.n_edge))
+        self._check(self.L.dgswem_get_flux(self.h, _dp(f)))
+        return f
+
+    def get_state(self, out=None):
+        if out is None:
+            out = [np.empty((self.ndof, self.n_elem)) for _ in range(3)]
+        t = C.c_double()
+        self._check(self.L.dgswem_get_state(self.h, C.byref(t), *[_dp(a) for a in out]))
+        return (t.value, *out)
+
+    def get_wetdry(self):
+        wet = np.empty(self.n_elem, dtype=np.uint8)
+        self._check(self.L.dgswem_get_wetdry(self.h, wet.ctypes.data_as(C.POINTER(C.c_uint8))))
+        return wet
+
+    def get_wind(self):
+        tau = np.empty((2, self.n_nodes))
+        self._check(self.L.dgswem_get_wind(self.h, _dp(tau)))
+        return tau
+
+    def launch_count(self) -> int:
+        return int(self.L.dgswem_launch_count(self.h))
+
+    KERNEL_KINDS = ("wind", "edge", "elem", "limwd")
+
+    def profile(self, enable: bool):
+        self._check(self.L.dgswem_profile(self.h, int(bool(enable))))
+
+    def profile_read(self) -> dict:
+        """{kind: (total_ms, launches)} since the last read."""
+        ms = (C.c_double * 4)()
+        cnt = (C.c_int64 * 4)()
+        self._check(self.L.dgswem_profile_read(self.h, ms, cnt))
+        return {k: (ms[i], int(cnt[i])) for i, k in enumerate(self.KERNEL_KINDS)}
+
+    def sync(self):
+        self._check(self.L.dgswem_sync(self.h))
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.dgswem_destroy(self.h)
+            self.h = None
+            self._tensors.clear()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,741 @@
+// dgswem.cu -- host side of the C ABI (include/dgswem.h): handle, validation, element-independent
+// tables, geometry, Hilbert renumbering, device layout and the per-step launch sequence.
+// No torch types here; device memory comes from the hooks (or cudaMalloc), work goes to one stream.
+#include "dgswem.h"
+#include "dgswem_kernels.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <numeric>
+#include <string>
+#include <vector>
+
+using namespace dgk;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+constexpr double kG_edge1 = 0.57735026918962576;   // 1/sqrt(3)
+constexpr double kG_edge2 = 0.77459666924148338;   // sqrt(3/5)
+
+inline long long round_up(long long n, long long m) { return (n + m - 1) / m * m; }
+
+// ------------------------------------------------------------------------------------ tables
+// Dubiner basis (eq. (4)), mode order 00,01,10,02,11,20, from barycentrics.
+void dubiner(double l1, double l2, double* phi, double* g1, double* g2) {
+  const double xi1 = 2.0 * l1 - 1.0;
+  const double xi2 = 2.0 * l2 - 1.0;
+  const double s = 0.5 * (1.0 - xi2);
+  const double r = 0.5 * (5.0 * xi2 + 3.0);
+  phi[0] = 1.0;
+  phi[1] = 0.5 * (3.0 * xi2 + 1.0);
+  phi[2] = xi1 + 0.5 * (1.0 + xi2);
+  phi[3] = 0.5 * (((5.0 * xi2) * xi2 + 2.0 * xi2) - 1.0);
+  phi[4] = phi[2] * r;
+  phi[5] = 0.5 * ((3.0 * phi[2]) * phi[2] - s * s);
+  g1[0] = 0.0;           g2[0] = 0.0;
+  g1[1] = 0.0;           g2[1] = 1.5;
+  g1[2] = 1.0;           g2[2] = 0.5;
+  g1[3] = 0.0;           g2[3] = 5.0 * xi2 + 1.0;
+  g1[4] = r;             g2[4] = 0.5 * r + 2.5 * phi[2];
+  g1[5] = 3.0 * phi[2];  g2[5] = 0.5 * (3.0 * phi[2] + s);
+}
+
+void make_tables(int p, Tables& T) {
+  std::memset(&T, 0, sizeof(T));
+  const int ndof = (p + 1) * (p + 2) / 2, nqe = p + 1, nqa = (p == 1) ? 3 : 6;
+  double ge[3] = {0, 0, 0}, we[3] = {0, 0, 0}, wa[6] = {0, 0, 0, 0, 0, 0};
+  if (p == 1) {
+    ge[0] = -kG_edge1; ge[1] = kG_edge1; we[0] = 1.0; we[1] = 1.0;
+    for (int i = 0; i < 3; ++i) {
+      for (int v = 0; v < 3; ++v) T.la[i][v] = (v == i) ? 2.0 / 3.0 : 1.0 / 6.0;
+      wa[i] = 2.0 / 3.0;
+    }
+  } else {
+    ge[0] = -kG_edge2; ge[1] = 0.0; ge[2] = kG_edge2;
+    we[0] = 5.0 / 9.0; we[1] = 8.0 / 9.0; we[2] = 5.0 / 9.0;
+    const double a1 = 0.445948490915965, w1 = 0.223381589678011;
+    const double a2 = 0.091576213509771, w2 = 0.109951743655322;
+    for (int i = 0; i < 3; ++i) {
+      for (int v = 0; v < 3; ++v) {
+        T.la[i][v] = (v == i) ? 1.0 - 2.0 * a1 : a1;
+        T.la[3 + i][v] = (v == i) ? 1.0 - 2.0 * a2 : a2;
+      }
+      wa[i] = 2.0 * w1;
+      wa[3 + i] = 2.0 * w2;
+    }
+  }
+  const double mass[6] = {2.0, 1.0, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 9.0, 2.0 / 15.0};
+  double invM[6];
+  for (int k = 0; k < 6; ++k) invM[k] = 1.0 / mass[k];
+  double phi[6], g1[6], g2[6];
+  for (int i = 0; i < nqa; ++i) {
+    dubiner(T.la[i][1], T.la[i][2], phi, g1, g2);
+    for (int k = 0; k < ndof; ++k) {
+      T.phiA[i][k] = phi[k]; T.dA1[i][k] = g1[k]; T.dA2[i][k] = g2[k];
+      T.wfac[i][k] = wa[i] * invM[k];
+      T.srfac[i][k] = T.wfac[i][k] * phi[k];
+    }
+  }
+  for (int j = 0; j < nqe; ++j) {
+    T.elam[j][0] = 0.5 * (1.0 - ge[j]);
+    T.elam[j][1] = 0.5 * (1.0 + ge[j]);
+  }
+  for (int l = 0; l < 3; ++l) {
+    const int va = (l + 1) % 3, vb = (l + 2) % 3;
+    for (int j = 0; j < nqe; ++j) {
+      double lam[3] = {0.0, 0.0, 0.0};
+      lam[va] = T.elam[j][0]; lam[vb] = T.elam[j][1];
+      dubiner(lam[1], lam[2], phi, g1, g2);
+      for (int k = 0; k < ndof; ++k) {
+        T.phiE[l][j][k] = phi[k];
+        T.efac[l][j][k] = (we[j] * invM[k]) * phi[k];
+      }
+    }
+  }
+  for (int v = 0; v < 3; ++v) {
+    double lam[3] = {0.0, 0.0, 0.0};
+    lam[v] = 1.0;
+    dubiner(lam[1], lam[2], phi, g1, g2);
+    for (int k = 0; k < ndof; ++k) T.phiV[v][k] = phi[k];
+  }
+}
+
+// ------------------------------------------------------------------------------------ Hilbert
+// index of (x, y) in [0, 2^16)^2 along the Hilbert curve
+inline uint32_t hilbert_d(uint32_t x, uint32_t y) {
+  const uint32_t n = 1u << 16;
+  uint32_t d = 0;
+  for (uint32_t s = n >> 1; s > 0; s >>= 1) {
+    const uint32_t rx = (x & s) ? 1u : 0u, ry = (y & s) ? 1u : 0u;
+    d += s * s * ((3u * rx) ^ ry);
+    if (ry == 0) {   // rotate / flip the quadrant
+      if (rx == 1) { x = (n - 1u) - x; y = (n - 1u) - y; }
+      const uint32_t t = x; x = y; y = t;
+    }
+  }
+  return d;
+}
+
+std::vector<int> hilbert_order(const std::vector<double>& px, const std::vector<double>& py) {
+  const size_t n = px.size();
+  double x0 = 1e300, x1 = -1e300, y0 = 1e300, y1 = -1e300;
+  for (size_t i = 0; i < n; ++i) {
+    x0 = std::min(x0, px[i]); x1 = std::max(x1, px[i]);
+    y0 = std::min(y0, py[i]); y1 = std::max(y1, py[i]);
+  }
+  const double span = std::max(std::max(x1 - x0, y1 - y0), 1e-300);
+  std::vector<uint64_t> key(n);
+  for (size_t i = 0; i < n; ++i) {
+    const uint32_t ix = (uint32_t)std::min(65535.0, (px[i] - x0) / span * 65535.0);
+    const uint32_t iy = (uint32_t)std::min(65535.0, (py[i] - y0) / span * 65535.0);
+    key[i] = ((uint64_t)hilbert_d(ix, iy) << 32) | (uint64_t)i;
+  }
+  std::sort(key.begin(), key.end());
+  std::vector<int> order(n);
+  for (size_t i = 0; i < n; ++i) order[i] = (int)(key[i] & 0xffffffffu);
+  return order;   // order[new] = old
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------ handle
+struct dgswem {
+  dgswem_params prm{};
+  int ndof = 0, nqe = 0, nqa = 0, nstage = 0;
+  long long nn = 0, ne = 0, nd = 0, ld = 0, ldd = 0, ldn = 0;
+  cudaStream_t stream = nullptr;
+  bool own_stream = false;
+  dgswem_devhooks hooks{};
+  bool have_hooks = false;
+  std::vector<void*> allocs;
+  std::string err;
+  long long launches = 0;
+
+  // optional per-kernel timing (dgswem_profile): CUDA events recorded on the stream around every launch
+  struct ProfRec { int kind; cudaEvent_t a, b; };
+  bool profiling = false;
+  std::vector<ProfRec> prof;
+  cudaEvent_t prof_start = nullptr;
+
+  // device
+  double* W[3] = {nullptr, nullptr, nullptr};
+  double *flux = nullptr, *mean = nullptr, *jinv = nullptr, *lfac = nullptr, *hv = nullptr;
+  double *en = nullptr, *ehb = nullptr, *tau = nullptr, *nxy = nullptr, *stage_buf = nullptr;
+  int2* edge_elem = nullptr;
+  int *einfo = nullptr, *elem_edge = nullptr, *nbr = nullptr, *tri = nullptr;
+  int *perm_e = nullptr, *inv_e = nullptr, *inv_d = nullptr;   // perm_e[new]=old, inv_e[old]=new, inv_d[old]=new
+  unsigned char *wet = nullptr, *wet_stage = nullptr;
+  int* flag = nullptr;
+  size_t stage_bytes = 0;
+
+  double t = 0.0;
+  double tide_amp = 0.0, tide_omega = 0.0, tide_phase = 0.0;
+  bool wind_on = false;
+  dgswem_holland hol{};
+
+  int fail(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof(buf), fmt, ap); va_end(ap);
+    err = buf;
+    return code;
+  }
+  int cuda_fail(cudaError_t e, const char* what) { return fail(DGSWEM_E_CUDA, "%s: %s", what, cudaGetErrorString(e)); }
+
+  void* dalloc(size_t bytes) {
+    void* p = nullptr;
+    if (bytes == 0) bytes = 256;
+    if (have_hooks) {
+      p = hooks.alloc(bytes, hooks.user);
+    } else if (cudaMalloc(&p, bytes) != cudaSuccess) {
+      p = nullptr;
+    }
+    if (p) allocs.push_back(p);
+    return p;
+  }
+  void release_all() {
+    for (void* p : allocs) {
+      if (have_hooks) hooks.free(p, hooks.user); else cudaFree(p);
+    }
+    allocs.clear();
+  }
+};
+
+#define CK(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return h->cuda_fail(e__, #call); } while (0)
+#define CKL(name) do { cudaError_t e__ = cudaGetLastError(); if (e__ != cudaSuccess) return h->cuda_fail(e__, name); h->launches++; } while (0)
+
+enum ProfKind { PK_WIND = 0, PK_EDGE = 1, PK_ELEM = 2, PK_LIMWD = 3, PK_COUNT = 4 };
+constexpr size_t kMaxProfRecords = 1 << 15;
+static inline void prof_begin(dgswem* h, int kind) {
+  if (!h->profiling || h->prof.size() >= kMaxProfRecords) return;
+  dgswem::ProfRec r; r.kind = kind; r.a = nullptr; r.b = nullptr;
+  if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) return;
+  cudaEventRecord(r.a, h->stream);
+  h->prof.push_back(r);
+  h->prof_start = r.a;
+}
+static inline void prof_end(dgswem* h) {
+  if (!h->profiling || h->prof_start == nullptr) return;
+  cudaEventRecord(h->prof.back().b, h->stream);
+  h->prof_start = nullptr;
+}
+
+namespace {
+
+template <typename T>
+int upload(dgswem* h, T*& dptr, const std::vector<T>& host) {
+  dptr = (T*)h->dalloc(host.size() * sizeof(T));
+  if (!dptr) return h->fail(DGSWEM_E_CUDA, "device allocation of %zu bytes failed", host.size() * sizeof(T));
+  CK(cudaMemcpyAsync(dptr, host.data(), host.size() * sizeof(T), cudaMemcpyHostToDevice, h->stream));
+  CK(cudaStreamSynchronize(h->stream));   // host vector may die after return
+  return 0;
+}
+
+inline int grid_for(long long n, int block) { return (int)((n + block - 1) / block); }
+
+int validate_mesh(dgswem* h, long long nn, const double* xy, long long ne, const int32_t* tri, long long nd,
+                  const int32_t* edge_elem, const int8_t* edge_local, const int32_t* edge_bc, const int32_t* elem_edge) {
+  for (long long e = 0; e < ne; ++e) {
+    for (int v = 0; v < 3; ++v)
+      if (tri[3 * e + v] < 0 || tri[3 * e + v] >= nn) return h->fail(DGSWEM_E_MESH, "element %lld: node id out of range", e);
+    const double* a = xy + 2 * (long long)tri[3 * e], *b = xy + 2 * (long long)tri[3 * e + 1], *c = xy + 2 * (long long)tri[3 * e + 2];
+    const double A2 = (b[0] - a[0]) * (c[1] - a[1]) - (c[0] - a[0]) * (b[1] - a[1]);
+    if (!(A2 > 0.0)) return h->fail(DGSWEM_E_MESH, "element %lld is not counter-clockwise (or degenerate)", e);
+    for (int l = 0; l < 3; ++l) {
+      const long long d = elem_edge[3 * e + l];
+      if (d < 0 || d >= nd) return h->fail(DGSWEM_E_MESH, "elem_edge[%lld][%d] out of range", e, l);
+      const bool plus = edge_elem[2 * d] == e && edge_local[2 * d] == l;
+      const bool minus = edge_elem[2 * d + 1] == e && edge_local[2 * d + 1] == l;
+      if (plus == minus) return h->fail(DGSWEM_E_MESH, "elem_edge[%lld][%d]=%lld does not point back to the element", e, l, d);
+    }
+  }
+  for (long long d = 0; d < nd; ++d) {
+    const long long ep = edge_elem[2 * d], em = edge_elem[2 * d + 1];
+    const int lp = edge_local[2 * d], lm = edge_local[2 * d + 1];
+    const int bc = edge_bc[d];
+    if (ep < 0 || ep >= ne || lp < 0 || lp > 2) return h->fail(DGSWEM_E_MESH, "edge %lld: bad e+ / local edge", d);
+    if (elem_edge[3 * ep + lp] != d) return h->fail(DGSWEM_E_MESH, "edge %lld: e+ does not list it", d);
+    if (em >= 0) {
+      if (em >= ne || lm < 0 || lm > 2 || em == ep) return h->fail(DGSWEM_E_MESH, "edge %lld: bad e- / local edge", d);
+      if (elem_edge[3 * em + lm] != d) return h->fail(DGSWEM_E_MESH, "edge %lld: e- does not list it", d);
+      if (bc != 0) return h->fail(DGSWEM_E_MESH, "edge %lld: interior edge with boundary code %d", d, bc);
+      // the two sides must share the same two nodes, traversed in opposite directions
+      const int a1 = tri[3 * ep + (lp + 1) % 3], b1 = tri[3 * ep + (lp + 2) % 3];
+      const int a2 = tri[3 * em + (lm + 1) % 3], b2 = tri[3 * em + (lm + 2) % 3];
+      if (a1 != b2 || b1 != a2) return h->fail(DGSWEM_E_MESH, "edge %lld: the two sides do not share the same nodes", d);
+    } else {
+      if (bc != 1 && bc != 2) return h->fail(DGSWEM_E_MESH, "edge %lld: boundary edge needs code 1 or 2, got %d", d, bc);
+    }
+  }
+  return 0;
+}
+
+template <int P>
+int launch_edge(dgswem* h, const double* w, double zeta_b) {
+  EdgeArgs a;
+  a.w = w; a.edge_elem = h->edge_elem; a.einfo = h->einfo; a.en = h->en; a.ehb = h->ehb; a.flux = h->flux;
+  a.nd = (int)h->nd; a.ld = h->ld; a.ldd = h->ldd;
+  a.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
+  a.zeta_b = zeta_b;
+  prof_begin(h, PK_EDGE);
+  k_edge<P><<<grid_for(h->nd, 256), 256, 0, h->stream>>>(a);
+  prof_end(h);
+  CKL("k_edge");
+  return 0;
+}
+
+template <int P, int MODE>
+int launch_elem(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b,
+                int first, bool fuse_wd, bool write_mean) {
+  ElemArgs A;
+  A.win = win; A.w0 = w0; A.wout = wout; A.flux = h->flux; A.elem_edge = h->elem_edge; A.jinv = h->jinv;
+  A.lfac = h->lfac; A.hv = h->hv; A.tri = h->tri; A.tau = h->tau; A.wet = h->wet;
+  A.mean = write_mean ? h->mean : nullptr;
+  A.ne = (int)h->ne; A.ld = h->ld; A.ldd = h->ldd; A.ldn = h->ldn;
+  A.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
+  A.dt = dt; A.a = a; A.b = b; A.first_stage = first; A.wind = h->wind_on ? 1 : 0; A.fuse_wetdry = fuse_wd ? 1 : 0;
+  prof_begin(h, PK_ELEM);
+  k_elem<P, MODE><<<grid_for(h->ne, 128), 128, 0, h->stream>>>(A);
+  prof_end(h);
+  CKL("k_elem");
+  return 0;
+}
+
+template <int P>
+int launch_limwd(dgswem* h, double* w) {
+  LimArgs A;
+  A.w = w; A.mean = h->mean; A.nbr = h->nbr; A.hv = h->hv; A.wet = h->wet; A.ne = (int)h->ne; A.ld = h->ld;
+  A.h0 = h->prm.h0_dry; A.limiter = h->prm.limiter; A.wetdry = h->prm.wetdry;
+  prof_begin(h, PK_LIMWD);
+  k_limwd<P><<<grid_for(h->ne, 128), 128, 0, h->stream>>>(A);
+  prof_end(h);
+  CKL("k_limwd");
+  return 0;
+}
+
+int launch_wind(dgswem* h, double t) {
+  WindArgs A;
+  A.nxy = h->nxy; A.tau = h->tau; A.nn = (int)h->nn; A.ldn = h->ldn;
+  A.cx = h->hol.x0 + h->hol.vx * t; A.cy = h->hol.y0 + h->hol.vy * t;
+  A.rmax = h->hol.rmax; A.dp = h->hol.dp; A.B = h->hol.B; A.rho_air = h->hol.rho_air; A.rho_water = h->hol.rho_water;
+  A.f = h->hol.f;
+  prof_begin(h, PK_WIND);
+  k_wind<<<grid_for(h->nn, 256), 256, 0, h->stream>>>(A);
+  prof_end(h);
+  CKL("k_wind");
+  return 0;
+}
+
+double tide_value(const dgswem* h, double t) {
+  if (h->tide_amp == 0.0) return 0.0;
+  return h->tide_amp * std::sin(h->tide_omega * t + h->tide_phase);
+}
+
+// one RK stage: EDGE -> GATHER+AREA+RK(+wet/dry) -> (limiter, wet/dry)
+template <int P>
+int run_stage(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b, int first,
+              double t_stage) {
+  int rc = launch_edge<P>(h, win, tide_value(h, t_stage));
+  if (rc) return rc;
+  const bool lim = h->prm.limiter != 0;
+  const bool wd = h->prm.wetdry != 0;
+  rc = launch_elem<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim);
+  if (rc) return rc;
+  if (lim) rc = launch_limwd<P>(h, wout);
+  return rc;
+}
+
+template <int P>
+int run_steps(dgswem* h, long long nsteps, double dt) {
+  // Shu-Osher SSP(2,2) / SSP(3,3) (R-2)
+  static const double A2[2] = {0.0, 0.5}, B2[2] = {1.0, 0.5}, C2[2] = {0.0, 1.0};
+  static const double A3[3] = {0.0, 0.75, 1.0 / 3.0}, B3[3] = {1.0, 0.25, 2.0 / 3.0}, C3[3] = {0.0, 1.0, 0.5};
+  const bool rk3 = h->prm.rk_order == 3;
+  const double* a = rk3 ? A3 : A2; const double* b = rk3 ? B3 : B2; const double* c = rk3 ? C3 : C2;
+  for (long long n = 0; n < nsteps; ++n) {
+    if (h->wind_on) { int rc = launch_wind(h, h->t); if (rc) return rc; }
+    // current state lives in W[0]; RK2: W0 -> W1 -> W0 ; RK3: W0 -> W1 -> W2 -> W0
+    int rc = run_stage<P>(h, h->W[0], h->W[0], h->W[1], dt, a[0], b[0], 1, h->t + c[0] * dt);
+    if (rc) return rc;
+    if (!rk3) {
+      rc = run_stage<P>(h, h->W[1], h->W[0], h->W[0], dt, a[1], b[1], 0, h->t + c[1] * dt);
+      if (rc) return rc;
+    } else {
+      rc = run_stage<P>(h, h->W[1], h->W[0], h->W[2], dt, a[1], b[1], 0, h->t + c[1] * dt);
+      if (rc) return rc;
+      rc = run_stage<P>(h, h->W[2], h->W[0], h->W[0], dt, a[2], b[2], 0, h->t + c[2] * dt);
+      if (rc) return rc;
+    }
+    h->t = h->t + dt;
+  }
+  return 0;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------ C ABI
+extern "C" {
+
+const char* dgswem_last_error(const dgswem_t* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+void dgswem_destroy(dgswem_t* h) {
+  if (!h) return;
+  cudaSetDevice(h->prm.device);
+  if (h->stream) cudaStreamSynchronize(h->stream);
+  for (auto& r : h->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+  h->prof.clear();
+  h->release_all();
+  if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
+  delete h;
+}
+
+int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* hooks, int64_t n_nodes,
+                  const double* xy, const double* bathy, int64_t n_elem, const int32_t* tri, int64_t n_edge,
+                  const int32_t* edge_elem, const int8_t* edge_local, const int32_t* edge_bc, const int32_t* elem_edge) {
+  if (!out) { g_create_error = "out is NULL"; return DGSWEM_E_ARG; }
+  *out = nullptr;
+  dgswem* h = new dgswem();
+  auto bail = [&](int code) { g_create_error = h->err; dgswem_destroy(h); return code; };
+  if (!prm || !xy || !bathy || !tri || !edge_elem || !edge_local || !edge_bc || !elem_edge)
+    return bail(h->fail(DGSWEM_E_ARG, "NULL argument"));
+  if (n_nodes < 3 || n_elem < 1 || n_edge < 3 || n_elem > 0x3fffffff || n_edge > 0x7ffffff0 || n_nodes > 0x7ffffff0)
+    return bail(h->fail(DGSWEM_E_ARG, "bad sizes"));
+  if ((prm->p != 1 && prm->p != 2) || (prm->rk_order != 2 && prm->rk_order != 3))
+    return bail(h->fail(DGSWEM_E_ARG, "p must be 1 or 2, rk_order 2 or 3"));
+  if (!(prm->h0_dry > 0.0) || !(prm->g > 0.0) || prm->cf < 0.0)
+    return bail(h->fail(DGSWEM_E_ARG, "need h0_dry > 0, g > 0, cf >= 0"));
+  h->prm = *prm;
+  h->ndof = (prm->p + 1) * (prm->p + 2) / 2; h->nqe = prm->p + 1; h->nqa = prm->p == 1 ? 3 : 6; h->nstage = prm->rk_order;
+  h->nn = n_nodes; h->ne = n_elem; h->nd = n_edge;
+  h->ld = round_up(n_elem, 64); h->ldd = round_up(n_edge, 64); h->ldn = round_up(n_nodes, 64);
+  int rc = validate_mesh(h, n_nodes, xy, n_elem, tri, n_edge, edge_elem, edge_local, edge_bc, elem_edge);
+  if (rc) return bail(rc);
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return bail(h->fail(DGSWEM_E_CUDA, "no CUDA device"));
+  if (prm->device < 0 || prm->device >= ndev) return bail(h->fail(DGSWEM_E_ARG, "device ordinal out of range"));
+  if (cudaSetDevice(prm->device) != cudaSuccess) return bail(h->fail(DGSWEM_E_CUDA, "cudaSetDevice failed"));
+  if (hooks && hooks->alloc && hooks->free) { h->hooks = *hooks; h->have_hooks = true; }
+  if (hooks && hooks->stream) {
+    h->stream = (cudaStream_t)hooks->stream;
+  } else {
+    if (cudaStreamCreateWithFlags(&h->stream, cudaStreamNonBlocking) != cudaSuccess)
+      return bail(h->fail(DGSWEM_E_CUDA, "cudaStreamCreate failed"));
+    h->own_stream = true;
+  }
+
+  auto body = [&]() -> int {
+    // ---- tables to constant memory (both degrees; identical for every handle)
+    Tables T1, T2;
+    make_tables(1, T1); make_tables(2, T2);
+    CK(cudaMemcpyToSymbolAsync(c_tab1, &T1, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaMemcpyToSymbolAsync(c_tab2, &T2, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+
+    const long long ne = h->ne, nd = h->nd, nn = h->nn, ld = h->ld, ldd = h->ldd, ldn = h->ldn;
+    // ---- renumbering (internal only): perm_e[new] = old
+    std::vector<int> perm_e(ne), inv_e(ne), perm_d(nd), inv_d(nd);
+    if (prm->reorder == 1) {
+      std::vector<double> cx(ne), cy(ne);
+      for (long long e = 0; e < ne; ++e) {
+        const int* t = tri + 3 * e;
+        cx[e] = (xy[2 * (long long)t[0]] + xy[2 * (long long)t[1]] + xy[2 * (long long)t[2]]) / 3.0;
+        cy[e] = (xy[2 * (long long)t[0] + 1] + xy[2 * (long long)t[1] + 1] + xy[2 * (long long)t[2] + 1]) / 3.0;
+      }
+      perm_e = hilbert_order(cx, cy);
+      std::vector<double> mx(nd), my(nd);
+      for (long long d = 0; d < nd; ++d) {
+        const long long ep = edge_elem[2 * d]; const int lp = edge_local[2 * d];
+        const long long a = tri[3 * ep + (lp + 1) % 3], b = tri[3 * ep + (lp + 2) % 3];
+        mx[d] = 0.5 * (xy[2 * a] + xy[2 * b]); my[d] = 0.5 * (xy[2 * a + 1] + xy[2 * b + 1]);
+      }
+      perm_d = hilbert_order(mx, my);
+    } else {
+      std::iota(perm_e.begin(), perm_e.end(), 0);
+      std::iota(perm_d.begin(), perm_d.end(), 0);
+    }
+    for (long long i = 0; i < ne; ++i) inv_e[perm_e[i]] = (int)i;
+    for (long long i = 0; i < nd; ++i) inv_d[perm_d[i]] = (int)i;
+
+    // ---- element geometry in internal order (same expression trees as the spec)
+    std::vector<double> jinv(4 * ld, 0.0), lfac(3 * ld, 0.0), hv(3 * ld, 0.0);
+    std::vector<int> ee_packed(3 * ld, 0), nbr(3 * ld, -1), trin(3 * ld, 0);
+    for (long long i = 0; i < ne; ++i) {
+      const long long e = perm_e[i];
+      const int* t = tri + 3 * e;
+      const double x0 = xy[2 * (long long)t[0]], y0 = xy[2 * (long long)t[0] + 1];
+      const double x1 = xy[2 * (long long)t[1]], y1 = xy[2 * (long long)t[1] + 1];
+      const double x2 = xy[2 * (long long)t[2]], y2 = xy[2 * (long long)t[2] + 1];
+      const double dx1 = x1 - x0, dy1 = y1 - y0, dx2 = x2 - x0, dy2 = y2 - y0;
+      const double A = 0.5 * (dx1 * dy2 - dx2 * dy1);
+      const double rA = 1.0 / A;
+      jinv[0 * ld + i] = dy2 * rA;
+      jinv[1 * ld + i] = (-dx2) * rA;
+      jinv[2 * ld + i] = (-dy1) * rA;
+      jinv[3 * ld + i] = dx1 * rA;
+      for (int l = 0; l < 3; ++l) {
+        const long long na = t[(l + 1) % 3], nb = t[(l + 2) % 3];
+        const double ex = xy[2 * nb] - xy[2 * na], ey = xy[2 * nb + 1] - xy[2 * na + 1];
+        const double L = std::sqrt(ex * ex + ey * ey);
+        lfac[l * ld + i] = L * rA;
+        hv[l * ld + i] = bathy[t[l]];
+        trin[l * ld + i] = t[l];
+        const long long d = elem_edge[3 * e + l];
+        const bool plus = edge_elem[2 * d] == e && edge_local[2 * d] == l;
+        ee_packed[l * ld + i] = inv_d[d] | (plus ? 0 : (int)0x80000000);
+        const long long other = plus ? edge_elem[2 * d + 1] : edge_elem[2 * d];
+        nbr[l * ld + i] = other >= 0 ? inv_e[other] : -1;
+      }
+    }
+    // ---- edge geometry in internal order, from the e+ side
+    std::vector<int2> ee(ldd, make_int2(0, -1));
+    std::vector<int> einfo(ldd, 1 << 4);
+    std::vector<double> en(2 * ldd, 0.0), ehb(2 * ldd, 0.0);
+    for (long long i = 0; i < nd; ++i) {
+      const long long d = perm_d[i];
+      const long long ep = edge_elem[2 * d], em = edge_elem[2 * d + 1];
+      const int lp = edge_local[2 * d], lm = em >= 0 ? edge_local[2 * d + 1] : 0;
+      const long long na = tri[3 * ep + (lp + 1) % 3], nb = tri[3 * ep + (lp + 2) % 3];
+      const double ex = xy[2 * nb] - xy[2 * na], ey = xy[2 * nb + 1] - xy[2 * na + 1];
+      const double L = std::sqrt(ex * ex + ey * ey);
+      const double rL = 1.0 / L;
+      en[i] = ey * rL;
+      en[ldd + i] = (-ex) * rL;
+      ehb[i] = bathy[na];
+      ehb[ldd + i] = bathy[nb];
+      ee[i] = make_int2(inv_e[ep], em >= 0 ? inv_e[em] : -1);
+      einfo[i] = lp | (lm << 2) | (edge_bc[d] << 4);
+    }
+    std::vector<double> nxy(2 * ldn, 0.0);
+    for (long long i = 0; i < nn; ++i) { nxy[i] = xy[2 * i]; nxy[ldn + i] = xy[2 * i + 1]; }
+
+    int r;
+    if ((r = upload(h, h->jinv, jinv))) return r;
+    if ((r = upload(h, h->lfac, lfac))) return r;
+    if ((r = upload(h, h->hv, hv))) return r;
+    if ((r = upload(h, h->elem_edge, ee_packed))) return r;
+    if ((r = upload(h, h->nbr, nbr))) return r;
+    if ((r = upload(h, h->tri, trin))) return r;
+    if ((r = upload(h, h->edge_elem, ee))) return r;
+    if ((r = upload(h, h->einfo, einfo))) return r;
+    if ((r = upload(h, h->en, en))) return r;
+    if ((r = upload(h, h->ehb, ehb))) return r;
+    if ((r = upload(h, h->nxy, nxy))) return r;
+    if (prm->reorder == 1) {
+      if ((r = upload(h, h->perm_e, perm_e))) return r;
+      if ((r = upload(h, h->inv_e, inv_e))) return r;
+      if ((r = upload(h, h->inv_d, inv_d))) return r;
+    }
+    const size_t wbytes = (size_t)3 * h->ndof * ld * sizeof(double);
+    for (int i = 0; i < h->nstage; ++i) {
+      h->W[i] = (double*)h->dalloc(wbytes);
+      if (!h->W[i]) return h->fail(DGSWEM_E_CUDA, "device allocation of %zu bytes failed", wbytes);
+      CK(cudaMemsetAsync(h->W[i], 0, wbytes, h->stream));
+    }
+    const size_t fbytes = (size_t)3 * h->nqe * ldd * sizeof(double);
+    h->stage_bytes = std::max(wbytes, fbytes);
+    h->flux = (double*)h->dalloc(fbytes);
+    h->mean = (double*)h->dalloc((size_t)3 * ld * sizeof(double));
+    h->tau = (double*)h->dalloc((size_t)2 * ldn * sizeof(double));
+    h->stage_buf = (double*)h->dalloc(h->stage_bytes);
+    h->wet = (unsigned char*)h->dalloc((size_t)ld);
+    h->wet_stage = (unsigned char*)h->dalloc((size_t)ld);
+    h->flag = (int*)h->dalloc(256);
+    if (!h->flux || !h->mean || !h->tau || !h->stage_buf || !h->wet || !h->wet_stage || !h->flag)
+      return h->fail(DGSWEM_E_CUDA, "device allocation failed");
+    CK(cudaMemsetAsync(h->flux, 0, fbytes, h->stream));
+    CK(cudaMemsetAsync(h->mean, 0, (size_t)3 * ld * sizeof(double), h->stream));
+    CK(cudaMemsetAsync(h->tau, 0, (size_t)2 * ldn * sizeof(double), h->stream));
+    CK(cudaMemsetAsync(h->wet, 1, (size_t)ld, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+  };
+  rc = body();
+  if (rc) return bail(rc);
+  *out = h;
+  return DGSWEM_OK;
+}
+
+int dgswem_set_state(dgswem_t* h, double t, const double* ze, const double* qx, const double* qy) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!ze || !qx || !qy) return h->fail(DGSWEM_E_ARG, "NULL state pointer");
+  CK(cudaSetDevice(h->prm.device));
+  const double* src[3] = {ze, qx, qy};
+  const size_t row = (size_t)h->ne * sizeof(double);
+  // stage in caller order (rows of length ne, leading dimension ld), then renumber on the device
+  double* stage = h->perm_e ? h->stage_buf : h->W[0];
+  for (int c = 0; c < 3; ++c)
+    CK(cudaMemcpy2DAsync(stage + (size_t)c * h->ndof * h->ld, (size_t)h->ld * sizeof(double), src[c], row, row, h->ndof,
+                         cudaMemcpyHostToDevice, h->stream));
+  if (h->perm_e) {
+    k_gather_rows<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->W[0], h->ld, stage, h->ld, h->perm_e, (int)h->ne, 3 * h->ndof);
+    CKL("k_gather_rows");
+  }
+  k_fill_bytes<<<grid_for(h->ld, 256), 256, 0, h->stream>>>(h->wet, 1, (int)h->ld);
+  CKL("k_fill_bytes");
+  if (h->prm.wetdry) {
+    if (h->prm.p == 1) k_wetdry_only<1><<<grid_for(h->ne, 128), 128, 0, h->stream>>>(h->W[0], h->hv, h->wet, (int)h->ne, h->ld, h->prm.h0_dry);
+    else k_wetdry_only<2><<<grid_for(h->ne, 128), 128, 0, h->stream>>>(h->W[0], h->hv, h->wet, (int)h->ne, h->ld, h->prm.h0_dry);
+    CKL("k_wetdry_only");
+  }
+  CK(cudaStreamSynchronize(h->stream));   // the caller's buffers may be reused after return
+  h->t = t;
+  return DGSWEM_OK;
+}
+
+int dgswem_set_tide(dgswem_t* h, double amp, double omega, double phase) {
+  if (!h) return DGSWEM_E_ARG;
+  h->tide_amp = amp; h->tide_omega = omega; h->tide_phase = phase;
+  return DGSWEM_OK;
+}
+
+int dgswem_set_wind_holland(dgswem_t* h, const dgswem_holland* hol) {
+  if (!h) return DGSWEM_E_ARG;
+  if (hol) {
+    if (!(hol->rmax > 0.0) || !(hol->rho_air > 0.0) || !(hol->rho_water > 0.0) || !(hol->B > 0.0))
+      return h->fail(DGSWEM_E_ARG, "Holland parameters must be positive");
+    h->hol = *hol; h->wind_on = true;
+  } else {
+    h->wind_on = false;
+  }
+  return DGSWEM_OK;
+}
+
+int dgswem_step(dgswem_t* h, int64_t nsteps, double dt) {
+  if (!h) return DGSWEM_E_ARG;
+  if (nsteps < 0 || !(dt > 0.0)) return h->fail(DGSWEM_E_ARG, "need nsteps >= 0 and dt > 0");
+  CK(cudaSetDevice(h->prm.device));
+  return h->prm.p == 1 ? run_steps<1>(h, nsteps, dt) : run_steps<2>(h, nsteps, dt);
+}
+
+int dgswem_eval_rhs(dgswem_t* h, double* rze, double* rqx, double* rqy) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!rze || !rqx || !rqy) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
+  CK(cudaSetDevice(h->prm.device));
+  int rc;
+  if (h->wind_on && (rc = launch_wind(h, h->t))) return rc;
+  double* rbuf = h->W[1];   // scratch: W[1] holds no live data between steps
+  if (h->prm.p == 1) {
+    if ((rc = launch_edge<1>(h, h->W[0], tide_value(h, h->t)))) return rc;
+    if ((rc = launch_elem<1, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, 0.0, 1.0, 1, false, false))) return rc;
+  } else {
+    if ((rc = launch_edge<2>(h, h->W[0], tide_value(h, h->t)))) return rc;
+    if ((rc = launch_elem<2, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, 0.0, 1.0, 1, false, false))) return rc;
+  }
+  const double* src = rbuf;
+  if (h->inv_e) {
+    k_gather_rows<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->stage_buf, h->ld, rbuf, h->ld, h->inv_e, (int)h->ne, 3 * h->ndof);
+    CKL("k_gather_rows");
+    src = h->stage_buf;
+  }
+  double* dst[3] = {rze, rqx, rqy};
+  const size_t row = (size_t)h->ne * sizeof(double);
+  for (int c = 0; c < 3; ++c)
+    CK(cudaMemcpy2DAsync(dst[c], row, src + (size_t)c * h->ndof * h->ld, (size_t)h->ld * sizeof(double), row, h->ndof,
+                         cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return DGSWEM_OK;
+}
+
+int dgswem_get_flux(dgswem_t* h, double* flux) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!flux) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
+  CK(cudaSetDevice(h->prm.device));
+  const double* src = h->flux;
+  if (h->inv_d) {
+    k_gather_rows<<<grid_for(h->nd, 256), 256, 0, h->stream>>>(h->stage_buf, h->ldd, h->flux, h->ldd, h->inv_d, (int)h->nd, 3 * h->nqe);
+    CKL("k_gather_rows");
+    src = h->stage_buf;
+  }
+  const size_t row = (size_t)h->nd * sizeof(double);
+  CK(cudaMemcpy2DAsync(flux, row, src, (size_t)h->ldd * sizeof(double), row, 3 * h->nqe, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return DGSWEM_OK;
+}
+
+int dgswem_get_state(dgswem_t* h, double* t, double* ze, double* qx, double* qy) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!ze || !qx || !qy) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
+  CK(cudaSetDevice(h->prm.device));
+  const double* src = h->W[0];
+  if (h->inv_e) {
+    k_gather_rows<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->stage_buf, h->ld, h->W[0], h->ld, h->inv_e, (int)h->ne, 3 * h->ndof);
+    CKL("k_gather_rows");
+    src = h->stage_buf;
+  }
+  CK(cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream));
+  k_check_finite<<<148 * 8, 256, 0, h->stream>>>(h->W[0], (long long)3 * h->ndof * h->ld, h->flag);
+  CKL("k_check_finite");
+  double* dst[3] = {ze, qx, qy};
+  const size_t row = (size_t)h->ne * sizeof(double);
+  for (int c = 0; c < 3; ++c)
+    CK(cudaMemcpy2DAsync(dst[c], row, src + (size_t)c * h->ndof * h->ld, (size_t)h->ld * sizeof(double), row, h->ndof,
+                         cudaMemcpyDeviceToHost, h->stream));
+  int flag = 0;
+  CK(cudaMemcpyAsync(&flag, h->flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  if (t) *t = h->t;
+  if (flag) return h->fail(DGSWEM_E_NONFINITE, "non-finite value in the state at t=%g", h->t);
+  return DGSWEM_OK;
+}
+
+int dgswem_get_wetdry(dgswem_t* h, uint8_t* wet) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!wet) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
+  CK(cudaSetDevice(h->prm.device));
+  const unsigned char* src = h->wet;
+  if (h->inv_e) {
+    k_gather_bytes<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->wet_stage, h->wet, h->inv_e, (int)h->ne);
+    CKL("k_gather_bytes");
+    src = h->wet_stage;
+  }
+  CK(cudaMemcpyAsync(wet, src, (size_t)h->ne, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return DGSWEM_OK;
+}
+
+int dgswem_get_wind(dgswem_t* h, double* tau) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!tau) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
+  CK(cudaSetDevice(h->prm.device));
+  const size_t row = (size_t)h->nn * sizeof(double);
+  CK(cudaMemcpy2DAsync(tau, row, h->tau, (size_t)h->ldn * sizeof(double), row, 2, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return DGSWEM_OK;
+}
+
+int64_t dgswem_launch_count(const dgswem_t* h) { return h ? h->launches : 0; }
+
+int dgswem_profile(dgswem_t* h, int enable) {
+  if (!h) return DGSWEM_E_ARG;
+  h->profiling = enable != 0;
+  return DGSWEM_OK;
+}
+
+int dgswem_profile_read(dgswem_t* h, double* ms, int64_t* count) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!ms || !count) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
+  CK(cudaSetDevice(h->prm.device));
+  CK(cudaStreamSynchronize(h->stream));
+  for (int k = 0; k < PK_COUNT; ++k) { ms[k] = 0.0; count[k] = 0; }
+  for (auto& r : h->prof) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) { ms[r.kind] += (double)t; count[r.kind]++; }
+    cudaEventDestroy(r.a); cudaEventDestroy(r.b);
+  }
+  h->prof.clear();
+  return DGSWEM_OK;
+}
+
+int dgswem_sync(dgswem_t* h) {
+  if (!h) return DGSWEM_E_ARG;
+  CK(cudaSetDevice(h->prm.device));
+  CK(cudaStreamSynchronize(h->stream));
+  return DGSWEM_OK;
+}
+
+}  // extern "C"
