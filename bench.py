@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py -- fp64 DOF-updates/s per RK stage of the DG-SWEM hot path on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C1|C2p1|C2p2|C4|C5] [--impl ours|reference]
+
+A "step" is one full explicit time step of the workload: WIND (if on) and, per RK stage, EDGE ->
+GATHER+AREA+RK(+wet/dry) -> (limiter+wet/dry), i.e. every row of SURVEY.md section 8(a).  Default
+workload: C3, the largest p=1 mesh (4,494,002 elements; BASELINE.json configs[2], the one the
+north_star quotes the roofline target on).  value = 3*ndof*N_e*n_stage*K / t (DOF-updates/s per RK
+stage), t = CUDA-event time of K steps on the stream the kernels run on, state resident in HBM.
+N > 1: independent replicas of the same workload, one per GPU ("replicas only"), weak
+scaling, max over ranks.  --impl reference times the CPU oracle on the host cores.
+Prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+import numpy as np  # noqa: E402
+
+METRIC = "fp64 DOF-updates/sec per RK stage"
+UNIT = "DOF-updates/s"
+
+
+def make_workload(name: str, scale: float = 1.0):
+    from workloads import c1, c2, c3, c4, c5
+    if name == "C3":
+        nn = max(20, int(round(1500 * scale)))
+        return c3(nn=nn)
+    if name == "C1":
+        return c1()
+    if name == "C2p1":
+        return c2(nq=max(8, int(512 * scale)), p=1)
+    if name == "C2p2":
+        return c2(nq=max(8, int(512 * scale)), p=2)
+    if name == "C4":
+        return c4(nqx=max(16, int(1024 * scale)), nqy=max(8, int(512 * scale)))
+    if name == "C5":
+        return c5(nn=max(20, int(round(1323 * scale))))
+    raise SystemExit(f"unknown workload {name}")
+
+
+# ---------------------------------------------------------------------------------------------
+# algorithmic bytes: what the two-kernel design must move per launch, every
+# array counted once (unique-read assumption: each element's state is read once by EDGE although
+# three edges use it; each flux value once by the element kernel although two elements use it).
+def alg_bytes(w, kind: str, stage_first: bool) -> float:
+    ne, nd = w.mesh.n_elem, w.mesh.n_edge
+    nn = w.mesh.n_nodes
+    ndof, nqe = w.ndof, w.params["p"] + 1
+    lim, wd, wind = w.params["limiter"], w.params["wetdry"], w.holland is not None
+    st = 3 * ndof * 8
+    if kind == "edge":
+        return nd * (8 + 4 + 16 + 16 + 3 * nqe * 8) + ne * st
+    if kind == "elem":
+        b = nd * 3 * nqe * 8 + ne * (st + 12 + 24 + 32 + 24 + 1 + st)
+        if not stage_first:
+            b += ne * st
+        if wd and not lim:
+            b += ne * 1
+        if lim:
+            b += ne * 24
+        if wind:
+            b += ne * 12 + nn * 16
+        return b
+    if kind == "limwd":
+        return ne * (st + 12 + 24 + 24 + 1 + st + 1)
+    if kind == "wind":
+        return nn * 32
+    raise ValueError(kind)
+
+
+def stage_bytes_total(w) -> float:
+    """Algorithmic bytes of one whole time step (all stages)."""
+    tot = alg_bytes(w, "wind", True) if w.holland is not None else 0.0
+    for s in range(w.n_stage):
+        tot += alg_bytes(w, "edge", s == 0) + alg_bytes(w, "elem", s == 0)
+        if w.params["limiter"]:
+            tot += alg_bytes(w, "limwd", s == 0)
+    return tot
+
+
+def load_peaks():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        d = json.loads(f.read_text())
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------
+def run_reference(args, rank: int):
+    """The CPU oracle, as it stands, on the host cores (bench contract: reference arm)."""
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    orc.build()
+    total = args.steps + args.warmup
+    # bounded sample: the full mesh if the run stays within a few minutes, else a smaller mesh of the same recipe
+    est_full = 2.4 * total + 20.0           # s: about 1.2 s per RK stage at 4.5 M elements on 8 cores
+    scale = 1.0 if (args.workload != "C3" or est_full < 150.0) else max(0.1, (150.0 / est_full) ** 0.5)
+    w = make_workload(args.workload, scale)
+    o = orc.Oracle.from_workload(w)
+    o.step(args.warmup, w.dt)
+    t0 = time.perf_counter()
+    o.step(args.steps, w.dt)
+    dt = time.perf_counter() - t0
+    value = w.dofs * w.n_stage * args.steps / dt
+    sample = f"{w.name}: {w.mesh.n_elem} elements, {args.steps} steps after {args.warmup} warm-up"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "n_elem": w.mesh.n_elem, "p": w.params["p"], "rk_order": w.params["rk_order"],
+                       "dt": w.dt, "kind": "CPU oracle (oracle/dgswem_oracle.c, gcc -O2 -ffp-contract=off, OpenMP)"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, rank: int, world: int, local_rank: int):
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    from paper_2508_21208_b200 import build as b
+    if rank == 0:
+        b.build()
+    if world > 1:
+        dist.barrier()
+    import paper_2508_21208_b200 as pk
+    torch.cuda.set_device(local_rank)
+    w = make_workload(args.workload)
+    g = pk.Dgswem.from_workload(w, reorder=args.reorder, device=local_rank)
+    dofs_stage = w.dofs * w.n_stage
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up
+    g.step(max(args.warmup, 3), w.dt)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    # ---- timed region: exactly K steps, device-resident state, CUDA events on the launching stream
+    g.profile(True)
+    g.profile_read()
+    l0 = g.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record(g.stream)
+    g.step(args.steps, w.dt)
+    ev1.record(g.stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = g.launch_count() - l0
+    prof = g.profile_read()
+    g.profile(False)
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        tt = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+    value = world * dofs_stage * args.steps / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers: set_state (H2D) + K steps + get_state/get_wetdry (D2H)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    hin = [pin(w.ze), pin(w.qx), pin(w.qy)]
+    hout = [pin(np.empty_like(w.ze)) for _ in range(3)]
+    g.set_state(0.0, *hin); g.step(1, w.dt); g.get_state(out=hout)      # warm the path
+    barrier()
+    t0 = time.perf_counter()
+    g.set_state(0.0, *hin)
+    g.step(args.steps, w.dt)
+    g.get_state(out=hout)
+    g.get_wetdry()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        tt = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = float(tt.item())
+    state_bytes = 3 * w.ndof * w.mesh.n_elem * 8
+    e2e = {"value": world * dofs_stage * args.steps / e2e_s, "unit": UNIT,
+           "h2d_bytes_per_step": state_bytes / args.steps, "d2h_bytes_per_step": (state_bytes + w.mesh.n_elem) / args.steps,
+           "call": f"dgswem_set_state + dgswem_step({args.steps}) + dgswem_get_state + dgswem_get_wetdry, pinned host buffers, "
+                   f"wall clock; bytes are the per-job copies divided by the {args.steps} steps"}
+    if rank != 0:
+        return
+
+    # ---- roofline of the dominant kernel (per-launch CUDA-event times from inside the timed region)
+    peak, peak_src = load_peaks()
+    per_kind = {}
+    for k, (tms, cnt) in prof.items():
+        if cnt:
+            nfirst = cnt // w.n_stage if k in ("edge", "elem", "limwd") else cnt
+            byts = (alg_bytes(w, k, True) * nfirst + alg_bytes(w, k, False) * (cnt - nfirst)) / cnt
+            per_kind[k] = {"launches": cnt, "avg_ms": tms / cnt, "alg_bytes_per_launch": byts,
+                           "achieved_gbs": byts / (tms / cnt * 1e-3) / 1e9, "share_of_step": tms / ms}
+    dom = max(per_kind, key=lambda k: per_kind[k]["avg_ms"] * per_kind[k]["launches"])
+    d = per_kind[dom]
+    traffic_file = ROOT / "profiles" / "traffic.json"
+    traffic = None
+    if traffic_file.exists():
+        try:
+            traffic = json.loads(traffic_file.read_text()).get(args.workload, {}).get(dom)
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": f"k_{dom}<{w.params['p']}>", "achieved": d["achieved_gbs"], "peak": peak, "unit": "GB/s",
+                "frac": d["achieved_gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
+                "alg_bytes_per_launch": d["alg_bytes_per_launch"], "avg_launch_ms": d["avg_ms"], "kernels": per_kind,
+                "whole_step": {"alg_bytes": stage_bytes_total(w), "achieved_gbs": stage_bytes_total(w) / (ms / args.steps * 1e-3) / 1e9,
+                               "frac_of_measured_peak": stage_bytes_total(w) / (ms / args.steps * 1e-3) / 1e9 / peak,
+                               "frac_of_8TBs_nominal": stage_bytes_total(w) / (ms / args.steps * 1e-3) / 1e9 / 8000.0}}
+
+    # ---- CPU baseline: the oracle on a bounded sample of the same workload, on this box's cores
+    cpu = None
+    if not args.no_cpu:
+        from oracle import oracle as orc
+        orc.build()
+        o = orc.Oracle.from_workload(w)
+        nsamp = max(1, min(args.steps, int(round(12.0 / (w.mesh.n_elem * w.n_stage * 0.28e-6 + 1e-3)))))
+        o.step(1, w.dt)
+        t0 = time.perf_counter()
+        o.step(nsamp, w.dt)
+        cs = time.perf_counter() - t0
+        cpu = {"value": dofs_stage * nsamp / cs, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+               "sample": f"{nsamp} steps of {w.name} (full mesh, {w.mesh.n_elem} elements) after 1 warm-up step, {cs:.1f} s"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": w.name, "n_elem": w.mesh.n_elem, "n_edge": w.mesh.n_edge, "n_nodes": w.mesh.n_nodes,
+                       "p": w.params["p"], "rk_order": w.params["rk_order"], "dt": w.dt, "limiter": w.params["limiter"],
+                       "wetdry": w.params["wetdry"], "wind": w.holland is not None, "tide": w.tide is not None,
+                       "reorder": args.reorder, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                       "l2": f"state {state_bytes / 1e6:.0f} MB per buffer + flux {w.mesh.n_edge * 3 * (w.params['p'] + 1) * 8 / 1e6:.0f} MB "
+                             "per stage exceed the 126 MB L2 (inputs larger than L2, no flush needed)"
+                             if state_bytes > 130e6 else "working set fits L2: a >L2 buffer is NOT flushed between steps; see DESIGN.md"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    g.close()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C3")
+    ap.add_argument("--reorder", type=int, default=1)
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    try:
+        run_ours(args, rank, world, local_rank)
+    finally:
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -118,6 +118,7 @@ class Dgswem:
                      reorder=int(reorder), device=int(device))
         self.device = torch.device("cuda", device)
         self._tensors = {}
+        self.stream = None
         hooks = None
         if use_torch_alloc:
             def _alloc(nbytes, _user):
@@ -132,9 +133,10 @@ class Dgswem:
                 self._tensors.pop(ptr, None)
 
             self._alloc_cb, self._free_cb = ALLOC_FN(_alloc), FREE_FN(_free)   # keep the callbacks alive
-            with torch.cuda.device(self.device):
-                stream = torch.cuda.current_stream().cuda_stream
-            hooks = DevHooks(self._alloc_cb, self._free_cb, None, C.c_void_p(stream))
+            # a dedicated (non-default) torch stream per handle: all kernels and copies of this model run
+            # on it; time it with torch.cuda.Event(...).record(model.stream)
+            self.stream = torch.cuda.Stream(device=self.device)
+            hooks = DevHooks(self._alloc_cb, self._free_cb, None, C.c_void_p(self.stream.cuda_stream))
         self.h = C.c_void_p()
         i32 = lambda a: a.ctypes.data_as(C.POINTER(C.c_int32))
         rc = L.dgswem_create(C.byref(self.h), C.byref(prm), C.byref(hooks) if hooks is not None else None,

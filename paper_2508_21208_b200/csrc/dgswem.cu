@@ -282,7 +282,7 @@ int launch_edge(dgswem* h, const double* w, double zeta_b) {
   a.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
   a.zeta_b = zeta_b;
   prof_begin(h, PK_EDGE);
-  k_edge<P><<<grid_for(h->nd, 256), 256, 0, h->stream>>>(a);
+  k_edge<P><<<grid_for(h->nd, DGK_EDGE_THREADS), DGK_EDGE_THREADS, 0, h->stream>>>(a);
   prof_end(h);
   CKL("k_edge");
   return 0;
@@ -299,7 +299,7 @@ int launch_elem(dgswem* h, const double* win, const double* w0, double* wout, do
   A.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
   A.dt = dt; A.a = a; A.b = b; A.first_stage = first; A.wind = h->wind_on ? 1 : 0; A.fuse_wetdry = fuse_wd ? 1 : 0;
   prof_begin(h, PK_ELEM);
-  k_elem<P, MODE><<<grid_for(h->ne, 128), 128, 0, h->stream>>>(A);
+  k_elem<P, MODE><<<grid_for(h->ne, DGK_ELEM_THREADS), DGK_ELEM_THREADS, 0, h->stream>>>(A);
   prof_end(h);
   CKL("k_elem");
   return 0;
