@@ -261,13 +261,14 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                            "achieved_gbs": byts / (tms / cnt * 1e-3) / 1e9, "share_of_step": tms / ms}
     dom = max(per_kind, key=lambda k: per_kind[k]["avg_ms"] * per_kind[k]["launches"])
     d = per_kind[dom]
-    traffic_file = ROOT / "profiles" / "traffic.json"
+    # DRAM bytes per launch of that kernel from the committed `ncu --set full` capture (profiles/traffic.csv)
     traffic = None
+    traffic_file = ROOT / "profiles" / "traffic.csv"
     if traffic_file.exists():
-        try:
-            traffic = json.loads(traffic_file.read_text()).get(args.workload, {}).get(dom)
-        except Exception:
-            traffic = None
+        for ln in traffic_file.read_text().splitlines()[1:]:
+            f = ln.split(",")
+            if len(f) >= 3 and f[0] == args.workload and f[1] == dom:
+                traffic = float(f[2])
     roofline = {"bound": "hbm", "kernel": f"k_{dom}<{w.params['p']}>", "achieved": d["achieved_gbs"], "peak": peak, "unit": "GB/s",
                 "frac": d["achieved_gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
                 "alg_bytes_per_launch": d["alg_bytes_per_launch"], "avg_launch_ms": d["avg_ms"], "kernels": per_kind,
