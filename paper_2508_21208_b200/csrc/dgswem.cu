@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <numeric>
 #include <string>
@@ -155,6 +156,7 @@ struct dgswem {
   std::vector<void*> allocs;
   std::string err;
   long long launches = 0;
+  int res_edge[2] = {0, 0};   // resident grid of the persistent edge kernel [p-1]
 
   // optional per-kernel timing (dgswem_profile): CUDA events recorded on the stream around every launch
   struct ProfRec { int kind; cudaEvent_t a, b; };
@@ -274,6 +276,15 @@ int validate_mesh(dgswem* h, long long nn, const double* xy, long long ne, const
   return 0;
 }
 
+// resident grid of a persistent kernel: CTAs per SM (occupancy API) x SM count
+template <typename K>
+int resident_ctas(K kernel, int threads, size_t smem, int device) {
+  int per_sm = 0, sms = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess) return 0;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return 0;
+  return per_sm * sms;
+}
+
 template <int P>
 int launch_edge(dgswem* h, const double* w, double zeta_b) {
   EdgeArgs a;
@@ -281,8 +292,13 @@ int launch_edge(dgswem* h, const double* w, double zeta_b) {
   a.nd = (int)h->nd; a.ld = h->ld; a.ldd = h->ldd;
   a.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
   a.zeta_b = zeta_b;
+  const int ntiles = grid_for(h->nd, DGK_EDGE_THREADS);
+  const int resident = h->res_edge[P - 1];
   prof_begin(h, PK_EDGE);
-  k_edge<P><<<grid_for(h->nd, DGK_EDGE_THREADS), DGK_EDGE_THREADS, 0, h->stream>>>(a);
+  if (DGK_PIPE_EDGE && resident > 0 && ntiles > resident)
+    k_edge_pipe<P><<<resident, DGK_EDGE_THREADS, 0, h->stream>>>(a, ntiles);
+  else
+    k_edge<P><<<ntiles, DGK_EDGE_THREADS, 0, h->stream>>>(a);
   prof_end(h);
   CKL("k_edge");
   return 0;
@@ -411,7 +427,7 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
   h->prm = *prm;
   h->ndof = (prm->p + 1) * (prm->p + 2) / 2; h->nqe = prm->p + 1; h->nqa = prm->p == 1 ? 3 : 6; h->nstage = prm->rk_order;
   h->nn = n_nodes; h->ne = n_elem; h->nd = n_edge;
-  h->ld = round_up(n_elem, 64); h->ldd = round_up(n_edge, 64); h->ldn = round_up(n_nodes, 64);
+  h->ld = round_up(n_elem, 256); h->ldd = round_up(n_edge, 256); h->ldn = round_up(n_nodes, 64);
   int rc = validate_mesh(h, n_nodes, xy, n_elem, tri, n_edge, edge_elem, edge_local, edge_bc, elem_edge);
   if (rc) return bail(rc);
 
@@ -435,6 +451,15 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     CK(cudaMemcpyToSymbolAsync(c_tab1, &T1, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
     CK(cudaMemcpyToSymbolAsync(c_tab2, &T2, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
     CK(cudaStreamSynchronize(h->stream));
+
+    h->res_edge[0] = resident_ctas(k_edge_pipe<1>, DGK_EDGE_THREADS, 0, prm->device);
+    h->res_edge[1] = resident_ctas(k_edge_pipe<2>, DGK_EDGE_THREADS, 0, prm->device);
+    // tuning / test knob: DGSWEM_PERSISTENT_CTAS=n caps the persistent grid at n CTAs (so that small
+    // meshes walk several tiles per CTA); 0 switches the persistent kernel off
+    if (const char* env = std::getenv("DGSWEM_PERSISTENT_CTAS")) {
+      const int cap = std::atoi(env);
+      for (int& r : h->res_edge) r = cap <= 0 ? 0 : std::min(r, cap);
+    }
 
     const long long ne = h->ne, nd = h->nd, nn = h->nn, ld = h->ld, ldd = h->ldd, ldn = h->ldn;
     // ---- renumbering (internal only): perm_e[new] = old
