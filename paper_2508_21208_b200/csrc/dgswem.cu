@@ -157,6 +157,7 @@ struct dgswem {
   std::string err;
   long long launches = 0;
   int res_edge[2] = {0, 0};   // resident grid of the persistent edge kernel [p-1]
+  int res_limwd = 0;          // same for the limiter kernel of this handle's p
 
   // optional per-kernel timing (dgswem_profile): CUDA events recorded on the stream around every launch
   struct ProfRec { int kind; cudaEvent_t a, b; };
@@ -172,7 +173,7 @@ struct dgswem {
   int *einfo = nullptr, *elem_edge = nullptr, *nbr = nullptr, *tri = nullptr;
   int *perm_e = nullptr, *inv_e = nullptr, *inv_d = nullptr;   // perm_e[new]=old, inv_e[old]=new, inv_d[old]=new
   unsigned char *wet = nullptr, *wet_stage = nullptr;
-  int* flag = nullptr;
+  int* nf_flag = nullptr;
   size_t stage_bytes = 0;
 
   double t = 0.0;
@@ -314,6 +315,8 @@ int launch_elem(dgswem* h, const double* win, const double* w0, double* wout, do
   A.ne = (int)h->ne; A.ld = h->ld; A.ldd = h->ldd; A.ldn = h->ldn;
   A.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
   A.dt = dt; A.a = a; A.b = b; A.first_stage = first; A.wind = h->wind_on ? 1 : 0; A.fuse_wetdry = fuse_wd ? 1 : 0;
+  // (a persistent form with next-tile index prefetch, as for the edge kernel, was measured slower: it needs
+  // more registers than the 128 the 4-CTA budget leaves, and the spills cost more than the prefetch saves)
   prof_begin(h, PK_ELEM);
   k_elem<P, MODE><<<grid_for(h->ne, DGK_ELEM_THREADS), DGK_ELEM_THREADS, 0, h->stream>>>(A);
   prof_end(h);
@@ -327,7 +330,8 @@ int launch_limwd(dgswem* h, double* w) {
   A.w = w; A.mean = h->mean; A.nbr = h->nbr; A.hv = h->hv; A.wet = h->wet; A.ne = (int)h->ne; A.ld = h->ld;
   A.h0 = h->prm.h0_dry; A.limiter = h->prm.limiter; A.wetdry = h->prm.wetdry;
   prof_begin(h, PK_LIMWD);
-  k_limwd<P><<<grid_for(h->ne, 128), 128, 0, h->stream>>>(A);
+  const int ntiles = grid_for(h->ne, 128);
+  k_limwd<P><<<std::max(1, std::min(ntiles, h->res_limwd > 0 ? h->res_limwd : ntiles)), 128, 0, h->stream>>>(A, ntiles);
   prof_end(h);
   CKL("k_limwd");
   return 0;
@@ -355,10 +359,10 @@ double tide_value(const dgswem* h, double t) {
 template <int P>
 int run_stage(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b, int first,
               double t_stage) {
-  int rc = launch_edge<P>(h, win, tide_value(h, t_stage));
-  if (rc) return rc;
   const bool lim = h->prm.limiter != 0;
   const bool wd = h->prm.wetdry != 0;
+  int rc = launch_edge<P>(h, win, tide_value(h, t_stage));
+  if (rc) return rc;
   rc = launch_elem<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim);
   if (rc) return rc;
   if (lim) rc = launch_limwd<P>(h, wout);
@@ -456,9 +460,11 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     h->res_edge[1] = resident_ctas(k_edge_pipe<2>, DGK_EDGE_THREADS, 0, prm->device);
     // tuning / test knob: DGSWEM_PERSISTENT_CTAS=n caps the persistent grid at n CTAs (so that small
     // meshes walk several tiles per CTA); 0 switches the persistent kernel off
+    h->res_limwd = prm->p == 1 ? resident_ctas(k_limwd<1>, 128, 0, prm->device) : resident_ctas(k_limwd<2>, 128, 0, prm->device);
     if (const char* env = std::getenv("DGSWEM_PERSISTENT_CTAS")) {
       const int cap = std::atoi(env);
       for (int& r : h->res_edge) r = cap <= 0 ? 0 : std::min(r, cap);
+      h->res_limwd = cap <= 0 ? 0 : std::min(h->res_limwd, cap);
     }
 
     const long long ne = h->ne, nd = h->nd, nn = h->nn, ld = h->ld, ldd = h->ldd, ldn = h->ldn;
@@ -472,18 +478,24 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
         cy[e] = (xy[2 * (long long)t[0] + 1] + xy[2 * (long long)t[1] + 1] + xy[2 * (long long)t[2] + 1]) / 3.0;
       }
       perm_e = hilbert_order(cx, cy);
-      std::vector<double> mx(nd), my(nd);
-      for (long long d = 0; d < nd; ++d) {
-        const long long ep = edge_elem[2 * d]; const int lp = edge_local[2 * d];
-        const long long a = tri[3 * ep + (lp + 1) % 3], b = tri[3 * ep + (lp + 2) % 3];
-        mx[d] = 0.5 * (xy[2 * a] + xy[2 * b]); my[d] = 0.5 * (xy[2 * a + 1] + xy[2 * b + 1]);
-      }
-      perm_d = hilbert_order(mx, my);
     } else {
       std::iota(perm_e.begin(), perm_e.end(), 0);
       std::iota(perm_d.begin(), perm_d.end(), 0);
     }
     for (long long i = 0; i < ne; ++i) inv_e[perm_e[i]] = (int)i;
+    if (prm->reorder == 1) {
+      // edges follow the elements: sorted by (first, second) of their two elements in the new element
+      // numbering, so an edge sits next to the first element that needs it and the
+      // state gather of consecutive edges walks consecutive elements
+      std::vector<uint64_t> key(nd);
+      for (long long d = 0; d < nd; ++d) {
+        const uint32_t ip = (uint32_t)inv_e[edge_elem[2 * d]];
+        const uint32_t im = edge_elem[2 * d + 1] >= 0 ? (uint32_t)inv_e[edge_elem[2 * d + 1]] : ip;
+        key[d] = ((uint64_t)std::min(ip, im) << 32) | (uint64_t)std::max(ip, im);
+      }
+      std::iota(perm_d.begin(), perm_d.end(), 0);
+      std::stable_sort(perm_d.begin(), perm_d.end(), [&](int x, int y) { return key[x] < key[y]; });
+    }
     for (long long i = 0; i < nd; ++i) inv_d[perm_d[i]] = (int)i;
 
     // ---- element geometry in internal order (same expression trees as the spec)
@@ -569,8 +581,8 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     h->stage_buf = (double*)h->dalloc(h->stage_bytes);
     h->wet = (unsigned char*)h->dalloc((size_t)ld);
     h->wet_stage = (unsigned char*)h->dalloc((size_t)ld);
-    h->flag = (int*)h->dalloc(256);
-    if (!h->flux || !h->mean || !h->tau || !h->stage_buf || !h->wet || !h->wet_stage || !h->flag)
+    h->nf_flag = (int*)h->dalloc(256);
+    if (!h->flux || !h->mean || !h->tau || !h->stage_buf || !h->wet || !h->wet_stage || !h->nf_flag)
       return h->fail(DGSWEM_E_CUDA, "device allocation failed");
     CK(cudaMemsetAsync(h->flux, 0, fbytes, h->stream));
     CK(cudaMemsetAsync(h->mean, 0, (size_t)3 * ld * sizeof(double), h->stream));
@@ -692,8 +704,8 @@ int dgswem_get_state(dgswem_t* h, double* t, double* ze, double* qx, double* qy)
     CKL("k_gather_rows");
     src = h->stage_buf;
   }
-  CK(cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream));
-  k_check_finite<<<148 * 8, 256, 0, h->stream>>>(h->W[0], (long long)3 * h->ndof * h->ld, h->flag);
+  CK(cudaMemsetAsync(h->nf_flag, 0, sizeof(int), h->stream));
+  k_check_finite<<<148 * 8, 256, 0, h->stream>>>(h->W[0], (long long)3 * h->ndof * h->ld, h->nf_flag);
   CKL("k_check_finite");
   double* dst[3] = {ze, qx, qy};
   const size_t row = (size_t)h->ne * sizeof(double);
@@ -701,7 +713,7 @@ int dgswem_get_state(dgswem_t* h, double* t, double* ze, double* qx, double* qy)
     CK(cudaMemcpy2DAsync(dst[c], row, src + (size_t)c * h->ndof * h->ld, (size_t)h->ld * sizeof(double), row, h->ndof,
                          cudaMemcpyDeviceToHost, h->stream));
   int flag = 0;
-  CK(cudaMemcpyAsync(&flag, h->flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaMemcpyAsync(&flag, h->nf_flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
   if (t) *t = h->t;
   if (flag) return h->fail(DGSWEM_E_NONFINITE, "non-finite value in the state at t=%g", h->t);
