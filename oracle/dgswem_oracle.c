@@ -9,9 +9,12 @@
  * SURVEY.md §8(c) / DESIGN.md "Readings" apply; each is marked [R-n] below.
  *
  * Arithmetic: every expression is written with one IEEE-754 binary64 operation
- * per C operator, evaluated left to right as parenthesised; build with
- * -ffp-contract=off (no fused multiply-add), no -ffast-math.  The wet/dry
- * decisions are taken in this precision.
+ * per C operator or fma() call, evaluated left to right as parenthesised.  Sums
+ * of products (polynomial evaluation, quadrature accumulation, dot products) are
+ * written with the IEEE-754-2008 fusedMultiplyAdd, C99 fma(a,b,c) = a*b+c rounded
+ * once, explicitly, where DESIGN.md section 2 says so; the compiler contracts
+ * nothing by itself (-ffp-contract=off, no -ffast-math).  The wet/dry decisions
+ * are taken in this precision.
  * OpenMP (optional) only parallelises loops whose iterations write disjoint
  * outputs, so the result is bit-identical to the serial run.
  */
@@ -127,12 +130,12 @@ int orc_make_tables(int p, orc_tables* T) {
 void orc_llf_flux(double g, double h0, double nx, double ny, double hq,
                   double zp, double qxp, double qyp, double zm, double qxm, double qym,
                   int bc, double zeta_b, double* fz, double* fqx, double* fqy) {
-  double qnp = qxp * nx + qyp * ny;
-  double qtp = qyp * nx - qxp * ny;
+  double qnp = fma(qyp, ny, qxp * nx);
+  double qtp = fma(qyp, nx, -(qxp * ny));
   double qnm, qtm;
   if (bc == 0) {
-    qnm = qxm * nx + qym * ny;
-    qtm = qym * nx - qxm * ny;
+    qnm = fma(qym, ny, qxm * nx);
+    qtm = fma(qym, nx, -(qxm * ny));
   } else if (bc == 1) {
     zm = zp; qnm = -qnp; qtm = qtp;
   } else {
@@ -147,14 +150,15 @@ void orc_llf_flux(double g, double h0, double nx, double ny, double hq,
   double lp = fabs(unp) + cp, lm = fabs(unm) + cm;
   double lam = (lp > lm) ? lp : lm;
   double hl = 0.5 * lam;
-  double Pp = (g * zp) * (0.5 * zp + hq);
-  double Pm = (g * zm) * (0.5 * zm + hq);
-  double f0 = 0.5 * (qnp + qnm) - hl * (zm - zp);
-  double fn = 0.5 * ((qnp * unp + Pp) + (qnm * unm + Pm)) - hl * (qnm - qnp);
-  double ft = 0.5 * (qtp * unp + qtm * unm) - hl * (qtm - qtp);
+  double Pp = (g * zp) * fma(0.5, zp, hq);
+  double Pm = (g * zm) * fma(0.5, zm, hq);
+  /* each bracket is symmetric in (+,-), so swapping the sides and negating n negates the flux bit for bit */
+  double f0 = fma(-hl, zm - zp, 0.5 * (qnp + qnm));
+  double fn = fma(-hl, qnm - qnp, 0.5 * (fma(qnp, unp, Pp) + fma(qnm, unm, Pm)));
+  double ft = fma(-hl, qtm - qtp, 0.5 * (qtp * unp + qtm * unm));
   *fz = f0;
-  *fqx = fn * nx - ft * ny;
-  *fqy = fn * ny + ft * nx;
+  *fqx = fma(fn, nx, -(ft * ny));
+  *fqy = fma(fn, ny, ft * nx);
 }
 
 /* ------------------------------------------------- deterministic exp / log */
@@ -169,22 +173,22 @@ double orc_det_exp(double x) {
   if (x < -700.0) return 0.0;
   if (x > 700.0) x = 700.0;
   double kf = rint(x * INV_LN2);
-  double r = (x - kf * LN2_HI) - kf * LN2_LO;
+  double r = fma(-kf, LN2_LO, fma(-kf, LN2_HI, x));
   /* Taylor series of e^r, |r| <= 0.35, degree 13, Horner */
   double q = 1.0 / 6227020800.0;
-  q = q * r + 1.0 / 479001600.0;
-  q = q * r + 1.0 / 39916800.0;
-  q = q * r + 1.0 / 3628800.0;
-  q = q * r + 1.0 / 362880.0;
-  q = q * r + 1.0 / 40320.0;
-  q = q * r + 1.0 / 5040.0;
-  q = q * r + 1.0 / 720.0;
-  q = q * r + 1.0 / 120.0;
-  q = q * r + 1.0 / 24.0;
-  q = q * r + 1.0 / 6.0;
-  q = q * r + 0.5;
-  q = q * r + 1.0;
-  q = q * r + 1.0;
+  q = fma(q, r, 1.0 / 479001600.0);
+  q = fma(q, r, 1.0 / 39916800.0);
+  q = fma(q, r, 1.0 / 3628800.0);
+  q = fma(q, r, 1.0 / 362880.0);
+  q = fma(q, r, 1.0 / 40320.0);
+  q = fma(q, r, 1.0 / 5040.0);
+  q = fma(q, r, 1.0 / 720.0);
+  q = fma(q, r, 1.0 / 120.0);
+  q = fma(q, r, 1.0 / 24.0);
+  q = fma(q, r, 1.0 / 6.0);
+  q = fma(q, r, 0.5);
+  q = fma(q, r, 1.0);
+  q = fma(q, r, 1.0);
   return ldexp(q, (int)kf);
 }
 
@@ -197,19 +201,19 @@ double orc_det_log(double x) {
   double s = f / (2.0 + f);
   double z = s * s;
   double q = 1.0 / 23.0;
-  q = q * z + 1.0 / 21.0;
-  q = q * z + 1.0 / 19.0;
-  q = q * z + 1.0 / 17.0;
-  q = q * z + 1.0 / 15.0;
-  q = q * z + 1.0 / 13.0;
-  q = q * z + 1.0 / 11.0;
-  q = q * z + 1.0 / 9.0;
-  q = q * z + 1.0 / 7.0;
-  q = q * z + 1.0 / 5.0;
-  q = q * z + 1.0 / 3.0;
-  q = q * z + 1.0;
+  q = fma(q, z, 1.0 / 21.0);
+  q = fma(q, z, 1.0 / 19.0);
+  q = fma(q, z, 1.0 / 17.0);
+  q = fma(q, z, 1.0 / 15.0);
+  q = fma(q, z, 1.0 / 13.0);
+  q = fma(q, z, 1.0 / 11.0);
+  q = fma(q, z, 1.0 / 9.0);
+  q = fma(q, z, 1.0 / 7.0);
+  q = fma(q, z, 1.0 / 5.0);
+  q = fma(q, z, 1.0 / 3.0);
+  q = fma(q, z, 1.0);
   double ef = (double)e;
-  return (ef * LN2_HI + (2.0 * s) * q) + ef * LN2_LO;
+  return fma(ef, LN2_LO, fma(ef, LN2_HI, (2.0 * s) * q));
 }
 
 /* ------------------------------------------------------------------- wind */
@@ -218,15 +222,15 @@ double orc_det_log(double x) {
 void orc_holland_node(const orc_holland* h, double cx, double cy, double x, double y,
                       double* tsx, double* tsy, double* Vout) {
   double dx = x - cx, dy = y - cy;
-  double r = sqrt(dx * dx + dy * dy);
+  double r = sqrt(fma(dy, dy, dx * dx));
   if (r < 1.0) { *tsx = 0.0; *tsy = 0.0; if (Vout) *Vout = 0.0; return; }
   double xb = orc_det_exp(h->B * orc_det_log(h->rmax / r));   /* (R/r)^B */
   double rf2 = 0.5 * (r * h->f);
-  double V = sqrt(((h->B / h->rho_air) * xb) * (h->dp * orc_det_exp(-xb)) + rf2 * rf2) - rf2;
+  double V = sqrt(fma((h->B / h->rho_air) * xb, h->dp * orc_det_exp(-xb), rf2 * rf2)) - rf2;
   double rr = 1.0 / r;
   double wx = (-(dy * rr)) * V;
   double wy = (dx * rr) * V;
-  double cd = (0.75 + 0.067 * V) * 1.0e-3;
+  double cd = fma(0.067, V, 0.75) * 1.0e-3;
   if (cd > 0.0035) cd = 0.0035;
   double k = ((h->rho_air / h->rho_water) * cd) * V;
   *tsx = k * wx;
@@ -271,7 +275,7 @@ static void vertex_values(const double* w, double* u) {
   double amb = w[0] - w[1];
   u[0] = amb - w[2];
   u[1] = amb + w[2];
-  u[2] = w[0] + 2.0 * w[1];
+  u[2] = fma(2.0, w[1], w[0]);
 }
 static void modes_from_vertices(const double* u, double* w) {
   double a = ((u[0] + u[1]) + u[2]) / 3.0;
@@ -306,7 +310,7 @@ static void thin_layer_momentum(double h0, const double* Hh, double* qx, double*
     for (int v = 0; v < 3; ++v) { kept[v] = wv[v] * qv[v]; R = R + (qv[v] - kept[v]); }
     if (W > 0.0) {
       double share = R / W;
-      for (int v = 0; v < 3; ++v) qv[v] = kept[v] + share * wv[v];
+      for (int v = 0; v < 3; ++v) qv[v] = fma(share, wv[v], kept[v]);
     } else {
       for (int v = 0; v < 3; ++v) qv[v] = 0.0;
     }
@@ -327,22 +331,22 @@ int orc_wetdry_elem(const orc_tables* T, double h0, const double* hv, double* ze
     int low = 0;
     for (int v = 0; v < 3 && !low; ++v) {
       double z = ze[0];
-      for (int k = 1; k < ndof; ++k) z = z + ze[k] * T->phiV[v][k];
+      for (int k = 1; k < ndof; ++k) z = fma(ze[k], T->phiV[v][k], z);
       if (z + hv[v] <= h1) low = 1;
     }
     for (int l = 0; l < 3 && !low; ++l) {
       int a = (l + 1) % 3, b = (l + 2) % 3;
       for (int j = 0; j < T->nqe && !low; ++j) {
         double z = ze[0];
-        for (int k = 1; k < ndof; ++k) z = z + ze[k] * T->phiE[l][j][k];
+        for (int k = 1; k < ndof; ++k) z = fma(ze[k], T->phiE[l][j][k], z);
         double hq = hv[a] * T->elam[j][0] + hv[b] * T->elam[j][1];
         if (z + hq <= h1) low = 1;
       }
     }
     for (int i = 0; i < T->nqa && !low; ++i) {
       double z = ze[0];
-      for (int k = 1; k < ndof; ++k) z = z + ze[k] * T->phiA[i][k];
-      double hq = (hv[0] * T->la[i][0] + hv[1] * T->la[i][1]) + hv[2] * T->la[i][2];
+      for (int k = 1; k < ndof; ++k) z = fma(ze[k], T->phiA[i][k], z);
+      double hq = fma(hv[2], T->la[i][2], fma(hv[1], T->la[i][1], hv[0] * T->la[i][0]));
       if (z + hq <= h1) low = 1;
     }
     if (low) for (int k = 3; k < 6; ++k) { ze[k] = 0.0; qx[k] = 0.0; qy[k] = 0.0; }
@@ -399,13 +403,13 @@ int orc_ssprk_step(int order, int64_t n, double* w, double* w0, double* rhs, dou
     rhs_fn(ctx, s, t + C[s] * dt, w, rhs);
     if (s == 0) {
 #pragma omp parallel for schedule(static)
-      for (int64_t i = 0; i < n; ++i) w[i] = w[i] + dt * rhs[i];
+      for (int64_t i = 0; i < n; ++i) w[i] = fma(dt, rhs[i], w[i]);
     } else {
       const double a = A[s], b = B[s];
 #pragma omp parallel for schedule(static)
       for (int64_t i = 0; i < n; ++i) {
-        double u = w[i] + dt * rhs[i];
-        w[i] = a * w0[i] + b * u;
+        double u = fma(dt, rhs[i], w[i]);
+        w[i] = fma(b, u, a * w0[i]);
       }
     }
     if (post_fn) post_fn(ctx, s, w);
@@ -537,21 +541,21 @@ static void edge_flux_all(orc_model* m, const double* w, double zeta_b) {
       const double* php = T->phiE[lp][j];
       double zp = ze[ep], qxp = qx[ep], qyp = qy[ep];
       for (int k = 1; k < ndof; ++k) {
-        zp = zp + ze[k * ne + ep] * php[k];
-        qxp = qxp + qx[k * ne + ep] * php[k];
-        qyp = qyp + qy[k * ne + ep] * php[k];
+        zp = fma(ze[k * ne + ep], php[k], zp);
+        qxp = fma(qx[k * ne + ep], php[k], qxp);
+        qyp = fma(qy[k * ne + ep], php[k], qyp);
       }
       double zm = 0.0, qxm = 0.0, qym = 0.0;
       if (bc == 0) {
         const double* phm = T->phiE[lm][nqe - 1 - j];
         zm = ze[em]; qxm = qx[em]; qym = qy[em];
         for (int k = 1; k < ndof; ++k) {
-          zm = zm + ze[k * ne + em] * phm[k];
-          qxm = qxm + qx[k * ne + em] * phm[k];
-          qym = qym + qy[k * ne + em] * phm[k];
+          zm = fma(ze[k * ne + em], phm[k], zm);
+          qxm = fma(qx[k * ne + em], phm[k], qxm);
+          qym = fma(qy[k * ne + em], phm[k], qym);
         }
       }
-      double hq = hba * T->elam[j][0] + hbb * T->elam[j][1];
+      double hq = hba * T->elam[j][0] + hbb * T->elam[j][1];   /* symmetric in (a,b): same value from either side */
       double fz, fx, fy;
       orc_llf_flux(m->prm.g, m->prm.h0_dry, nx, ny, hq, zp, qxp, qyp, zm, qxm, qym, bc, zeta_b, &fz, &fx, &fy);
       m->flux[(0 * nqe + j) * nd + d] = fz;
@@ -585,9 +589,8 @@ static void elem_rhs_all(orc_model* m, const double* w, double* rhs, double* sca
         for (int c = 0; c < 3; ++c) {
           double t = lf * m->flux[(c * nqe + jj) * nd + d];
           for (int k = 0; k < ndof; ++k) {
-            double term = T->efac[l][j][k] * t;
-            if (plus) r[c][k] = r[c][k] - term; else r[c][k] = r[c][k] + term;
-            sc[c][k] += fabs(term);
+            if (plus) r[c][k] = fma(-T->efac[l][j][k], t, r[c][k]); else r[c][k] = fma(T->efac[l][j][k], t, r[c][k]);
+            sc[c][k] += fabs(T->efac[l][j][k] * t);
           }
         }
       }
@@ -595,31 +598,31 @@ static void elem_rhs_all(orc_model* m, const double* w, double* rhs, double* sca
     /* ---- AREA ---- */
     double x1x = m->jinv[e], x1y = m->jinv[ne + e], x2x = m->jinv[2 * ne + e], x2y = m->jinv[3 * ne + e];
     double hv0 = m->hv[e], hv1 = m->hv[ne + e], hv2 = m->hv[2 * ne + e];
-    double dhx = 0.5 * ((hv1 - hv0) * x1x + (hv2 - hv0) * x2x);   /* grad h_b, constant */
-    double dhy = 0.5 * ((hv1 - hv0) * x1y + (hv2 - hv0) * x2y);
+    double dhx = 0.5 * fma(hv2 - hv0, x2x, (hv1 - hv0) * x1x);   /* grad h_b, constant */
+    double dhy = 0.5 * fma(hv2 - hv0, x2y, (hv1 - hv0) * x1y);
     int wet = m->wet[e];
     const int32_t* tn = m->tri + 3 * e;
     for (int i = 0; i < nqa; ++i) {
       double z = ze[e], u_qx = qx[e], u_qy = qy[e];
       for (int k = 1; k < ndof; ++k) {                              /* Alg. 1 lines 10-15 */
-        z = z + ze[k * ne + e] * T->phiA[i][k];
-        u_qx = u_qx + qx[k * ne + e] * T->phiA[i][k];
-        u_qy = u_qy + qy[k * ne + e] * T->phiA[i][k];
+        z = fma(ze[k * ne + e], T->phiA[i][k], z);
+        u_qx = fma(qx[k * ne + e], T->phiA[i][k], u_qx);
+        u_qy = fma(qy[k * ne + e], T->phiA[i][k], u_qy);
       }
-      double hq = (hv0 * T->la[i][0] + hv1 * T->la[i][1]) + hv2 * T->la[i][2];
+      double hq = fma(hv2, T->la[i][2], fma(hv1, T->la[i][1], hv0 * T->la[i][0]));
       double H = z + hq;
       double Hc = (H > h0) ? H : h0;
       double rH = 1.0 / Hc;
       double u = u_qx * rH, v = u_qy * rH;
       double gz = g * z;
-      double P = gz * (0.5 * z + hq);
+      double P = gz * fma(0.5, z, hq);
       double F[3][2];                                               /* eqs (7)-(9) */
       F[0][0] = u_qx;         F[0][1] = u_qy;
-      F[1][0] = u_qx * u + P; F[1][1] = u_qx * v;
-      F[2][0] = F[1][1];      F[2][1] = u_qy * v + P;
+      F[1][0] = fma(u_qx, u, P); F[1][1] = u_qx * v;
+      F[2][0] = F[1][1];         F[2][1] = fma(u_qy, v, P);
       double tau = 0.0, tsx = 0.0, tsy = 0.0;
       if (wet) {                                                    /* friction, wind: wet elements only [R-6] */
-        tau = (cf * sqrt(u_qx * u_qx + u_qy * u_qy)) * (rH * rH);
+        tau = (cf * sqrt(fma(u_qy, u_qy, u_qx * u_qx))) * (rH * rH);
         if (m->wind_on) {
           /* wind stress, linear from the three nodes, ramped by the local depth with the same
            * thin-layer weight as the wet/dry momentum rule: clamp((H-H0)/(H1-H0),0,1), H1=10 H0
@@ -629,21 +632,21 @@ static void elem_rhs_all(orc_model* m, const double* w, double* rhs, double* sca
           if (H <= h0) ramp = 0.0;
           else if (H >= 10.0 * h0) ramp = 1.0;
           else ramp = (H - h0) * (1.0 / (10.0 * h0 - h0));
-          tsx = ramp * ((tx[tn[0]] * T->la[i][0] + tx[tn[1]] * T->la[i][1]) + tx[tn[2]] * T->la[i][2]);
-          tsy = ramp * ((ty[tn[0]] * T->la[i][0] + ty[tn[1]] * T->la[i][1]) + ty[tn[2]] * T->la[i][2]);
+          tsx = ramp * fma(tx[tn[2]], T->la[i][2], fma(tx[tn[1]], T->la[i][1], tx[tn[0]] * T->la[i][0]));
+          tsy = ramp * fma(ty[tn[2]], T->la[i][2], fma(ty[tn[1]], T->la[i][1], ty[tn[0]] * T->la[i][0]));
         }
       }
       double S[3];
       S[0] = 0.0;                                                   /* rain R: out of scope */
-      S[1] = ((gz * dhx - tau * u_qx) + fc * u_qy) + tsx;
-      S[2] = ((gz * dhy - tau * u_qy) - fc * u_qx) + tsy;
+      S[1] = fma(fc, u_qy, fma(-tau, u_qx, gz * dhx)) + tsx;
+      S[2] = fma(-fc, u_qx, fma(-tau, u_qy, gz * dhy)) + tsy;
       for (int k = 0; k < ndof; ++k) {                              /* Alg. 1 lines 26-35 */
-        double gxk = T->dphiA1[i][k] * x1x + T->dphiA2[i][k] * x2x;
-        double gyk = T->dphiA1[i][k] * x1y + T->dphiA2[i][k] * x2y;
+        double gxk = fma(T->dphiA2[i][k], x2x, T->dphiA1[i][k] * x1x);
+        double gyk = fma(T->dphiA2[i][k], x2y, T->dphiA1[i][k] * x1y);
         double xf = T->wfac[i][k] * gxk, yf = T->wfac[i][k] * gyk, sf = T->srfac[i][k];
-        r[0][k] = r[0][k] + (xf * F[0][0] + yf * F[0][1]);
-        r[1][k] = r[1][k] + ((xf * F[1][0] + yf * F[1][1]) + sf * S[1]);
-        r[2][k] = r[2][k] + ((xf * F[2][0] + yf * F[2][1]) + sf * S[2]);
+        r[0][k] = fma(yf, F[0][1], fma(xf, F[0][0], r[0][k]));
+        r[1][k] = fma(sf, S[1], fma(yf, F[1][1], fma(xf, F[1][0], r[1][k])));
+        r[2][k] = fma(sf, S[2], fma(yf, F[2][1], fma(xf, F[2][0], r[2][k])));
         for (int c = 0; c < 3; ++c)
           sc[c][k] += fabs(xf * F[c][0]) + fabs(yf * F[c][1]) + (c ? fabs(sf * (gz * (c == 1 ? dhx : dhy))) +
                       fabs(sf * (tau * (c == 1 ? u_qx : u_qy))) + fabs(sf * (fc * (c == 1 ? u_qy : u_qx))) +
