@@ -148,6 +148,23 @@ class ClockSampler:
 
 
 # ---------------------------------------------------------------------------------------------
+# N > 1: independent replicas (the path does not shard in this build), no collective on the
+# data path; the ranks only agree on the slowest replica's time.
+def max_over_ranks(x: float, world: int, device) -> float:
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def whole_job_value(world: int, dofs_stage: int, steps: int, seconds: float) -> float:
+    """DOF-updates/s of the whole job: every replica advances `steps` steps in `seconds` (max over ranks)."""
+    return world * dofs_stage * steps / seconds
+
+
 def run_reference(args, rank: int):
     """The CPU oracle, as it stands, on the host cores (bench contract: reference arm)."""
     if rank != 0:
@@ -219,11 +236,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     prof = g.profile_read()
     g.profile(False)
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        tt = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
-    value = world * dofs_stage * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, "cuda")
+    value = whole_job_value(world, dofs_stage, args.steps, ms * 1e-3)
 
     # ---- end to end through the C ABI with host buffers: set_state (H2D) + K steps + get_state/get_wetdry (D2H)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
@@ -238,12 +252,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     g.get_wetdry()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        tt = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_s = float(tt.item())
+    e2e_s = max_over_ranks(e2e_s, world, "cuda")
     state_bytes = 3 * w.ndof * w.mesh.n_elem * 8
-    e2e = {"value": world * dofs_stage * args.steps / e2e_s, "unit": UNIT,
+    e2e = {"value": whole_job_value(world, dofs_stage, args.steps, e2e_s), "unit": UNIT,
            "h2d_bytes_per_step": state_bytes / args.steps, "d2h_bytes_per_step": (state_bytes + w.mesh.n_elem) / args.steps,
            "call": f"dgswem_set_state + dgswem_step({args.steps}) + dgswem_get_state + dgswem_get_wetdry, pinned host buffers, "
                    f"wall clock; bytes are the per-job copies divided by the {args.steps} steps"}
