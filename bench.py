@@ -55,7 +55,7 @@ def make_workload(name: str, scale: float = 1.0):
 # algorithmic bytes: what the two-kernel design must move per launch, every
 # array counted once (unique-read assumption: each element's state is read once by EDGE although
 # three edges use it; each flux value once by the element kernel although two elements use it).
-def alg_bytes(w, kind: str, stage_first: bool) -> float:
+def alg_bytes(w, kind: str, stage_first: bool, fused: bool = False) -> float:
     ne, nd = w.mesh.n_elem, w.mesh.n_edge
     nn = w.mesh.n_nodes
     ndof, nqe = w.ndof, w.params["p"] + 1
@@ -63,6 +63,20 @@ def alg_bytes(w, kind: str, stage_first: bool) -> float:
     st = 3 * ndof * 8
     if kind == "edge":
         return nd * (8 + 4 + 16 + 16 + 3 * nqe * 8) + ne * st
+    if kind == "elem" and fused:
+        # element-centric stage kernel (A1-A5, A7): state once (the neighbours' rows are other elements' own
+        # rows: unique-read assumption), neighbour table 12, normals 48, L/A 24, Jacobian 32, vertex bathymetry
+        # 24, wet flag 1, new state; no flux buffer, no edge records
+        b = ne * (st + 12 + 48 + 24 + 32 + 24 + 1 + st)
+        if not stage_first:
+            b += ne * st
+        if wd and not lim:
+            b += ne * 1
+        if lim:
+            b += ne * 24
+        if wind:
+            b += ne * 12 + nn * 16
+        return b
     if kind == "elem":
         b = nd * 3 * nqe * 8 + ne * (st + 12 + 24 + 32 + 24 + 1 + st)
         if not stage_first:
@@ -81,11 +95,11 @@ def alg_bytes(w, kind: str, stage_first: bool) -> float:
     raise ValueError(kind)
 
 
-def stage_bytes_total(w) -> float:
+def stage_bytes_total(w, fused: bool = False) -> float:
     """Algorithmic bytes of one whole time step (all stages)."""
     tot = alg_bytes(w, "wind", True) if w.holland is not None else 0.0
     for s in range(w.n_stage):
-        tot += alg_bytes(w, "edge", s == 0) + alg_bytes(w, "elem", s == 0)
+        tot += (0.0 if fused else alg_bytes(w, "edge", s == 0)) + alg_bytes(w, "elem", s == 0, fused)
         if w.params["limiter"]:
             tot += alg_bytes(w, "limwd", s == 0)
     return tot
@@ -209,6 +223,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     w = make_workload(args.workload)
     g = pk.Dgswem.from_workload(w, reorder=args.reorder, device=local_rank)
     dofs_stage = w.dofs * w.n_stage
+    fused = g.stage_form() == 1
 
     def barrier():
         if world > 1:
@@ -267,7 +282,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     for k, (tms, cnt) in prof.items():
         if cnt:
             nfirst = cnt // w.n_stage if k in ("edge", "elem", "limwd") else cnt
-            byts = (alg_bytes(w, k, True) * nfirst + alg_bytes(w, k, False) * (cnt - nfirst)) / cnt
+            byts = (alg_bytes(w, k, True, fused) * nfirst + alg_bytes(w, k, False, fused) * (cnt - nfirst)) / cnt
             per_kind[k] = {"launches": cnt, "avg_ms": tms / cnt, "alg_bytes_per_launch": byts,
                            "achieved_gbs": byts / (tms / cnt * 1e-3) / 1e9, "share_of_step": tms / ms}
     dom = max(per_kind, key=lambda k: per_kind[k]["avg_ms"] * per_kind[k]["launches"])
@@ -278,14 +293,20 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     if traffic_file.exists():
         for ln in traffic_file.read_text().splitlines()[1:]:
             f = ln.split(",")
-            if len(f) >= 3 and f[0] == args.workload and f[1] == dom:
+            if len(f) >= 3 and f[0] == args.workload and f[1] == ("stage" if (fused and dom == "elem") else dom):
                 traffic = float(f[2])
-    roofline = {"bound": "hbm", "kernel": f"k_{dom}<{w.params['p']}>", "achieved": d["achieved_gbs"], "peak": peak, "unit": "GB/s",
+    kname = "k_stage" if (fused and dom == "elem") else f"k_{dom}"
+    sb = stage_bytes_total(w, fused)
+    # SURVEY.md section 8(d)'s figure for the flux-buffer design (591 B per element-stage at p = 1), for reference
+    sb_survey = stage_bytes_total(w, False)
+    roofline = {"bound": "hbm", "kernel": f"{kname}<{w.params['p']}>", "achieved": d["achieved_gbs"], "peak": peak, "unit": "GB/s",
                 "frac": d["achieved_gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
                 "alg_bytes_per_launch": d["alg_bytes_per_launch"], "avg_launch_ms": d["avg_ms"], "kernels": per_kind,
-                "whole_step": {"alg_bytes": stage_bytes_total(w), "achieved_gbs": stage_bytes_total(w) / (ms / args.steps * 1e-3) / 1e9,
-                               "frac_of_measured_peak": stage_bytes_total(w) / (ms / args.steps * 1e-3) / 1e9 / peak,
-                               "frac_of_8TBs_nominal": stage_bytes_total(w) / (ms / args.steps * 1e-3) / 1e9 / 8000.0}}
+                "whole_step": {"alg_bytes": sb, "achieved_gbs": sb / (ms / args.steps * 1e-3) / 1e9,
+                               "frac_of_measured_peak": sb / (ms / args.steps * 1e-3) / 1e9 / peak,
+                               "frac_of_8TBs_nominal": sb / (ms / args.steps * 1e-3) / 1e9 / 8000.0,
+                               "alg_bytes_flux_buffer_design": sb_survey,
+                               "frac_of_measured_peak_at_flux_buffer_bytes": sb_survey / (ms / args.steps * 1e-3) / 1e9 / peak}}
 
     # ---- CPU baseline: the oracle on a bounded sample of the same workload, on this box's cores
     cpu = None
@@ -307,7 +328,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             "config": {"workload": w.name, "n_elem": w.mesh.n_elem, "n_edge": w.mesh.n_edge, "n_nodes": w.mesh.n_nodes,
                        "p": w.params["p"], "rk_order": w.params["rk_order"], "dt": w.dt, "limiter": w.params["limiter"],
                        "wetdry": w.params["wetdry"], "wind": w.holland is not None, "tide": w.tide is not None,
-                       "reorder": args.reorder, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                       "reorder": args.reorder, "stage_form": "element-centric stage kernel (no flux buffer)" if fused
+                       else "edge kernel + element kernel (flux buffer)", "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                        "l2": f"state {state_bytes / 1e6:.0f} MB per buffer + flux {w.mesh.n_edge * 3 * (w.params['p'] + 1) * 8 / 1e6:.0f} MB "
                              "per stage exceed the 126 MB L2 (inputs larger than L2, no flush needed)"
                              if state_bytes > 130e6 else "working set fits L2: a >L2 buffer is NOT flushed between steps; see DESIGN.md"},

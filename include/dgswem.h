@@ -100,6 +100,16 @@ int dgswem_get_wetdry(dgswem_t*, uint8_t* wet);
 /* Nodal kinematic wind stress tau_s/rho_0 of the last WIND evaluation, [2][n_nodes] (test hook). */
 int dgswem_get_wind(dgswem_t*, double* tau);
 
+/* TEST HOOK: the kernels' reciprocal and square-root routines next to the IEEE
+ * operators, on n caller-supplied arguments x (host): out (host, [4][n]) = rcp_rn(x), sqrt_rn(x), 1.0/x, sqrt(x).
+ * Arguments outside the routines' stated range give unspecified values in rows 0 and 1. */
+int dgswem_test_math(dgswem_t*, int64_t n, const double* x, double* out);
+
+/* Which form of the RK stage this handle runs: 0 = edge kernel + element kernel with the per-edge flux
+ * buffer, 1 = element-centric stage kernel without it (default for p = 1; DGSWEM_FUSED=0/1 in the environment of
+ * dgswem_create overrides).  Both give the same bits. */
+int dgswem_stage_form(const dgswem_t*);
+
 /* Number of kernels launched by this handle so far (for bench.py's gpu_launches). */
 int64_t dgswem_launch_count(const dgswem_t*);
 

@@ -43,7 +43,7 @@ class DgswemError(RuntimeError):
 
 EXPORTS = ["dgswem_create", "dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_step",
            "dgswem_eval_rhs", "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_wind",
-           "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
+           "dgswem_test_math", "dgswem_stage_form", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
 
 _lib = None
 
@@ -71,6 +71,8 @@ def load_library():
     L.dgswem_get_state.argtypes = [VP, PD, PD, PD, PD]
     L.dgswem_get_wetdry.argtypes = [VP, C.POINTER(C.c_uint8)]
     L.dgswem_get_wind.argtypes = [VP, PD]
+    L.dgswem_test_math.argtypes = [VP, I64, PD, PD]
+    L.dgswem_stage_form.argtypes = [VP]; L.dgswem_stage_form.restype = C.c_int
     L.dgswem_launch_count.argtypes = [VP]; L.dgswem_launch_count.restype = I64
     L.dgswem_profile.argtypes = [VP, C.c_int]; L.dgswem_profile.restype = C.c_int
     L.dgswem_profile_read.argtypes = [VP, PD, C.POINTER(I64)]; L.dgswem_profile_read.restype = C.c_int
@@ -212,6 +214,17 @@ class Dgswem:
         tau = np.empty((2, self.n_nodes))
         self._check(self.L.dgswem_get_wind(self.h, _dp(tau)))
         return tau
+
+    def test_math(self, x):
+        """TEST HOOK: (rcp_rn(x), sqrt_rn(x), 1.0/x, sqrt(x)) evaluated by the device routines."""
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        out = np.empty((4, x.size))
+        self._check(self.L.dgswem_test_math(self.h, C.c_int64(x.size), _dp(x), _dp(out)))
+        return out
+
+    def stage_form(self) -> int:
+        """0: edge kernel + element kernel (flux buffer); 1: element-centric stage kernel."""
+        return int(self.L.dgswem_stage_form(self.h))
 
     def launch_count(self) -> int:
         return int(self.L.dgswem_launch_count(self.h))

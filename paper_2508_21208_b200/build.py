@@ -30,7 +30,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and LIB.exists() and LIB.stat().st_mtime >= max(d.stat().st_mtime for d in DEPS):
         return LIB
     tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
-    cmd = [nvcc(), *NVCC_FLAGS, "-I", str(ROOT / "include"), "-I", str(PKG / "csrc"), "-o", str(tmp), str(SRC)]
+    extra = os.environ.get("DGSWEM_NVCC_EXTRA", "").split()   # tuning sweeps: e.g. -DDGK_STAGE_MINB=4
+    cmd = [nvcc(), *NVCC_FLAGS, *extra, "-I", str(ROOT / "include"), "-I", str(PKG / "csrc"), "-o", str(tmp), str(SRC)]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd))

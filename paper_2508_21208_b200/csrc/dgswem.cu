@@ -170,7 +170,9 @@ struct dgswem {
   double *flux = nullptr, *mean = nullptr, *jinv = nullptr, *lfac = nullptr, *hv = nullptr;
   double *en = nullptr, *ehb = nullptr, *tau = nullptr, *nxy = nullptr, *stage_buf = nullptr;
   int2* edge_elem = nullptr;
-  int *einfo = nullptr, *elem_edge = nullptr, *nbr = nullptr, *tri = nullptr;
+  int *einfo = nullptr, *elem_edge = nullptr, *nbr = nullptr, *tri = nullptr, *nbinfo = nullptr;
+  double* enl = nullptr;
+  bool fused = false;         // element-centric stage kernel (k_stage) instead of k_edge + k_elem
   int *perm_e = nullptr, *inv_e = nullptr, *inv_d = nullptr;   // perm_e[new]=old, inv_e[old]=new, inv_d[old]=new
   unsigned char *wet = nullptr, *wet_stage = nullptr;
   int* nf_flag = nullptr;
@@ -311,6 +313,7 @@ int launch_elem(dgswem* h, const double* win, const double* w0, double* wout, do
   ElemArgs A;
   A.win = win; A.w0 = w0; A.wout = wout; A.flux = h->flux; A.elem_edge = h->elem_edge; A.jinv = h->jinv;
   A.lfac = h->lfac; A.hv = h->hv; A.tri = h->tri; A.tau = h->tau; A.wet = h->wet;
+  A.nbinfo = nullptr; A.enl = nullptr; A.zeta_b = 0.0;
   A.mean = write_mean ? h->mean : nullptr;
   A.ne = (int)h->ne; A.ld = h->ld; A.ldd = h->ldd; A.ldn = h->ldn;
   A.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
@@ -321,6 +324,25 @@ int launch_elem(dgswem* h, const double* win, const double* w0, double* wout, do
   k_elem<P, MODE><<<grid_for(h->ne, DGK_ELEM_THREADS), DGK_ELEM_THREADS, 0, h->stream>>>(A);
   prof_end(h);
   CKL("k_elem");
+  return 0;
+}
+
+// A1-A5 (+A7) in one launch (element-centric form, no flux buffer)
+template <int P, int MODE>
+int launch_stage(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b,
+                 int first, bool fuse_wd, bool write_mean, double zeta_b) {
+  ElemArgs A;
+  A.win = win; A.w0 = w0; A.wout = wout; A.flux = h->flux; A.elem_edge = h->elem_edge; A.jinv = h->jinv;
+  A.lfac = h->lfac; A.hv = h->hv; A.tri = h->tri; A.tau = h->tau; A.wet = h->wet;
+  A.nbinfo = h->nbinfo; A.enl = h->enl; A.zeta_b = zeta_b;
+  A.mean = write_mean ? h->mean : nullptr;
+  A.ne = (int)h->ne; A.ld = h->ld; A.ldd = h->ldd; A.ldn = h->ldn;
+  A.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
+  A.dt = dt; A.a = a; A.b = b; A.first_stage = first; A.wind = h->wind_on ? 1 : 0; A.fuse_wetdry = fuse_wd ? 1 : 0;
+  prof_begin(h, PK_ELEM);
+  k_stage<P, MODE><<<grid_for(h->ne, DGK_ELEM_THREADS), DGK_ELEM_THREADS, 0, h->stream>>>(A);
+  prof_end(h);
+  CKL("k_stage");
   return 0;
 }
 
@@ -361,9 +383,14 @@ int run_stage(dgswem* h, const double* win, const double* w0, double* wout, doub
               double t_stage) {
   const bool lim = h->prm.limiter != 0;
   const bool wd = h->prm.wetdry != 0;
-  int rc = launch_edge<P>(h, win, tide_value(h, t_stage));
-  if (rc) return rc;
-  rc = launch_elem<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim);
+  int rc;
+  if (h->fused) {
+    rc = launch_stage<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim, tide_value(h, t_stage));
+  } else {
+    rc = launch_edge<P>(h, win, tide_value(h, t_stage));
+    if (rc) return rc;
+    rc = launch_elem<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim);
+  }
   if (rc) return rc;
   if (lim) rc = launch_limwd<P>(h, wout);
   return rc;
@@ -422,12 +449,15 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
   auto bail = [&](int code) { g_create_error = h->err; dgswem_destroy(h); return code; };
   if (!prm || !xy || !bathy || !tri || !edge_elem || !edge_local || !edge_bc || !elem_edge)
     return bail(h->fail(DGSWEM_E_ARG, "NULL argument"));
-  if (n_nodes < 3 || n_elem < 1 || n_edge < 3 || n_elem > 0x3fffffff || n_edge > 0x7ffffff0 || n_nodes > 0x7ffffff0)
+  if (n_nodes < 3 || n_elem < 1 || n_edge < 3 || n_elem > 0x1fffffff || n_edge > 0x7ffffff0 || n_nodes > 0x7ffffff0)
     return bail(h->fail(DGSWEM_E_ARG, "bad sizes"));
   if ((prm->p != 1 && prm->p != 2) || (prm->rk_order != 2 && prm->rk_order != 3))
     return bail(h->fail(DGSWEM_E_ARG, "p must be 1 or 2, rk_order 2 or 3"));
   if (!(prm->h0_dry > 0.0) || !(prm->g > 0.0) || prm->cf < 0.0)
     return bail(h->fail(DGSWEM_E_ARG, "need h0_dry > 0, g > 0, cf >= 0"));
+  // range of the kernels' reciprocal / square-root routines (rcp_rn, sqrt_rn): arguments are H_c >= h0_dry and g * H_c
+  if (!(prm->h0_dry >= 1e-100) || !(prm->g * prm->h0_dry >= 1e-100) || !(prm->g <= 1e100) || !(prm->h0_dry <= 1e100))
+    return bail(h->fail(DGSWEM_E_ARG, "need 1e-100 <= h0_dry <= 1e100, g <= 1e100 and g*h0_dry >= 1e-100"));
   h->prm = *prm;
   h->ndof = (prm->p + 1) * (prm->p + 2) / 2; h->nqe = prm->p + 1; h->nqa = prm->p == 1 ? 3 : 6; h->nstage = prm->rk_order;
   h->nn = n_nodes; h->ne = n_elem; h->nd = n_edge;
@@ -467,6 +497,10 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
       h->res_limwd = cap <= 0 ? 0 : std::min(h->res_limwd, cap);
     }
 
+    // DGSWEM_FUSED=1/0: element-centric stage kernel (no flux buffer) on/off; default: on for p = 1
+    h->fused = prm->p == 1;
+    if (const char* env = std::getenv("DGSWEM_FUSED")) h->fused = std::atoi(env) != 0;
+
     const long long ne = h->ne, nd = h->nd, nn = h->nn, ld = h->ld, ldd = h->ldd, ldn = h->ldn;
     // ---- renumbering (internal only): perm_e[new] = old
     std::vector<int> perm_e(ne), inv_e(ne), perm_d(nd), inv_d(nd);
@@ -500,7 +534,8 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
 
     // ---- element geometry in internal order (same expression trees as the spec)
     std::vector<double> jinv(4 * ld, 0.0), lfac(3 * ld, 0.0), hv(3 * ld, 0.0);
-    std::vector<int> ee_packed(3 * ld, 0), nbr(3 * ld, -1), trin(3 * ld, 0);
+    std::vector<int> ee_packed(3 * ld, 0), nbr(3 * ld, -1), trin(3 * ld, 0), nbinfo(3 * ld, (int)0x80000001);
+    std::vector<double> enl(6 * ld, 0.0);
     for (long long i = 0; i < ne; ++i) {
       const long long e = perm_e[i];
       const int* t = tri + 3 * e;
@@ -526,6 +561,18 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
         ee_packed[l * ld + i] = inv_d[d] | (plus ? 0 : (int)0x80000000);
         const long long other = plus ? edge_elem[2 * d + 1] : edge_elem[2 * d];
         nbr[l * ld + i] = other >= 0 ? inv_e[other] : -1;
+        // element-centric form: neighbour id | its local edge << 29 (or bit 31 | boundary code), and the
+        // outward normal: the e+ side's normal (computed from the e+ vertices, as for the edge kernel) or its negative
+        const int lo = plus ? edge_local[2 * d + 1] : edge_local[2 * d];
+        nbinfo[l * ld + i] = other >= 0 ? (inv_e[other] | (lo << 29)) : (int)(0x80000000u | (unsigned)edge_bc[d]);
+        const long long ep = edge_elem[2 * d];
+        const int lp = edge_local[2 * d];
+        const long long pa = tri[3 * ep + (lp + 1) % 3], pb = tri[3 * ep + (lp + 2) % 3];
+        const double px = xy[2 * pb] - xy[2 * pa], py = xy[2 * pb + 1] - xy[2 * pa + 1];
+        const double rL = 1.0 / std::sqrt(px * px + py * py);
+        const double nx = py * rL, ny = (-px) * rL;
+        enl[(2 * l) * ld + i] = plus ? nx : -nx;
+        enl[(2 * l + 1) * ld + i] = plus ? ny : -ny;
       }
     }
     // ---- edge geometry in internal order, from the e+ side
@@ -556,6 +603,8 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     if ((r = upload(h, h->hv, hv))) return r;
     if ((r = upload(h, h->elem_edge, ee_packed))) return r;
     if ((r = upload(h, h->nbr, nbr))) return r;
+    if ((r = upload(h, h->nbinfo, nbinfo))) return r;
+    if ((r = upload(h, h->enl, enl))) return r;
     if ((r = upload(h, h->tri, trin))) return r;
     if ((r = upload(h, h->edge_elem, ee))) return r;
     if ((r = upload(h, h->einfo, einfo))) return r;
@@ -656,7 +705,11 @@ int dgswem_eval_rhs(dgswem_t* h, double* rze, double* rqx, double* rqy) {
   int rc;
   if (h->wind_on && (rc = launch_wind(h, h->t))) return rc;
   double* rbuf = h->W[1];   // scratch: W[1] holds no live data between steps
-  if (h->prm.p == 1) {
+  if (h->fused) {
+    rc = h->prm.p == 1 ? launch_stage<1, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, 0.0, 1.0, 1, false, false, tide_value(h, h->t))
+                       : launch_stage<2, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, 0.0, 1.0, 1, false, false, tide_value(h, h->t));
+    if (rc) return rc;
+  } else if (h->prm.p == 1) {
     if ((rc = launch_edge<1>(h, h->W[0], tide_value(h, h->t)))) return rc;
     if ((rc = launch_elem<1, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, 0.0, 1.0, 1, false, false))) return rc;
   } else {
@@ -682,6 +735,10 @@ int dgswem_get_flux(dgswem_t* h, double* flux) {
   if (!h) return DGSWEM_E_ARG;
   if (!flux) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
   CK(cudaSetDevice(h->prm.device));
+  if (h->fused) {   // the element-centric stage kernel keeps no flux buffer: evaluate A1 on the current state
+    int rc = h->prm.p == 1 ? launch_edge<1>(h, h->W[0], tide_value(h, h->t)) : launch_edge<2>(h, h->W[0], tide_value(h, h->t));
+    if (rc) return rc;
+  }
   const double* src = h->flux;
   if (h->inv_d) {
     k_gather_rows<<<grid_for(h->nd, 256), 256, 0, h->stream>>>(h->stage_buf, h->ldd, h->flux, h->ldd, h->inv_d, (int)h->nd, 3 * h->nqe);
@@ -744,6 +801,23 @@ int dgswem_get_wind(dgswem_t* h, double* tau) {
   CK(cudaStreamSynchronize(h->stream));
   return DGSWEM_OK;
 }
+
+int dgswem_test_math(dgswem_t* h, int64_t n, const double* x, double* out) {
+  if (!h) return DGSWEM_E_ARG;
+  if (n < 1 || !x || !out) return h->fail(DGSWEM_E_ARG, "need n >= 1 and non-NULL pointers");
+  CK(cudaSetDevice(h->prm.device));
+  double* dx = (double*)h->dalloc((size_t)n * sizeof(double));
+  double* dout = (double*)h->dalloc((size_t)4 * n * sizeof(double));
+  if (!dx || !dout) return h->fail(DGSWEM_E_CUDA, "device allocation failed");
+  CK(cudaMemcpyAsync(dx, x, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  k_test_math<<<grid_for(n, 256), 256, 0, h->stream>>>(dx, (long long)n, dout);
+  CKL("k_test_math");
+  CK(cudaMemcpyAsync(out, dout, (size_t)4 * n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return DGSWEM_OK;   // the two scratch buffers stay with the handle until dgswem_destroy
+}
+
+int dgswem_stage_form(const dgswem_t* h) { return (h && h->fused) ? 1 : 0; }
 
 int64_t dgswem_launch_count(const dgswem_t* h) { return h ? h->launches : 0; }
 
