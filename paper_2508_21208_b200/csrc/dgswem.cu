@@ -358,7 +358,8 @@ int launch_stage(dgswem* h, const double* win, const double* w0, double* wout, d
   A.ne = (int)h->ne; A.ld = h->ld; A.ldd = h->ldd; A.ldn = h->ldn;
   A.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
   A.dt = dt; A.a = a; A.b = b; A.first_stage = first; A.wind = h->wind_on ? 1 : 0; A.fuse_wetdry = fuse_wd ? 1 : 0;
-  // (a persistent form with next-tile neighbour-table prefetch was measured slower: 425 vs 374 us on C3)
+  // (persistent forms were measured slower on C3: next-tile neighbour-table prefetch 425 us, per-warp cp.async
+  // staging of the next tile's rows in shared memory 445 us, against 374 us)
   prof_begin(h, PK_ELEM);
   k_stage<P, MODE><<<grid_for(h->ne, DGK_STAGE_THREADS), DGK_STAGE_THREADS, 0, h->stream>>>(A);
   prof_end(h);
