@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- fp64 DOF-updates/s per RK stage of the DG-SWEM hot path on B200 (BASELINE.json metric).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C1|C2p1|C2p2|C4|C5] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C1|C2p1|C2p2|C4|C5|H] [--impl ours|reference]
 
 A "step" is one full explicit time step of the workload: WIND (if on) and, per RK stage, EDGE ->
 GATHER+AREA+RK(+wet/dry) -> (limiter+wet/dry), i.e. every row of SURVEY.md section 8(a).  Default
@@ -38,6 +38,9 @@ def make_workload(name: str, scale: float = 1.0):
     if name == "C3":
         nn = max(20, int(round(1500 * scale)))
         return c3(nn=nn)
+    if name == "H":
+        # the paper's Harvey / TX2008 mesh size (6,675,517 elements) on the C3 recipe: 2 x 1827^2 = 6,675,858
+        return c3(nn=max(20, int(round(1828 * scale))))
     if name == "C1":
         return c1()
     if name == "C2p1":

@@ -340,7 +340,17 @@ int launch_elem(dgswem* h, const double* win, const double* w0, double* wout, do
   // (a persistent form with next-tile index prefetch, as for the edge kernel, was measured slower: it needs
   // more registers than the 128 the 4-CTA budget leaves, and the spills cost more than the prefetch saves)
   prof_begin(h, PK_ELEM);
-  k_elem<P, MODE><<<grid_for(h->ne, DGK_ELEM_THREADS), DGK_ELEM_THREADS, 0, h->stream>>>(A);
+  const int grid = grid_for(h->ne, DGK_ELEM_THREADS);
+  if constexpr (MODE == MODE_UPDATE) {
+    switch ((first ? 1 : 0) | (h->wind_on ? 2 : 0)) {   // specialised on (first stage, wind), as k_stage
+      case 0: k_elem<P, MODE, 0><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
+      case 1: k_elem<P, MODE, 1><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
+      case 2: k_elem<P, MODE, 2><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
+      default: k_elem<P, MODE, 3><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
+    }
+  } else {
+    k_elem<P, MODE, -1><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A);
+  }
   prof_end(h);
   CKL("k_elem");
   return 0;
@@ -361,7 +371,18 @@ int launch_stage(dgswem* h, const double* win, const double* w0, double* wout, d
   // (persistent forms were measured slower on C3: next-tile neighbour-table prefetch 425 us, per-warp cp.async
   // staging of the next tile's rows in shared memory 445 us, against 374 us)
   prof_begin(h, PK_ELEM);
-  k_stage<P, MODE><<<grid_for(h->ne, DGK_STAGE_THREADS), DGK_STAGE_THREADS, 0, h->stream>>>(A);
+  const int grid = grid_for(h->ne, DGK_STAGE_THREADS);
+  if constexpr (MODE == MODE_UPDATE) {
+    // specialised on (first stage, wind): no w^n registers in stage 1, no wind registers without wind
+    switch ((first ? 1 : 0) | (h->wind_on ? 2 : 0)) {
+      case 0: k_stage<P, MODE, 0><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      case 1: k_stage<P, MODE, 1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      case 2: k_stage<P, MODE, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      default: k_stage<P, MODE, 3><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+    }
+  } else {
+    k_stage<P, MODE, -1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A);
+  }
   prof_end(h);
   CKL("k_stage");
   return 0;
