@@ -62,3 +62,59 @@ def test_sass_has_fp64_and_no_float_atomics():
     body = sass[sass.index("k_elem"):]
     assert "DMUL" in body and "DADD" in body
     assert "RED." not in sass and "ATOM" not in sass
+
+
+def _raw_create(lib, w, *, params=None, tri=None, edge_elem=None, edge_bc=None, elem_edge=None):
+    """dgswem_create through ctypes with NULL hooks (no torch, no device memory before validation)."""
+    import ctypes as C
+    import numpy as np
+    from paper_2508_21208_b200.binding import Params
+    m = w.mesh
+    prm = dict(w.params) if params is None else params
+    P = Params(p=int(prm["p"]), rk_order=int(prm["rk_order"]), g=prm["g"], cf=prm["cf"], coriolis_f=prm["coriolis_f"],
+               h0_dry=prm["h0_dry"], limiter=int(prm["limiter"]), wetdry=int(prm["wetdry"]), reorder=1, device=0)
+    xy = np.ascontiguousarray(m.xy, dtype=np.float64)
+    bathy = np.ascontiguousarray(w.bathy, dtype=np.float64)
+    tri = np.ascontiguousarray(m.tri if tri is None else tri, dtype=np.int32)
+    ee = np.ascontiguousarray(m.edge_elem if edge_elem is None else edge_elem, dtype=np.int32)
+    el = np.ascontiguousarray(m.edge_local, dtype=np.int8)
+    bc = np.ascontiguousarray(m.edge_bc if edge_bc is None else edge_bc, dtype=np.int32)
+    eled = np.ascontiguousarray(m.elem_edge if elem_edge is None else elem_edge, dtype=np.int32)
+    dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+    ip = lambda a: a.ctypes.data_as(C.POINTER(C.c_int32))
+    h = C.c_void_p()
+    rc = lib.dgswem_create(C.byref(h), C.byref(P), None, xy.shape[0], dp(xy), dp(bathy), tri.shape[0], ip(tri), ee.shape[0],
+                           ip(ee), el.ctypes.data_as(C.POINTER(C.c_int8)), ip(bc), ip(eled))
+    msg = lib.dgswem_last_error(None)
+    if rc == 0:
+        lib.dgswem_destroy(h)
+    return rc, (msg.decode() if msg else "")
+
+
+def test_create_validates_arguments_and_mesh_on_the_host(lib):
+    """Argument and mesh validation runs before any CUDA call, so its error codes can be checked here:
+    -1 bad parameter, -2 inconsistent tables (orientation, edge/element cross references, boundary codes);
+    a valid mesh gets as far as the device (0 with a GPU, -3 'no CUDA device' without)."""
+    import numpy as np
+    from workloads import c1
+    w = c1(nq=4)
+    m = w.mesh
+    for key, val in (("p", 3), ("rk_order", 4), ("h0_dry", 0.0), ("h0_dry", 1e-200), ("g", -9.81), ("cf", -1.0)):
+        bad = dict(w.params); bad[key] = val
+        rc, msg = _raw_create(lib, w, params=bad)
+        assert rc == -1, (key, val, rc, msg)
+    rc, msg = _raw_create(lib, w, tri=m.tri[:, ::-1].copy())                 # clockwise elements
+    assert rc == -2 and "counter-clockwise" in msg
+    tri = m.tri.copy(); tri[3, 1] = m.n_nodes + 5                             # node id out of range
+    assert _raw_create(lib, w, tri=tri)[0] == -2
+    ee = m.edge_elem.copy(); ee[0, 0] = (ee[0, 0] + 1) % m.n_elem             # edge points at the wrong element
+    assert _raw_create(lib, w, edge_elem=ee)[0] == -2
+    eled = m.elem_edge.copy(); eled[2, 0], eled[2, 1] = eled[2, 1], eled[2, 0]   # local edges swapped
+    assert _raw_create(lib, w, elem_edge=eled)[0] == -2
+    bc = m.edge_bc.copy(); bc[np.flatnonzero(m.edge_elem[:, 1] >= 0)[0]] = 1  # interior edge with a boundary code
+    assert _raw_create(lib, w, edge_bc=bc)[0] == -2
+    bc = m.edge_bc.copy(); bc[np.flatnonzero(m.edge_elem[:, 1] < 0)[0]] = 0   # boundary edge without one
+    assert _raw_create(lib, w, edge_bc=bc)[0] == -2
+    rc, msg = _raw_create(lib, w)
+    import torch
+    assert rc == (0 if torch.cuda.is_available() else -3), (rc, msg)
