@@ -684,34 +684,34 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
       const double dx1 = x1 - x0, dy1 = y1 - y0, dx2 = x2 - x0, dy2 = y2 - y0;
       const double A = 0.5 * (dx1 * dy2 - dx2 * dy1);
       const double rA = 1.0 / A;
-      jinv[0 * ld + i] = dy2 * rA;
-      jinv[1 * ld + i] = (-dx2) * rA;
-      jinv[2 * ld + i] = (-dy1) * rA;
-      jinv[3 * ld + i] = dx1 * rA;
+      jinv[tix(4, 0, i)] = dy2 * rA;
+      jinv[tix(4, 1, i)] = (-dx2) * rA;
+      jinv[tix(4, 2, i)] = (-dy1) * rA;
+      jinv[tix(4, 3, i)] = dx1 * rA;
       for (int l = 0; l < 3; ++l) {
         const long long na = t[(l + 1) % 3], nb = t[(l + 2) % 3];
         const double ex = xy[2 * nb] - xy[2 * na], ey = xy[2 * nb + 1] - xy[2 * na + 1];
         const double L = std::sqrt(ex * ex + ey * ey);
-        lfac[l * ld + i] = L * rA;
-        hv[l * ld + i] = bathy[t[l]];
-        trin[l * ld + i] = t[l];
+        lfac[tix(3, l, i)] = L * rA;
+        hv[tix(3, l, i)] = bathy[t[l]];
+        trin[tix(3, l, i)] = t[l];
         const long long d = elem_edge[3 * e + l];
         const bool plus = edge_elem[2 * d] == e && edge_local[2 * d] == l;
-        ee_packed[l * ld + i] = inv_d[d] | (plus ? 0 : (int)0x80000000);
+        ee_packed[tix(3, l, i)] = inv_d[d] | (plus ? 0 : (int)0x80000000);
         const long long other = plus ? edge_elem[2 * d + 1] : edge_elem[2 * d];
-        nbr[l * ld + i] = other >= 0 ? inv_e[other] : -1;
+        nbr[tix(3, l, i)] = other >= 0 ? inv_e[other] : -1;
         // element-centric form: neighbour id | its local edge << 29 (or bit 31 | boundary code), and the
         // outward normal: the e+ side's normal (computed from the e+ vertices, as for the edge kernel) or its negative
         const int lo = plus ? edge_local[2 * d + 1] : edge_local[2 * d];
-        nbinfo[l * ld + i] = other >= 0 ? (inv_e[other] | (lo << 29)) : (int)(0x80000000u | (unsigned)edge_bc[d]);
+        nbinfo[tix(3, l, i)] = other >= 0 ? (inv_e[other] | (lo << 29)) : (int)(0x80000000u | (unsigned)edge_bc[d]);
         const long long ep = edge_elem[2 * d];
         const int lp = edge_local[2 * d];
         const long long pa = tri[3 * ep + (lp + 1) % 3], pb = tri[3 * ep + (lp + 2) % 3];
         const double px = xy[2 * pb] - xy[2 * pa], py = xy[2 * pb + 1] - xy[2 * pa + 1];
         const double rL = 1.0 / std::sqrt(px * px + py * py);
         const double nx = py * rL, ny = (-px) * rL;
-        enl[(2 * l) * ld + i] = plus ? nx : -nx;
-        enl[(2 * l + 1) * ld + i] = plus ? ny : -ny;
+        enl[tix(6, 2 * l, i)] = plus ? nx : -nx;
+        enl[tix(6, 2 * l + 1, i)] = plus ? ny : -ny;
       }
     }
     // ---- edge geometry in internal order, from the e+ side
@@ -793,15 +793,13 @@ int dgswem_set_state(dgswem_t* h, double t, const double* ze, const double* qx, 
   CK(cudaSetDevice(h->prm.device));
   const double* src[3] = {ze, qx, qy};
   const size_t row = (size_t)h->ne * sizeof(double);
-  // stage in caller order (rows of length ne, leading dimension ld), then renumber on the device
-  double* stage = h->perm_e ? h->stage_buf : h->W[0];
+  // stage in caller order (rows of length ne, leading dimension ld), then renumber into the tiled layout on the device
+  double* stage = h->stage_buf;
   for (int c = 0; c < 3; ++c)
     CK(cudaMemcpy2DAsync(stage + (size_t)c * h->ndof * h->ld, (size_t)h->ld * sizeof(double), src[c], row, row, h->ndof,
                          cudaMemcpyHostToDevice, h->stream));
-  if (h->perm_e) {
-    k_gather_rows<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->W[0], h->ld, stage, h->ld, h->perm_e, (int)h->ne, 3 * h->ndof);
-    CKL("k_gather_rows");
-  }
+  k_rows_to_tiled<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->W[0], stage, h->ld, h->perm_e, (int)h->ne, 3 * h->ndof);
+  CKL("k_rows_to_tiled");
   k_fill_bytes<<<grid_for(h->ld, 256), 256, 0, h->stream>>>(h->wet, 1, (int)h->ld);
   CKL("k_fill_bytes");
   if (h->prm.wetdry) {
@@ -858,12 +856,9 @@ int dgswem_eval_rhs(dgswem_t* h, double* rze, double* rqx, double* rqy) {
     if ((rc = launch_edge<2>(h, h->W[0], scal(h, 0, tide_value(h, h->t))))) return rc;
     if ((rc = launch_elem<2, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, 0.0, 1.0, 1, false, false))) return rc;
   }
-  const double* src = rbuf;
-  if (h->inv_e) {
-    k_gather_rows<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->stage_buf, h->ld, rbuf, h->ld, h->inv_e, (int)h->ne, 3 * h->ndof);
-    CKL("k_gather_rows");
-    src = h->stage_buf;
-  }
+  k_tiled_to_rows<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->stage_buf, h->ld, rbuf, h->inv_e, (int)h->ne, 3 * h->ndof);
+  CKL("k_tiled_to_rows");
+  const double* src = h->stage_buf;
   double* dst[3] = {rze, rqx, rqy};
   const size_t row = (size_t)h->ne * sizeof(double);
   for (int c = 0; c < 3; ++c)
@@ -897,12 +892,9 @@ int dgswem_get_state(dgswem_t* h, double* t, double* ze, double* qx, double* qy)
   if (!h) return DGSWEM_E_ARG;
   if (!ze || !qx || !qy) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
   CK(cudaSetDevice(h->prm.device));
-  const double* src = h->W[0];
-  if (h->inv_e) {
-    k_gather_rows<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->stage_buf, h->ld, h->W[0], h->ld, h->inv_e, (int)h->ne, 3 * h->ndof);
-    CKL("k_gather_rows");
-    src = h->stage_buf;
-  }
+  k_tiled_to_rows<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->stage_buf, h->ld, h->W[0], h->inv_e, (int)h->ne, 3 * h->ndof);
+  CKL("k_tiled_to_rows");
+  const double* src = h->stage_buf;
   CK(cudaMemsetAsync(h->nf_flag, 0, sizeof(int), h->stream));
   k_check_finite<<<148 * 8, 256, 0, h->stream>>>(h->W[0], (long long)3 * h->ndof * h->ld, h->nf_flag);
   CKL("k_check_finite");
