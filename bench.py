@@ -211,6 +211,58 @@ def run_reference(args, rank: int):
     print(json.dumps(line), flush=True)
 
 
+def run_decomp(args, rank: int, world: int, local_rank: int):
+    """--decomp P: ONE mesh split into partitions with halo exchange every RK stage (strong scaling).
+    world == 1: P partitions on this GPU (LocalTransport; measures the cost of the decomposition machinery itself).
+    world > 1: one partition per rank, NCCL isend/irecv of the packed halos (functional path, host-ordered per stage:
+    no graphs, no overlap yet; not measurable on this one-GPU box)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2508_21208_b200 import build as b
+    if rank == 0:
+        b.build()
+    if world > 1:
+        dist.barrier()
+    from paper_2508_21208_b200.decomp import PartitionedDgswem, DistTransport
+    torch.cuda.set_device(local_rank)
+    w = make_workload(args.workload)
+    m = w.mesh
+    n_parts = world if world > 1 else max(1, args.decomp)
+    pd = PartitionedDgswem(w.params, m.xy, w.bathy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, n_parts,
+                           tide=w.tide, holland=w.holland, reorder=args.reorder, device=local_rank,
+                           parts=[rank] if world > 1 else None, transport=DistTransport() if world > 1 else None)
+    pd.set_state(0.0, w.ze, w.qx, w.qy)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    pd.step(max(args.warmup, 3), w.dt)
+    barrier()
+    l0 = sum(g.launch_count() for g in pd.handles)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    pd.step(args.steps, w.dt)
+    ev1.record()
+    barrier()
+    ms = max_over_ranks(ev0.elapsed_time(ev1), world, "cuda")
+    launches = sum(g.launch_count() for g in pd.handles) - l0
+    if rank != 0:
+        return
+    value = w.dofs * w.n_stage * args.steps / (ms * 1e-3)      # the whole (single) mesh, whatever the number of ranks
+    ghosts = sum(s.n_local - s.n_owned for s in pd.subs)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": w.name, "n_elem": m.n_elem, "p": w.params["p"], "rk_order": w.params["rk_order"], "dt": w.dt,
+                       "parallelism": f"domain decomposition: {n_parts} partitions on {world} GPU(s), halo exchange every RK stage",
+                       "ghost_elements": int(ghosts), "transport": "NCCL isend/irecv" if world > 1 else "device copies (one GPU)"},
+            "gpu_launches": int(launches), "e2e": None, "roofline": None, "cpu_baseline": None}
+    print(json.dumps(line), flush=True)
+    pd.close()
+
+
 def run_ours(args, rank: int, world: int, local_rank: int):
     import torch
     import torch.distributed as dist
@@ -360,6 +412,8 @@ def main():
     ap.add_argument("--workload", default="C3")
     ap.add_argument("--reorder", type=int, default=1)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--decomp", type=int, default=0, help="domain decomposition instead of replicas: one partition per rank "
+                    "(N > 1), or this many partitions on the one GPU (N = 1)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -373,7 +427,10 @@ def main():
         torch.cuda.set_device(local_rank)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     try:
-        run_ours(args, rank, world, local_rank)
+        if args.decomp > 0:
+            run_decomp(args, rank, world, local_rank)
+        else:
+            run_ours(args, rank, world, local_rank)
     finally:
         if world > 1:
             import torch.distributed as dist

@@ -84,6 +84,25 @@ int dgswem_set_wind_holland(dgswem_t*, const dgswem_holland*);
  * stage EDGE -> GATHER+AREA+RK update -> limiter -> wet/dry.  Asynchronous on the stream. */
 int dgswem_step(dgswem_t*, int64_t nsteps, double dt);
 
+/* ---- Stage-granular stepping and halo lists: building blocks of a domain-decomposed run (
+ * PAPER.md:476-519 "Multiple GPUs").  A driver splits the mesh into partitions with one layer of edge-neighbour
+ * ghost elements (whose outer edges it closes as land edges), creates one handle per partition and, for every step,
+ * calls  begin_step;  for s in 0..rk_order-1: { stage_rhs(s); [limiter on: exchange what=1; stage_limit(s);]
+ * exchange what=0 };  end_step  -- where "exchange" = halo_pack on the owner, transport, halo_unpack on the ghost side.
+ * The ghost elements' own results are meaningless and are overwritten by every exchange; owned elements then get the
+ * same bits as in an undivided run.  dgswem_step must not be called between begin_step and end_step.
+ *   dgswem_set_halo: element ids (caller numbering of this handle) to pack (owned elements that are ghosts elsewhere)
+ *   and to unpack (this handle's ghosts); copied.  what = 0: the stage buffer written last (3*ndof rows; the current
+ *   state between steps), what = 1: the RK-updated means (3 rows).  buf: [rows][n_send] resp. [rows][n_recv] doubles,
+ *   host memory (buf_on_device = 0, synchronous) or device memory (1, asynchronous on the handle's stream). */
+int dgswem_begin_step(dgswem_t*, double dt);
+int dgswem_stage_rhs(dgswem_t*, int s);
+int dgswem_stage_limit(dgswem_t*, int s);
+int dgswem_end_step(dgswem_t*);
+int dgswem_set_halo(dgswem_t*, int64_t n_send, const int32_t* send_ids, int64_t n_recv, const int32_t* recv_ids);
+int dgswem_halo_pack(dgswem_t*, int what, double* buf, int buf_on_device);
+int dgswem_halo_unpack(dgswem_t*, int what, const double* buf, int buf_on_device);
+
 /* TEST HOOK: L_h(current state) (eq. (5)) at the current time, each [ndof][n_elem]. */
 int dgswem_eval_rhs(dgswem_t*, double* rze, double* rqx, double* rqy);
 

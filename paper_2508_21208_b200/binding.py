@@ -43,7 +43,8 @@ class DgswemError(RuntimeError):
 
 EXPORTS = ["dgswem_create", "dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_step",
            "dgswem_eval_rhs", "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_wind",
-           "dgswem_test_math", "dgswem_stage_form", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
+           "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_limit", "dgswem_end_step", "dgswem_set_halo",
+           "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_stage_form", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
 
 _lib = None
 
@@ -72,6 +73,13 @@ def load_library():
     L.dgswem_get_wetdry.argtypes = [VP, C.POINTER(C.c_uint8)]
     L.dgswem_get_wind.argtypes = [VP, PD]
     L.dgswem_test_math.argtypes = [VP, I64, PD, PD]
+    L.dgswem_begin_step.argtypes = [VP, D]
+    L.dgswem_stage_rhs.argtypes = [VP, C.c_int]
+    L.dgswem_stage_limit.argtypes = [VP, C.c_int]
+    L.dgswem_end_step.argtypes = [VP]
+    L.dgswem_set_halo.argtypes = [VP, I64, PI32, I64, PI32]
+    L.dgswem_halo_pack.argtypes = [VP, C.c_int, C.c_void_p, C.c_int]
+    L.dgswem_halo_unpack.argtypes = [VP, C.c_int, C.c_void_p, C.c_int]
     L.dgswem_stage_form.argtypes = [VP]; L.dgswem_stage_form.restype = C.c_int
     L.dgswem_launch_count.argtypes = [VP]; L.dgswem_launch_count.restype = I64
     L.dgswem_profile.argtypes = [VP, C.c_int]; L.dgswem_profile.restype = C.c_int
@@ -80,7 +88,9 @@ def load_library():
     L.dgswem_last_error.argtypes = [VP]; L.dgswem_last_error.restype = C.c_char_p
     L.dgswem_destroy.argtypes = [VP]; L.dgswem_destroy.restype = None
     for name in ("dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_step", "dgswem_eval_rhs",
-                 "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_wind", "dgswem_sync"):
+                 "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_wind", "dgswem_sync",
+                 "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_limit", "dgswem_end_step", "dgswem_set_halo",
+                 "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math"):
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -214,6 +224,42 @@ class Dgswem:
         tau = np.empty((2, self.n_nodes))
         self._check(self.L.dgswem_get_wind(self.h, _dp(tau)))
         return tau
+
+    # ---- stage-granular stepping and halo lists (domain decomposition building blocks)
+    def begin_step(self, dt):
+        self._check(self.L.dgswem_begin_step(self.h, float(dt)))
+
+    def stage_rhs(self, s):
+        self._check(self.L.dgswem_stage_rhs(self.h, int(s)))
+
+    def stage_limit(self, s):
+        self._check(self.L.dgswem_stage_limit(self.h, int(s)))
+
+    def end_step(self):
+        self._check(self.L.dgswem_end_step(self.h))
+
+    def set_halo(self, send_ids, recv_ids):
+        snd = np.ascontiguousarray(send_ids, dtype=np.int32)
+        rcv = np.ascontiguousarray(recv_ids, dtype=np.int32)
+        self.n_send, self.n_recv = snd.size, rcv.size
+        i32 = lambda a: a.ctypes.data_as(C.POINTER(C.c_int32))
+        self._check(self.L.dgswem_set_halo(self.h, snd.size, i32(snd), rcv.size, i32(rcv)))
+
+    def halo_rows(self, what):
+        return 3 * self.ndof if what == 0 else 3
+
+    def halo_pack(self, what, buf):
+        """buf: torch CUDA tensor (asynchronous on the handle's stream) or numpy array, [rows][n_send] float64."""
+        if isinstance(buf, np.ndarray):
+            self._check(self.L.dgswem_halo_pack(self.h, int(what), C.c_void_p(buf.ctypes.data), 0))
+        else:
+            self._check(self.L.dgswem_halo_pack(self.h, int(what), C.c_void_p(buf.data_ptr()), 1))
+
+    def halo_unpack(self, what, buf):
+        if isinstance(buf, np.ndarray):
+            self._check(self.L.dgswem_halo_unpack(self.h, int(what), C.c_void_p(buf.ctypes.data), 0))
+        else:
+            self._check(self.L.dgswem_halo_unpack(self.h, int(what), C.c_void_p(buf.data_ptr()), 1))
 
     def test_math(self, x):
         """TEST HOOK: (rcp_rn(x), sqrt_rn(x), 1.0/x, sqrt(x)) evaluated by the device routines."""

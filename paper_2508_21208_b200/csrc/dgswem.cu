@@ -190,6 +190,13 @@ struct dgswem {
   StepGraph graph_many, graph_one;
   double graph_dt = 0.0; bool graph_wind = false; bool graph_tide = false;
 
+  // stage-granular stepping and halo lists (dgswem_begin_step ... dgswem_halo_unpack)
+  double step_dt = 0.0;        // dt of the step in progress (0: none)
+  double* last_out = nullptr;  // stage buffer written by the last dgswem_stage_rhs (W[0] between steps)
+  int *halo_send = nullptr, *halo_recv = nullptr;   // internal element ids
+  long long n_send = 0, n_recv = 0;
+  double* halo_buf = nullptr;  // device staging for host-side pack/unpack, [rows][max(n_send, n_recv)]
+
   double t = 0.0;
   double tide_amp = 0.0, tide_omega = 0.0, tide_phase = 0.0;
   bool wind_on = false;
@@ -419,10 +426,10 @@ double tide_value(const dgswem* h, double t) {
   return h->tide_amp * std::sin(h->tide_omega * t + h->tide_phase);
 }
 
-// one RK stage: EDGE -> GATHER+AREA+RK(+wet/dry) -> (limiter, wet/dry)
+// one RK stage, first part: EDGE -> GATHER+AREA+RK (+wet/dry when no limiter follows)
 template <int P>
-int run_stage(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b, int first,
-              double t_stage, int stage) {
+int run_stage_rhs(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b, int first,
+                  double t_stage, int stage) {
   const bool lim = h->prm.limiter != 0;
   const bool wd = h->prm.wetdry != 0;
   int rc;
@@ -433,8 +440,16 @@ int run_stage(dgswem* h, const double* win, const double* w0, double* wout, doub
     if (rc) return rc;
     rc = launch_elem<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim);
   }
+  return rc;
+}
+
+// one RK stage: first part, then the limiter + wet/dry pass over the RK-updated means (limiter on)
+template <int P>
+int run_stage(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b, int first,
+              double t_stage, int stage) {
+  int rc = run_stage_rhs<P>(h, win, w0, wout, dt, a, b, first, t_stage, stage);
   if (rc) return rc;
-  if (lim) rc = launch_limwd<P>(h, wout);
+  if (h->prm.limiter != 0) rc = launch_limwd<P>(h, wout);
   return rc;
 }
 
@@ -771,6 +786,7 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     h->wet_stage = (unsigned char*)h->dalloc((size_t)ld);
     h->nf_flag = (int*)h->dalloc(256);
     h->step_ctr = (int*)h->dalloc(256);
+    h->last_out = h->W[0];
     if (const char* env = std::getenv("DGSWEM_GRAPH")) h->graphs_on = std::atoi(env) != 0;
     if (!h->flux || !h->mean || !h->tau || !h->stage_buf || !h->wet || !h->wet_stage || !h->nf_flag || !h->step_ctr)
       return h->fail(DGSWEM_E_CUDA, "device allocation failed");
@@ -809,6 +825,8 @@ int dgswem_set_state(dgswem_t* h, double t, const double* ze, const double* qx, 
   }
   CK(cudaStreamSynchronize(h->stream));   // the caller's buffers may be reused after return
   h->t = t;
+  h->step_dt = 0.0;
+  h->last_out = h->W[0];
   return DGSWEM_OK;
 }
 
@@ -834,8 +852,134 @@ int dgswem_set_wind_holland(dgswem_t* h, const dgswem_holland* hol) {
 int dgswem_step(dgswem_t* h, int64_t nsteps, double dt) {
   if (!h) return DGSWEM_E_ARG;
   if (nsteps < 0 || !(dt > 0.0)) return h->fail(DGSWEM_E_ARG, "need nsteps >= 0 and dt > 0");
+  if (h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a stage-granular step is in progress (dgswem_end_step)");
   CK(cudaSetDevice(h->prm.device));
   return h->prm.p == 1 ? run_steps<1>(h, nsteps, dt) : run_steps<2>(h, nsteps, dt);
+}
+
+// ---- stage-granular stepping + halo lists: the building blocks of a domain-decomposed run
+namespace {
+struct StageBufs { const double* win; const double* w0; double* wout; double a, b, c; int first; };
+inline StageBufs stage_bufs(dgswem* h, int s) {
+  const bool rk3 = h->prm.rk_order == 3;
+  const double* a = rk3 ? kA3 : kA2; const double* b = rk3 ? kB3 : kB2; const double* c = rk3 ? kC3 : kC2;
+  StageBufs B;
+  B.a = a[s]; B.b = b[s]; B.c = c[s]; B.first = s == 0; B.w0 = h->W[0];
+  if (s == 0) { B.win = h->W[0]; B.wout = h->W[1]; }
+  else if (!rk3 || s == 2) { B.win = h->W[s]; B.wout = h->W[0]; }
+  else { B.win = h->W[1]; B.wout = h->W[2]; }
+  return B;
+}
+}  // namespace
+
+int dgswem_begin_step(dgswem_t* h, double dt) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!(dt > 0.0)) return h->fail(DGSWEM_E_ARG, "need dt > 0");
+  if (h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a step is already in progress");
+  CK(cudaSetDevice(h->prm.device));
+  if (h->wind_on) { int rc = launch_wind(h, h->t); if (rc) return rc; }
+  h->step_dt = dt;
+  h->last_out = h->W[0];
+  return DGSWEM_OK;
+}
+
+int dgswem_stage_rhs(dgswem_t* h, int s) {
+  if (!h) return DGSWEM_E_ARG;
+  if (h->step_dt == 0.0) return h->fail(DGSWEM_E_ARG, "no step in progress (dgswem_begin_step)");
+  if (s < 0 || s >= h->nstage) return h->fail(DGSWEM_E_ARG, "stage index out of range");
+  CK(cudaSetDevice(h->prm.device));
+  const StageBufs B = stage_bufs(h, s);
+  const double ts = h->t + B.c * h->step_dt;
+  const int rc = h->prm.p == 1 ? run_stage_rhs<1>(h, B.win, B.w0, B.wout, h->step_dt, B.a, B.b, B.first, ts, s)
+                               : run_stage_rhs<2>(h, B.win, B.w0, B.wout, h->step_dt, B.a, B.b, B.first, ts, s);
+  if (rc == 0) h->last_out = B.wout;
+  return rc;
+}
+
+int dgswem_stage_limit(dgswem_t* h, int s) {
+  if (!h) return DGSWEM_E_ARG;
+  if (h->step_dt == 0.0) return h->fail(DGSWEM_E_ARG, "no step in progress (dgswem_begin_step)");
+  if (s < 0 || s >= h->nstage) return h->fail(DGSWEM_E_ARG, "stage index out of range");
+  if (h->prm.limiter == 0) return DGSWEM_OK;
+  CK(cudaSetDevice(h->prm.device));
+  const StageBufs B = stage_bufs(h, s);
+  return h->prm.p == 1 ? launch_limwd<1>(h, B.wout) : launch_limwd<2>(h, B.wout);
+}
+
+int dgswem_end_step(dgswem_t* h) {
+  if (!h) return DGSWEM_E_ARG;
+  if (h->step_dt == 0.0) return h->fail(DGSWEM_E_ARG, "no step in progress (dgswem_begin_step)");
+  h->t = h->t + h->step_dt;
+  h->step_dt = 0.0;
+  h->last_out = h->W[0];
+  return DGSWEM_OK;
+}
+
+int dgswem_set_halo(dgswem_t* h, int64_t n_send, const int32_t* send_ids, int64_t n_recv, const int32_t* recv_ids) {
+  if (!h) return DGSWEM_E_ARG;
+  if (n_send < 0 || n_recv < 0 || (n_send > 0 && !send_ids) || (n_recv > 0 && !recv_ids)) return h->fail(DGSWEM_E_ARG, "bad halo lists");
+  CK(cudaSetDevice(h->prm.device));
+  // caller numbering -> internal numbering (host copy of inv_e)
+  std::vector<int> inv;
+  if (h->inv_e) {
+    inv.resize((size_t)h->ne);
+    CK(cudaMemcpyAsync(inv.data(), h->inv_e, (size_t)h->ne * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+  }
+  auto conv = [&](int64_t n, const int32_t* ids, std::vector<int>& out) -> bool {
+    out.resize((size_t)std::max<int64_t>(n, 1));
+    for (int64_t i = 0; i < n; ++i) {
+      if (ids[i] < 0 || ids[i] >= h->ne) return false;
+      out[(size_t)i] = inv.empty() ? ids[i] : inv[(size_t)ids[i]];
+    }
+    return true;
+  };
+  std::vector<int> snd, rcv;
+  if (!conv(n_send, send_ids, snd) || !conv(n_recv, recv_ids, rcv)) return h->fail(DGSWEM_E_ARG, "halo element id out of range");
+  int r;
+  if ((r = upload(h, h->halo_send, snd))) return r;
+  if ((r = upload(h, h->halo_recv, rcv))) return r;
+  h->n_send = n_send; h->n_recv = n_recv;
+  h->halo_buf = (double*)h->dalloc((size_t)3 * h->ndof * (size_t)std::max<int64_t>(std::max(n_send, n_recv), 1) * sizeof(double));
+  if (!h->halo_buf) return h->fail(DGSWEM_E_CUDA, "device allocation failed");
+  return DGSWEM_OK;
+}
+
+static int halo_rows(const dgswem* h, int what) { return what == 0 ? 3 * h->ndof : 3; }
+
+int dgswem_halo_pack(dgswem_t* h, int what, double* buf, int buf_on_device) {
+  if (!h) return DGSWEM_E_ARG;
+  if ((what != 0 && what != 1) || (!buf && h->n_send > 0)) return h->fail(DGSWEM_E_ARG, "bad halo_pack arguments");
+  if (h->n_send == 0) return DGSWEM_OK;
+  CK(cudaSetDevice(h->prm.device));
+  const int rows = halo_rows(h, what);
+  const double* src = what == 0 ? h->last_out : h->mean;
+  double* dbuf = buf_on_device ? buf : h->halo_buf;
+  k_halo_pack<<<grid_for(h->n_send, 256), 256, 0, h->stream>>>(dbuf, src, h->halo_send, (int)h->n_send, rows);
+  CKL("k_halo_pack");
+  if (!buf_on_device) {
+    CK(cudaMemcpyAsync(buf, dbuf, (size_t)rows * h->n_send * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+  }
+  return DGSWEM_OK;
+}
+
+int dgswem_halo_unpack(dgswem_t* h, int what, const double* buf, int buf_on_device) {
+  if (!h) return DGSWEM_E_ARG;
+  if ((what != 0 && what != 1) || (!buf && h->n_recv > 0)) return h->fail(DGSWEM_E_ARG, "bad halo_unpack arguments");
+  if (h->n_recv == 0) return DGSWEM_OK;
+  CK(cudaSetDevice(h->prm.device));
+  const int rows = halo_rows(h, what);
+  double* dst = what == 0 ? h->last_out : h->mean;
+  const double* dbuf = buf;
+  if (!buf_on_device) {
+    CK(cudaMemcpyAsync(h->halo_buf, buf, (size_t)rows * h->n_recv * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    dbuf = h->halo_buf;
+  }
+  k_halo_unpack<<<grid_for(h->n_recv, 256), 256, 0, h->stream>>>(dst, dbuf, h->halo_recv, (int)h->n_recv, rows);
+  CKL("k_halo_unpack");
+  if (!buf_on_device) CK(cudaStreamSynchronize(h->stream));
+  return DGSWEM_OK;
 }
 
 int dgswem_eval_rhs(dgswem_t* h, double* rze, double* rqx, double* rqy) {

@@ -1,0 +1,179 @@
+"""Domain-decomposed driver on top of the stage-granular C ABI.
+
+One `Dgswem` handle per partition (`partition.py`: owned elements + one layer of ghosts), and per time step
+
+    begin_step;  for every RK stage s:  stage_rhs(s);  [limiter on: exchange means; stage_limit(s)];  exchange state;  end_step
+
+where an exchange is `halo_pack` on the owner, transport, `halo_unpack` on the ghost side.  Every step of the arithmetic
+runs in the library's kernels; this module only orders the calls and moves the packed halo buffers:
+
+  * `LocalTransport`: all partitions live in this process (on one GPU): device-to-device copies between the packed
+    buffers.  This is what the GPU tests run: a partitioned run must reproduce the undivided run bit for bit.
+  * `DistTransport`: one partition per rank of a `torch.distributed` group (NCCL between GPUs over NVLink; gloo with
+    host tensors in the CPU test of the exchange plan): `batch_isend_irecv` of one contiguous slice per neighbour rank.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from .partition import partition, SubMesh
+
+
+class HaloPlan:
+    """Column offsets of every neighbour part in a partition's packed send / receive buffers ([rows][n])."""
+
+    def __init__(self, sub: SubMesh):
+        self.send_ids, self.recv_ids, self.peers, scnt, rcnt = sub.halo_lists()
+        self.send_off, self.recv_off = {}, {}
+        so = ro = 0
+        for q, sc, rc in zip(self.peers, scnt, rcnt):
+            self.send_off[q] = (so, sc); so += sc
+            self.recv_off[q] = (ro, rc); ro += rc
+        self.n_send, self.n_recv = so, ro
+
+
+class LocalTransport:
+    """All partitions in one process: copy each packed slice to its destination's receive buffer."""
+
+    def exchange(self, plans, send_bufs, recv_bufs):
+        for p, plan in enumerate(plans):
+            for q in plan.peers:
+                so, sc = plan.send_off[q]
+                ro, rc = plans[q].recv_off[p]
+                if sc != rc:
+                    raise RuntimeError("halo plans of two partitions disagree")
+                if sc:
+                    recv_bufs[q][:, ro:ro + rc] = send_bufs[p][:, so:so + sc]
+
+
+class DistTransport:
+    """One partition per rank: one isend / irecv per neighbour rank, slices made contiguous per peer."""
+
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        self.dist, self.group = dist, group
+        self.rank = dist.get_rank(group)
+
+    def exchange(self, plans, send_bufs, recv_bufs):
+        # plans / buffers hold only this rank's partition, at index 0
+        plan, snd, rcv = plans[0], send_bufs[0], recv_bufs[0]
+        ops, stage = [], []
+        for q in plan.peers:
+            so, sc = plan.send_off[q]
+            ro, rc = plan.recv_off[q]
+            if sc:
+                s = snd[:, so:so + sc].contiguous()
+                ops.append(self.dist.P2POp(self.dist.isend, s, q, self.group))
+            if rc:
+                r = rcv.new_empty((rcv.shape[0], rc))
+                stage.append((r, ro, rc))
+                ops.append(self.dist.P2POp(self.dist.irecv, r, q, self.group))
+        if ops:
+            for w in self.dist.batch_isend_irecv(ops):
+                w.wait()
+        for r, ro, rc in stage:
+            rcv[:, ro:ro + rc] = r
+
+
+class PartitionedDgswem:
+    """The undivided model's interface (set_state / step / get_state / get_wetdry) on a partitioned mesh.
+
+    parts=None: this process drives every partition (LocalTransport, one GPU).  parts=[r]: this process drives partition r
+    only and `transport` must be a DistTransport whose ranks are the part ids."""
+
+    def __init__(self, params, xy, bathy, tri, edge_elem, edge_local, edge_bc, elem_edge, n_parts, *, tide=None, holland=None,
+                 reorder=1, device=0, parts=None, transport=None, part_of_element=None):
+        import torch
+        from .binding import Dgswem
+        self.torch = torch
+        self.subs = partition(xy, tri, edge_elem, edge_local, edge_bc, elem_edge, n_parts, part=part_of_element)
+        self.mine = list(range(n_parts)) if parts is None else list(parts)
+        self.transport = transport if transport is not None else LocalTransport()
+        self.n_elem = int(np.asarray(tri).shape[0])
+        self.limiter = bool(params["limiter"])
+        self.n_stage = int(params["rk_order"])
+        bathy = np.asarray(bathy, dtype=np.float64)
+        self.handles, self.plans, self.sbuf, self.rbuf = [], [], [], []
+        for p in self.mine:
+            sm = self.subs[p]
+            g = Dgswem(params, sm.xy, bathy[sm.node_gid], sm.tri, sm.edge_elem, sm.edge_local, sm.edge_bc, sm.elem_edge,
+                       reorder=reorder, device=device)
+            if tide is not None:
+                g.set_tide(*tide)
+            if holland is not None:
+                g.set_wind_holland(holland)
+            plan = HaloPlan(sm)
+            g.set_halo(plan.send_ids, plan.recv_ids)
+            rows = g.halo_rows(0)
+            dev = torch.device("cuda", device)
+            self.sbuf.append(torch.empty((rows, max(plan.n_send, 1)), dtype=torch.float64, device=dev))
+            self.rbuf.append(torch.empty((rows, max(plan.n_recv, 1)), dtype=torch.float64, device=dev))
+            self.handles.append(g)
+            self.plans.append(plan)
+        self.ndof = self.handles[0].ndof
+        # LocalTransport indexes plans by part id: only valid when this process drives all parts
+        if parts is not None and isinstance(self.transport, LocalTransport):
+            raise ValueError("driving a subset of the partitions needs a DistTransport")
+
+    # ------------------------------------------------------------------
+    def _exchange(self, what):
+        rows = self.handles[0].halo_rows(what)
+        # contiguous [rows][n_send] / [rows][n_recv] views of the preallocated buffers, as the library packs them
+        snd = [b.view(-1)[:rows * pl.n_send].view(rows, pl.n_send) for b, pl in zip(self.sbuf, self.plans)]
+        rcv = [b.view(-1)[:rows * pl.n_recv].view(rows, pl.n_recv) for b, pl in zip(self.rbuf, self.plans)]
+        for g, pl, s in zip(self.handles, self.plans, snd):
+            if pl.n_send:
+                g.halo_pack(what, s)
+        for g in self.handles:
+            g.sync()
+        self.transport.exchange(self.plans, snd, rcv)
+        self.torch.cuda.synchronize()
+        for g, pl, r in zip(self.handles, self.plans, rcv):
+            if pl.n_recv:
+                g.halo_unpack(what, r)
+        for g in self.handles:
+            g.sync()
+
+    def set_state(self, t, ze, qx, qy):
+        for p, g in zip(self.mine, self.handles):
+            gid = self.subs[p].elem_gid
+            g.set_state(t, np.ascontiguousarray(ze[:, gid]), np.ascontiguousarray(qx[:, gid]), np.ascontiguousarray(qy[:, gid]))
+
+    def step(self, nsteps, dt):
+        for _ in range(int(nsteps)):
+            for g in self.handles:
+                g.begin_step(dt)
+            for s in range(self.n_stage):
+                for g in self.handles:
+                    g.stage_rhs(s)
+                if self.limiter:
+                    self._exchange(1)
+                    for g in self.handles:
+                        g.stage_limit(s)
+                self._exchange(0)
+            for g in self.handles:
+                g.end_step()
+
+    def get_state(self):
+        """(t, ze, qx, qy) of the elements this process owns, scattered into global-size arrays (others stay NaN)."""
+        out = [np.full((self.ndof, self.n_elem), np.nan) for _ in range(3)]
+        t = None
+        for p, g in zip(self.mine, self.handles):
+            sm = self.subs[p]
+            t, *st = g.get_state()
+            own = sm.elem_gid[:sm.n_owned]
+            for c in range(3):
+                out[c][:, own] = st[c][:, :sm.n_owned]
+        return (t, *out)
+
+    def get_wetdry(self):
+        out = np.full(self.n_elem, 255, dtype=np.uint8)
+        for p, g in zip(self.mine, self.handles):
+            sm = self.subs[p]
+            out[sm.elem_gid[:sm.n_owned]] = g.get_wetdry()[:sm.n_owned]
+        return out
+
+    def close(self):
+        for g in self.handles:
+            g.close()
+        self.handles = []

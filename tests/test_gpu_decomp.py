@@ -1,0 +1,81 @@
+"""Domain decomposition: a run split into partitions with one layer of
+ghost elements, stepped through the stage-granular C ABI with a halo exchange per RK stage (and one of the means before
+the limiter pass), must reproduce the undivided run BIT FOR BIT on every owned element -- state, time and wet/dry mask.
+All partitions live on the one GPU of this box (LocalTransport); the multi-rank transport is covered on CPU in
+tests/test_partition.py."""
+import numpy as np
+import pytest
+
+from workloads import c2, c3, c4, c5
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def G():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2508_21208_b200 import build
+    build.build()
+    import paper_2508_21208_b200 as pk
+    return pk
+
+
+CASES = {
+    "c3-tide-wetdry": lambda: c3(nn=40, nsteps=25),
+    "c4-limiter-wind": lambda: c4(nqx=48, nqy=24, nsteps=40),
+    "c5-p2-rk3-all": lambda: c5(nn=30, nsteps=20),
+    "c2-p1-friction": lambda: c2(nq=24, p=1, state="hump", nsteps=20),
+}
+
+
+@pytest.mark.parametrize("fused", ["0", "1"], ids=["edge+elem", "stage"])
+@pytest.mark.parametrize("n_parts", [2, 5])
+@pytest.mark.parametrize("case", sorted(CASES))
+def test_partitioned_run_equals_undivided_run(G, monkeypatch, case, n_parts, fused):
+    from paper_2508_21208_b200.decomp import PartitionedDgswem
+    monkeypatch.setenv("DGSWEM_FUSED", fused)
+    w = CASES[case]()
+    m = w.mesh
+    ref = G.Dgswem.from_workload(w, reorder=1)
+    ref.step(w.nsteps, w.dt)
+    t_ref, *s_ref = ref.get_state()
+    wet_ref = ref.get_wetdry()
+    ref.close()
+    pd = PartitionedDgswem(w.params, m.xy, w.bathy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, n_parts,
+                           tide=w.tide, holland=w.holland)
+    assert sum(s.n_owned for s in pd.subs) == m.n_elem
+    assert all(s.n_local > s.n_owned for s in pd.subs)            # every partition has ghosts
+    pd.set_state(0.0, w.ze, w.qx, w.qy)
+    pd.step(w.nsteps, w.dt)
+    t, *s = pd.get_state()
+    assert t == t_ref
+    for c in range(3):
+        assert np.array_equal(s[c], s_ref[c])
+    assert np.array_equal(pd.get_wetdry(), wet_ref)
+    pd.close()
+
+
+def test_stage_api_equals_dgswem_step_and_rejects_misuse(G):
+    """begin_step / stage_rhs / stage_limit / end_step on an undivided mesh (no halo) is dgswem_step; misuse is an error."""
+    w = c4(nqx=32, nqy=16, nsteps=15)
+    a = G.Dgswem.from_workload(w)
+    b = G.Dgswem.from_workload(w)
+    a.step(15, w.dt)
+    for _ in range(15):
+        b.begin_step(w.dt)
+        for s in range(w.n_stage):
+            b.stage_rhs(s); b.stage_limit(s)
+        b.end_step()
+    for x, y in zip(a.get_state(), b.get_state()):
+        assert np.array_equal(x, y)
+    with pytest.raises(G.DgswemError):
+        b.stage_rhs(0)                      # no step in progress
+    b.begin_step(w.dt)
+    with pytest.raises(G.DgswemError):
+        b.step(1, w.dt)                     # dgswem_step inside a stage-granular step
+    with pytest.raises(G.DgswemError):
+        b.stage_rhs(7)
+    b.end_step()
+    a.close(); b.close()

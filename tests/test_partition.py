@@ -1,0 +1,119 @@
+"""Host-side domain decomposition (paper_2508_21208_b200/partition.py, decomp.py transports): invariants of the
+partitions and halo plans, the library's own mesh validation of every local mesh, and the multi-rank transport on CPU
+(gloo, world_size 2 and 3)."""
+import socket
+import sys
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+def _mesh():
+    from workloads import c3
+    return c3(nn=30)
+
+
+@pytest.mark.parametrize("n_parts", [2, 3, 7])
+def test_partition_invariants(n_parts):
+    from paper_2508_21208_b200.partition import partition
+    w = _mesh(); m = w.mesh
+    subs = partition(m.xy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, n_parts)
+    owned = np.concatenate([s.elem_gid[:s.n_owned] for s in subs])
+    assert np.array_equal(np.sort(owned), np.arange(m.n_elem))             # every element owned exactly once
+    nbr = {}                                                                # edge-neighbours of every element
+    for (a, b) in m.edge_elem:
+        if b >= 0:
+            nbr.setdefault(int(a), set()).add(int(b)); nbr.setdefault(int(b), set()).add(int(a))
+    for s in subs:
+        own = set(s.elem_gid[:s.n_owned].tolist())
+        ghosts = set(s.elem_gid[s.n_owned:].tolist())
+        want = set().union(*[nbr.get(e, set()) for e in own]) - own
+        assert ghosts == want                                               # exactly one layer of edge-neighbours
+        assert np.array_equal(m.tri[s.elem_gid], s.node_gid[s.tri])         # same triangles, same vertex order
+        # local tables are mutually consistent and every owned element's edges keep their global meaning
+        for le in range(s.n_local):
+            for l in range(3):
+                d = s.elem_edge[le, l]
+                side = 0 if (s.edge_elem[d, 0] == le and s.edge_local[d, 0] == l) else 1
+                assert s.edge_elem[d, side] == le and s.edge_local[d, side] == l
+                gd = m.elem_edge[s.elem_gid[le], l]
+                if le < s.n_owned:
+                    ge = m.edge_elem[gd]
+                    if ge[1] >= 0:                                          # interior globally: both sides local, same orientation
+                        assert np.array_equal(s.elem_gid[s.edge_elem[d]], ge) and s.edge_bc[d] == 0
+                    else:
+                        assert s.edge_elem[d, 1] == -1 and s.edge_bc[d] == m.edge_bc[gd]
+        # halo lists: what q sends to p is what p expects from q, element by element
+        for q, ids in s.recv.items():
+            assert np.array_equal(s.elem_gid[ids], subs[q].elem_gid[subs[q].send[s.part]])
+            assert (ids >= s.n_owned).all() and (subs[q].send[s.part] < subs[q].n_owned).all()
+        assert sum(v.size for v in s.recv.values()) == s.n_local - s.n_owned
+
+
+def test_local_meshes_pass_the_library_validation():
+    """dgswem_create validates tables on the host before touching CUDA: every local mesh must get past it."""
+    import ctypes as C
+    import torch
+    from paper_2508_21208_b200 import build, load_library
+    from paper_2508_21208_b200.binding import Params
+    from paper_2508_21208_b200.partition import partition
+    build.build()
+    lib = load_library()
+    w = _mesh(); m = w.mesh
+    prm = w.params
+    P = Params(p=int(prm["p"]), rk_order=int(prm["rk_order"]), g=prm["g"], cf=prm["cf"], coriolis_f=prm["coriolis_f"],
+               h0_dry=prm["h0_dry"], limiter=int(prm["limiter"]), wetdry=int(prm["wetdry"]), reorder=1, device=0)
+    for s in partition(m.xy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, 4):
+        xy = np.ascontiguousarray(s.xy); b = np.ascontiguousarray(w.bathy[s.node_gid])
+        tri = np.ascontiguousarray(s.tri); ee = np.ascontiguousarray(s.edge_elem); el = np.ascontiguousarray(s.edge_local)
+        bc = np.ascontiguousarray(s.edge_bc); eled = np.ascontiguousarray(s.elem_edge)
+        dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double)); ip = lambda a: a.ctypes.data_as(C.POINTER(C.c_int32))
+        h = C.c_void_p()
+        rc = lib.dgswem_create(C.byref(h), C.byref(P), None, xy.shape[0], dp(xy), dp(b), tri.shape[0], ip(tri), ee.shape[0], ip(ee),
+                               el.ctypes.data_as(C.POINTER(C.c_int8)), ip(bc), ip(eled))
+        assert rc == (0 if torch.cuda.is_available() else -3), lib.dgswem_last_error(None)
+        if rc == 0:
+            lib.dgswem_destroy(h)
+
+
+def _free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out_dir):
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, str(ROOT))
+    from paper_2508_21208_b200.partition import partition
+    from paper_2508_21208_b200.decomp import HaloPlan, DistTransport
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    try:
+        w = _mesh(); m = w.mesh
+        sub = partition(m.xy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, world)[rank]
+        plan = HaloPlan(sub)
+        rows = 3
+        # every rank "packs" a code of the global id of each element it sends: row r carries gid * 10 + r
+        gid_s = torch.from_numpy(sub.elem_gid[plan.send_ids].astype(np.float64))
+        snd = torch.stack([gid_s * 10 + r for r in range(rows)])
+        rcv = torch.full((rows, plan.n_recv), -1.0, dtype=torch.float64)
+        DistTransport().exchange([plan], [snd], [rcv])
+        gid_r = torch.from_numpy(sub.elem_gid[plan.recv_ids].astype(np.float64))
+        ok = all(torch.equal(rcv[r], gid_r * 10 + r) for r in range(rows))
+        Path(out_dir, f"rank{rank}.txt").write_text(f"{int(ok)} {plan.n_send} {plan.n_recv}")
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_dist_transport_delivers_every_ghost_gloo(tmp_path, world):
+    import torch.multiprocessing as mp
+    port = _free_port()
+    mp.spawn(_worker, args=(world, port, str(tmp_path)), nprocs=world, join=True)
+    for r in range(world):
+        ok, ns, nr = (tmp_path / f"rank{r}.txt").read_text().split()
+        assert ok == "1" and int(ns) > 0 and int(nr) > 0
