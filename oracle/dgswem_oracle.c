@@ -791,6 +791,31 @@ void orc_get_state(orc_model* m, double* t, double* ze, double* qx, double* qy) 
   memcpy(qy, m->w + 2 * n, sizeof(double) * n);
 }
 
+/* Nodal output ("to output the state variables, we convert the modal representation to a nodal
+ * representation by averaging the neighboring elements of each node"): value of every incident element's polynomial at
+ * the node (basis at the vertices, modes k ascending), summed in ascending element order, divided by the count. */
+void orc_get_nodal(orc_model* m, double* zn, double* qxn, double* qyn) {
+  const int64_t ne = m->n_elem, nn = m->n_nodes;
+  const int ndof = m->T.ndof;
+  double* out[3] = {zn, qxn, qyn};
+  int32_t* cnt = (int32_t*)calloc((size_t)nn, sizeof(int32_t));
+  for (int c = 0; c < 3; ++c) for (int64_t n = 0; n < nn; ++n) out[c][n] = 0.0;
+  for (int64_t e = 0; e < ne; ++e) {
+    for (int v = 0; v < 3; ++v) {
+      const int64_t n = m->tri[3 * e + v];
+      for (int c = 0; c < 3; ++c) {
+        const double* w = m->w + ((int64_t)c * ndof) * ne;
+        double val = w[e];
+        for (int k = 1; k < ndof; ++k) val = fma(w[(int64_t)k * ne + e], m->T.phiV[v][k], val);
+        out[c][n] = out[c][n] + val;
+      }
+      cnt[n] += 1;
+    }
+  }
+  for (int c = 0; c < 3; ++c) for (int64_t n = 0; n < nn; ++n) if (cnt[n] > 0) out[c][n] = out[c][n] / (double)cnt[n];
+  free(cnt);
+}
+
 void orc_get_wetdry(orc_model* m, uint8_t* wet) { memcpy(wet, m->wet, (size_t)m->n_elem); }
 
 void orc_get_geometry(orc_model* m, double* area, double* jinv, double* lfac, double* enx, double* eny) {

@@ -90,6 +90,7 @@ void orc_eval_rhs(orc_model*, double* rze, double* rqx, double* rqy, double* sze
 void orc_get_flux(orc_model*, double* flux /*[3][nqe][n_edge]*/);   /* of the last RHS evaluation */
 void orc_get_state(orc_model*, double* t, double* ze, double* qx, double* qy);
 void orc_get_wetdry(orc_model*, uint8_t* wet);
+void orc_get_nodal(orc_model*, double* zn, double* qxn, double* qyn);   /* [n_nodes] each: element-averaged nodal output */
 void orc_get_geometry(orc_model*, double* area /*[n_elem]*/, double* jinv /*[4][n_elem]*/, double* lfac /*[3][n_elem]*/,
                       double* enx /*[n_edge]*/, double* eny /*[n_edge]*/);
 void orc_get_wind(orc_model*, double* tau /*[2][n_nodes]*/);

@@ -108,6 +108,8 @@ def lib():
     L.orc_get_wetdry.argtypes = [VP, C.POINTER(C.c_uint8)]
     L.orc_get_geometry.argtypes = [VP, PD, PD, PD, PD, PD]
     L.orc_get_wind.argtypes = [VP, PD]
+    L.orc_get_nodal.argtypes = [VP, PD, PD, PD]
+    L.orc_get_nodal.restype = None
     L.orc_num_threads.restype = C.c_int
     _lib = L
     return L
@@ -289,6 +291,11 @@ class Oracle:
         enx = np.zeros(self.n_edge); eny = np.zeros(self.n_edge)
         self.L.orc_get_geometry(self.h, _dp(area), _dp(jinv), _dp(lfac), _dp(enx), _dp(eny))
         return area, jinv, lfac, enx, eny
+
+    def get_nodal(self):
+        out = [np.zeros(self.n_nodes) for _ in range(3)]
+        self.L.orc_get_nodal(self.h, *[_dp(a) for a in out])
+        return out
 
     def get_wind(self):
         tau = np.zeros((2, self.n_nodes))

@@ -321,3 +321,53 @@ def test_wind_moves_with_time_and_enters_rhs_only_when_wet(O):
     o.step(3, w.dt)
     o.eval_rhs()
     assert np.abs(o.get_wind() - tau0).max() > 0
+
+
+def test_nodal_output_pins(O):
+    """orc_get_nodal (averaging the incident elements at every node): a continuous piecewise-linear field is
+    returned exactly as its nodal values (every incident element has that value at the node); a discontinuous one
+    gives the plain mean of the incident elements' vertex values (recomputed here with numpy's scatter-add from the
+    closed-form vertex values u0 = a-b-c, u1 = a-b+c, u2 = a+2b of SURVEY.md 8(c.1)); interior nodes of the regular C1
+    mesh see 6 elements, corner nodes 1 or 2."""
+    from workloads import c1
+    from workloads.configs import _modal
+    w = c1(nq=6)
+    m = w.mesh
+    rng = np.random.default_rng(4)
+    o = O.Oracle.from_workload(w)
+    # (1) continuous linear field per variable
+    f = [lambda x, y: 0.3 + 1e-4 * x - 2e-4 * y, lambda x, y: 1.0 + 3e-4 * x, lambda x, y: -2.0 + 5e-5 * y + 1e-4 * x]
+    nodal = [fi(m.xy[:, 0], m.xy[:, 1]) for fi in f]
+    st = [_modal(nv, m, 1) for nv in nodal]
+    o.set_state(0.0, *st)
+    for got, want in zip(o.get_nodal(), nodal):
+        assert np.abs(got - want).max() <= 1e-13 * np.abs(want).max()
+    # (2) random discontinuous modes against a numpy scatter-add of the closed-form vertex values
+    st = [rng.uniform(-1, 1, (3, m.n_elem)) for _ in range(3)]
+    o.set_state(0.0, *st)
+    _, *st = o.get_state()          # (set_state runs the initial wet/dry pass; compare on what is stored)
+    cnt = np.zeros(m.n_nodes); np.add.at(cnt, m.tri.ravel(), 1.0)
+    assert cnt.max() == 6 and cnt.min() in (1, 2)
+    for got, (a, b, c) in zip(o.get_nodal(), st):
+        verts = np.stack([a - b - c, a - b + c, a + 2 * b], axis=1)      # [n_elem, 3]
+        acc = np.zeros(m.n_nodes); np.add.at(acc, m.tri.ravel(), verts.ravel())
+        assert np.abs(got - acc / cnt).max() <= 1e-14
+
+
+def test_nodal_output_p2_uses_all_six_modes(O):
+    """p = 2: vertex values from the closed-form table of SURVEY.md 8(c.1): phi00=(1,1,1), phi01=(-1,-1,2), phi10=(-1,1,0),
+    phi02=(1,1,3), phi11=(1,-1,0), phi20=(1,1,0)."""
+    from workloads import c2
+    w = c2(nq=6, p=2, state="rest")
+    m = w.mesh
+    rng = np.random.default_rng(8)
+    prm = dict(w.params); prm["wetdry"] = 0
+    o = O.Oracle(prm, m.xy, w.bathy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge)
+    st = [rng.uniform(-1, 1, (6, m.n_elem)) for _ in range(3)]
+    o.set_state(0.0, *st)
+    V = np.array([[1, 1, 1], [-1, -1, 2], [-1, 1, 0], [1, 1, 3], [1, -1, 0], [1, 1, 0]], dtype=np.float64)   # [k][v]
+    cnt = np.zeros(m.n_nodes); np.add.at(cnt, m.tri.ravel(), 1.0)
+    for got, wv in zip(o.get_nodal(), st):
+        verts = wv.T @ V                                             # [n_elem, 3]
+        acc = np.zeros(m.n_nodes); np.add.at(acc, m.tri.ravel(), verts.ravel())
+        assert np.abs(got - acc / cnt).max() <= 1e-13
