@@ -116,6 +116,11 @@ int dgswem_get_state(dgswem_t*, double* t, double* ze, double* qx, double* qy);
 /* Wet (1) / dry (0) flag per element, caller's order. */
 int dgswem_get_wetdry(dgswem_t*, uint8_t* wet);
 
+/* Nodal output ("we convert the modal representation to a nodal representation by averaging the
+ * neighboring elements of each node"): for every node the mean over its incident elements of the element's polynomial
+ * evaluated at that node (summed in ascending caller element id); zn, qxn, qyn: [n_nodes] each, host.  Synchronises. */
+int dgswem_get_nodal(dgswem_t*, double* zn, double* qxn, double* qyn);
+
 /* Nodal kinematic wind stress tau_s/rho_0 of the last WIND evaluation, [2][n_nodes] (test hook). */
 int dgswem_get_wind(dgswem_t*, double* tau);
 

@@ -42,7 +42,7 @@ class DgswemError(RuntimeError):
 
 
 EXPORTS = ["dgswem_create", "dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_step",
-           "dgswem_eval_rhs", "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_wind",
+           "dgswem_eval_rhs", "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_nodal", "dgswem_get_wind",
            "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_limit", "dgswem_end_step", "dgswem_set_halo",
            "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_stage_form", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
 
@@ -72,6 +72,7 @@ def load_library():
     L.dgswem_get_state.argtypes = [VP, PD, PD, PD, PD]
     L.dgswem_get_wetdry.argtypes = [VP, C.POINTER(C.c_uint8)]
     L.dgswem_get_wind.argtypes = [VP, PD]
+    L.dgswem_get_nodal.argtypes = [VP, PD, PD, PD]
     L.dgswem_test_math.argtypes = [VP, I64, PD, PD]
     L.dgswem_begin_step.argtypes = [VP, D]
     L.dgswem_stage_rhs.argtypes = [VP, C.c_int]
@@ -90,7 +91,7 @@ def load_library():
     for name in ("dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_step", "dgswem_eval_rhs",
                  "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_wind", "dgswem_sync",
                  "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_limit", "dgswem_end_step", "dgswem_set_halo",
-                 "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math"):
+                 "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_get_nodal"):
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -219,6 +220,12 @@ class Dgswem:
         wet = np.empty(self.n_elem, dtype=np.uint8)
         self._check(self.L.dgswem_get_wetdry(self.h, wet.ctypes.data_as(C.POINTER(C.c_uint8))))
         return wet
+
+    def get_nodal(self):
+        """Element-averaged nodal values: [zeta, Qx, Qy], each [n_nodes]."""
+        out = [np.empty(self.n_nodes) for _ in range(3)]
+        self._check(self.L.dgswem_get_nodal(self.h, *[_dp(a) for a in out]))
+        return out
 
     def get_wind(self):
         tau = np.empty((2, self.n_nodes))

@@ -173,6 +173,7 @@ struct dgswem {
   int *einfo = nullptr, *elem_edge = nullptr, *nbr = nullptr, *tri = nullptr, *nbinfo = nullptr;
   double* enl = nullptr;
   bool fused = false;         // element-centric stage kernel (k_stage) instead of k_edge + k_elem
+  int *node_ptr = nullptr, *node_ev = nullptr;   // node -> (internal element * 4 + vertex), ascending caller element id
   int *perm_e = nullptr, *inv_e = nullptr, *inv_d = nullptr;   // perm_e[new]=old, inv_e[old]=new, inv_d[old]=new
   unsigned char *wet = nullptr, *wet_stage = nullptr;
   int* nf_flag = nullptr;
@@ -748,6 +749,14 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
       ee[i] = make_int2(inv_e[ep], em >= 0 ? inv_e[em] : -1);
       einfo[i] = lp | (lm << 2) | (edge_bc[d] << 4);
     }
+    // node -> incident (element, vertex) lists for the nodal output, in ascending caller element id
+    std::vector<int> node_ptr(nn + 1, 0), node_ev(3 * ne, 0);
+    for (long long e = 0; e < ne; ++e) for (int v = 0; v < 3; ++v) node_ptr[tri[3 * e + v] + 1]++;
+    for (long long n = 0; n < nn; ++n) node_ptr[n + 1] += node_ptr[n];
+    {
+      std::vector<int> fill(node_ptr.begin(), node_ptr.end() - 1);
+      for (long long e = 0; e < ne; ++e) for (int v = 0; v < 3; ++v) node_ev[fill[tri[3 * e + v]]++] = inv_e[e] * 4 + v;
+    }
     std::vector<double> nxy(2 * ldn, 0.0);
     for (long long i = 0; i < nn; ++i) { nxy[i] = xy[2 * i]; nxy[ldn + i] = xy[2 * i + 1]; }
 
@@ -765,6 +774,8 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     if ((r = upload(h, h->en, en))) return r;
     if ((r = upload(h, h->ehb, ehb))) return r;
     if ((r = upload(h, h->nxy, nxy))) return r;
+    if ((r = upload(h, h->node_ptr, node_ptr))) return r;
+    if ((r = upload(h, h->node_ev, node_ev))) return r;
     if (prm->reorder == 1) {
       if ((r = upload(h, h->perm_e, perm_e))) return r;
       if ((r = upload(h, h->inv_e, inv_e))) return r;
@@ -1066,6 +1077,22 @@ int dgswem_get_wetdry(dgswem_t* h, uint8_t* wet) {
     src = h->wet_stage;
   }
   CK(cudaMemcpyAsync(wet, src, (size_t)h->ne, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return DGSWEM_OK;
+}
+
+int dgswem_get_nodal(dgswem_t* h, double* zn, double* qxn, double* qyn) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!zn || !qxn || !qyn) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
+  CK(cudaSetDevice(h->prm.device));
+  double* out = h->stage_buf;   // [3][ldn] (3 * ldn <= the state-sized staging buffer: n_nodes < n_elem + 3 for any triangulation with a boundary)
+  if ((size_t)3 * h->ldn * sizeof(double) > h->stage_bytes) return h->fail(DGSWEM_E_ARG, "nodal output needs n_nodes <= ndof * n_elem");
+  if (h->prm.p == 1) k_nodal<1><<<grid_for(h->nn, 256), 256, 0, h->stream>>>(out, h->ldn, h->W[0], h->node_ptr, h->node_ev, (int)h->nn);
+  else k_nodal<2><<<grid_for(h->nn, 256), 256, 0, h->stream>>>(out, h->ldn, h->W[0], h->node_ptr, h->node_ev, (int)h->nn);
+  CKL("k_nodal");
+  double* dst[3] = {zn, qxn, qyn};
+  for (int c = 0; c < 3; ++c)
+    CK(cudaMemcpyAsync(dst[c], out + (size_t)c * h->ldn, (size_t)h->nn * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
   return DGSWEM_OK;
 }

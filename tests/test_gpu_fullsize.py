@@ -51,6 +51,8 @@ def full_size_case(O, G, w, nsteps):
         assert np.array_equal(sg[c], sc[c])
     wet_cpu, wet_gpu = o.get_wetdry(), g.get_wetdry()
     assert np.array_equal(wet_gpu, wet_cpu)
+    for a, b in zip(g.get_nodal(), o.get_nodal()):
+        assert np.array_equal(a, b)
     g.close()
     return sg, wet_gpu
 
