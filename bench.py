@@ -244,6 +244,7 @@ def run_decomp(args, rank: int, world: int, local_rank: int):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
     pd.step(args.steps, w.dt)
+    pd.join()                                   # the current stream waits for every partition's stream
     ev1.record()
     barrier()
     ms = max_over_ranks(ev0.elapsed_time(ev1), world, "cuda")

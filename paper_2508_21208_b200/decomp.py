@@ -121,18 +121,32 @@ class PartitionedDgswem:
         # contiguous [rows][n_send] / [rows][n_recv] views of the preallocated buffers, as the library packs them
         snd = [b.view(-1)[:rows * pl.n_send].view(rows, pl.n_send) for b, pl in zip(self.sbuf, self.plans)]
         rcv = [b.view(-1)[:rows * pl.n_recv].view(rows, pl.n_recv) for b, pl in zip(self.rbuf, self.plans)]
+        # stream-ordered, no host synchronisation: pack on each handle's stream -> transport on the current stream
+        # once every pack is done -> unpack on each handle's stream once the transport is done.  (A handle's next pack
+        # comes after its unpack, which has waited for the transport: the buffers are free again by then.)
+        torch = self.torch
+        comm = torch.cuda.current_stream()
         for g, pl, s in zip(self.handles, self.plans, snd):
             if pl.n_send:
                 g.halo_pack(what, s)
-        for g in self.handles:
-            g.sync()
+            ev = torch.cuda.Event()
+            ev.record(g.stream)
+            comm.wait_event(ev)
         self.transport.exchange(self.plans, snd, rcv)
-        self.torch.cuda.synchronize()
+        done = torch.cuda.Event()
+        done.record(comm)
         for g, pl, r in zip(self.handles, self.plans, rcv):
+            g.stream.wait_event(done)
             if pl.n_recv:
                 g.halo_unpack(what, r)
+
+    def join(self):
+        """Make torch's current stream wait for everything enqueued on the partitions' streams (for timing with events)."""
+        comm = self.torch.cuda.current_stream()
         for g in self.handles:
-            g.sync()
+            ev = self.torch.cuda.Event()
+            ev.record(g.stream)
+            comm.wait_event(ev)
 
     def set_state(self, t, ze, qx, qy):
         for p, g in zip(self.mine, self.handles):
