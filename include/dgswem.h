@@ -8,13 +8,17 @@
  *
  * Conventions
  *   - every pointer argument is HOST memory owned by the caller; it is copied in or out during
- *     the call and never retained.  All device memory is owned by the handle.
+ *     the call and never retained (only exception: the halo buffers of dgswem_halo_pack / _unpack when
+ *     flagged buf_on_device).  All other device memory is owned by the handle.
  *   - element arrays are [ndof][n_elem] doubles, mode index slow, in the CALLER's element order
  *     (any internal reordering is invisible); ndof = (p+1)(p+2)/2; mode order 00,01,10,(02,11,20).
  *   - triangles are counter-clockwise, 0-based; local edge l joins local vertices (l+1)%3 -> (l+2)%3.
  *   - return value 0 = success; <0 = error (DGSWEM_E_*), text via dgswem_last_error().
  *   - calls on one handle must not be concurrent.  Work is enqueued on the handle's stream;
  *     get_* calls synchronise it.
+ *   - environment, read by dgswem_create (tuning / test knobs; every setting gives the same bits):
+ *     DGSWEM_FUSED=0/1 form of the RK stage (see dgswem_stage_form), DGSWEM_GRAPH=0 plain stream launches instead of
+ *     CUDA-graph replay in dgswem_step, DGSWEM_PERSISTENT_CTAS=n cap (0: off) on the persistent kernels' grids.
  */
 #ifndef DGSWEM_H
 #define DGSWEM_H
