@@ -118,3 +118,33 @@ def test_create_validates_arguments_and_mesh_on_the_host(lib):
     rc, msg = _raw_create(lib, w)
     import torch
     assert rc == (0 if torch.cuda.is_available() else -3), (rc, msg)
+
+
+def test_create_rejects_null_and_degenerate_sizes(lib):
+    """NULL tables, an empty mesh and out-of-range sizes are argument errors (-1), found before any CUDA call."""
+    import ctypes as C
+    import numpy as np
+    from paper_2508_21208_b200.binding import Params
+    from workloads import c1
+    w = c1(nq=2)
+    m = w.mesh
+    prm = w.params
+    P = Params(p=1, rk_order=2, g=prm["g"], cf=0.0, coriolis_f=0.0, h0_dry=prm["h0_dry"], limiter=0, wetdry=0, reorder=1, device=0)
+    xy = np.ascontiguousarray(m.xy); b = np.ascontiguousarray(w.bathy); tri = np.ascontiguousarray(m.tri, dtype=np.int32)
+    ee = np.ascontiguousarray(m.edge_elem, dtype=np.int32); el = np.ascontiguousarray(m.edge_local, dtype=np.int8)
+    bc = np.ascontiguousarray(m.edge_bc, dtype=np.int32); eled = np.ascontiguousarray(m.elem_edge, dtype=np.int32)
+    dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double)); ip = lambda a: a.ctypes.data_as(C.POINTER(C.c_int32))
+    i8 = el.ctypes.data_as(C.POINTER(C.c_int8))
+    h = C.c_void_p()
+    full = [C.byref(h), C.byref(P), None, m.n_nodes, dp(xy), dp(b), m.n_elem, ip(tri), m.n_edge, ip(ee), i8, ip(bc), ip(eled)]
+    for pos in (1, 4, 5, 7, 9, 10, 11, 12):                       # params and every table pointer
+        a = list(full); a[pos] = None
+        assert lib.dgswem_create(*a) == -1
+    for pos, val in ((3, 2), (6, 0), (8, 2), (6, -5)):            # n_nodes < 3, n_elem < 1, n_edge < 3, negative
+        a = list(full); a[pos] = val
+        assert lib.dgswem_create(*a) == -1
+    assert lib.dgswem_create(None, *full[1:]) == -1               # no place to put the handle
+    # calls on a NULL handle are argument errors, not crashes
+    assert lib.dgswem_step(None, 1, 1.0) == -1 and lib.dgswem_sync(None) == -1 and lib.dgswem_begin_step(None, 1.0) == -1
+    assert lib.dgswem_launch_count(None) == 0 and lib.dgswem_stage_form(None) == 0
+    lib.dgswem_destroy(None)
