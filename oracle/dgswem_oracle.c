@@ -747,6 +747,23 @@ void orc_set_state(orc_model* m, double t, const double* ze, const double* qx, c
   if (m->prm.wetdry) wetdry_all(m, m->w);       /* initialises the wet mask */
 }
 
+/* TEST HOOKS for the pins of limiter_all / wetdry_all (no arithmetic of their own): load a state and wet flags as
+ * given, without the initial wet/dry pass; apply the post-stage sequence SLOPELIM -> WETDRY (either part optional)
+ * to the current state exactly as a stage does. */
+void orc_set_state_raw(orc_model* m, double t, const double* ze, const double* qx, const double* qy, const uint8_t* wet) {
+  const int64_t n = (int64_t)m->T.ndof * m->n_elem;
+  memcpy(m->w, ze, sizeof(double) * n);
+  memcpy(m->w + n, qx, sizeof(double) * n);
+  memcpy(m->w + 2 * n, qy, sizeof(double) * n);
+  m->t = t;
+  memcpy(m->wet, wet, (size_t)m->n_elem);
+}
+
+void orc_apply_post(orc_model* m, int do_limiter, int do_wetdry) {
+  if (do_limiter) limiter_all(m, m->w);
+  if (do_wetdry) wetdry_all(m, m->w);
+}
+
 void orc_set_tide(orc_model* m, double amp, double omega, double phase) {
   m->tide_amp = amp; m->tide_omega = omega; m->tide_phase = phase;
 }

@@ -81,6 +81,9 @@ orc_model* orc_create(const orc_params* prm,
 void orc_destroy(orc_model*);
 const orc_tables* orc_get_tables(const orc_model*);
 void orc_set_state(orc_model*, double t, const double* ze, const double* qx, const double* qy);
+/* test hooks: state + wet flags as given (no initial wet/dry pass); the post-stage sequence limiter -> wet/dry on the current state */
+void orc_set_state_raw(orc_model*, double t, const double* ze, const double* qx, const double* qy, const uint8_t* wet);
+void orc_apply_post(orc_model*, int do_limiter, int do_wetdry);
 void orc_set_tide(orc_model*, double amp, double omega, double phase);
 void orc_set_wind_holland(orc_model*, const orc_holland* /* NULL = off */);
 void orc_step(orc_model*, int64_t nsteps, double dt);

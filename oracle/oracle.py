@@ -99,6 +99,8 @@ def lib():
     L.orc_destroy.argtypes = [VP]
     L.orc_get_tables.argtypes = [VP]; L.orc_get_tables.restype = C.POINTER(Tables)
     L.orc_set_state.argtypes = [VP, D, PD, PD, PD]
+    L.orc_set_state_raw.argtypes = [VP, D, PD, PD, PD, C.POINTER(C.c_uint8)]
+    L.orc_apply_post.argtypes = [VP, C.c_int, C.c_int]
     L.orc_set_tide.argtypes = [VP, D, D, D]
     L.orc_set_wind_holland.argtypes = [VP, C.POINTER(Holland)]
     L.orc_step.argtypes = [VP, I64, D]
@@ -246,6 +248,17 @@ class Oracle:
     def set_state(self, t, ze, qx, qy):
         ze, qx, qy = self._chk(ze), self._chk(qx), self._chk(qy)
         self.L.orc_set_state(self.h, float(t), _dp(ze), _dp(qx), _dp(qy))
+
+    def set_state_raw(self, t, ze, qx, qy, wet):
+        """Test hook: state and wet flags as given, no initial wet/dry pass."""
+        ze, qx, qy = self._chk(ze), self._chk(qx), self._chk(qy)
+        wet = np.ascontiguousarray(wet, dtype=np.uint8)
+        assert wet.shape == (self.n_elem,)
+        self.L.orc_set_state_raw(self.h, float(t), _dp(ze), _dp(qx), _dp(qy), wet.ctypes.data_as(C.POINTER(C.c_uint8)))
+
+    def apply_post(self, limiter=True, wetdry=True):
+        """Test hook: the post-stage sequence SLOPELIM -> WETDRY on the current state."""
+        self.L.orc_apply_post(self.h, int(bool(limiter)), int(bool(wetdry)))
 
     def set_tide(self, amp, omega, phase):
         self.L.orc_set_tide(self.h, amp, omega, phase)

@@ -6,7 +6,7 @@ tests/test_partition.py."""
 import numpy as np
 import pytest
 
-from workloads import c2, c3, c4, c5
+from workloads import c2, c3, c4, c5, perturbed
 
 pytestmark = pytest.mark.gpu
 
@@ -23,6 +23,7 @@ def G():
 
 
 CASES = {
+    "c3-nonzero-state": lambda: perturbed(c3(nn=40, nsteps=25)),
     "c3-tide-wetdry": lambda: c3(nn=40, nsteps=25),
     "c4-limiter-wind": lambda: c4(nqx=48, nqy=24, nsteps=40),
     "c5-p2-rk3-all": lambda: c5(nn=30, nsteps=20),
@@ -33,11 +34,16 @@ CASES = {
 @pytest.mark.parametrize("fused", ["0", "1"], ids=["edge+elem", "stage"])
 @pytest.mark.parametrize("n_parts", [2, 5])
 @pytest.mark.parametrize("case", sorted(CASES))
-def test_partitioned_run_equals_undivided_run(G, monkeypatch, case, n_parts, fused):
+def test_partitioned_run_equals_undivided_run(O, G, monkeypatch, case, n_parts, fused):
+    """... and the ORACLE's run, directly (not only transitively through the undivided GPU run)."""
     from paper_2508_21208_b200.decomp import PartitionedDgswem
     monkeypatch.setenv("DGSWEM_FUSED", fused)
     w = CASES[case]()
     m = w.mesh
+    o = O.Oracle.from_workload(w)
+    o.step(w.nsteps, w.dt)
+    t_orc, *s_orc = o.get_state()
+    wet_orc = o.get_wetdry()
     ref = G.Dgswem.from_workload(w, reorder=1)
     ref.step(w.nsteps, w.dt)
     t_ref, *s_ref = ref.get_state()
@@ -54,6 +60,9 @@ def test_partitioned_run_equals_undivided_run(G, monkeypatch, case, n_parts, fus
     for c in range(3):
         assert np.array_equal(s[c], s_ref[c])
     assert np.array_equal(pd.get_wetdry(), wet_ref)
+    assert t == t_orc and np.array_equal(pd.get_wetdry(), wet_orc)
+    for c in range(3):
+        assert np.array_equal(s[c], s_orc[c])
     pd.close()
 
 

@@ -8,7 +8,7 @@ runs are covered on the small meshes of test_gpu_parity.py.
 import numpy as np
 import pytest
 
-from workloads import c2, c3, c4, c5
+from workloads import c2, c3, c4, c5, perturbed
 
 pytestmark = pytest.mark.gpu
 
@@ -63,6 +63,25 @@ def test_c3_full_size(O, G):
     assert w.mesh.n_elem == 4_494_002
     sg, _ = full_size_case(O, G, w, 3)
     assert np.abs(sg[0]).max() > 0
+
+
+def test_c3_full_size_nonzero_state(O, G):
+    """The bench workload's mesh, tide and launch configuration on NON-ZERO data: smooth waves plus seeded noise in all
+    three modes of zeta, Qx, Qy (0.3 m / 1 m2/s) in every element, so the 4.49 M-element permuted neighbour gather,
+    the Hilbert renumbering and every mode are compared on values that differ from element to element (from rest,
+    3 steps move only the east boundary column).  RHS, flux buffer, state, mask and nodal output bit for bit."""
+    w = perturbed(c3())
+    assert w.mesh.n_elem == 4_494_002
+    assert min(np.abs(a).min() for a in (w.ze, w.qx, w.qy)) > 0
+    sg, _ = full_size_case(O, G, w, 3)
+    assert all(np.abs(a).min() > 0 for a in sg)
+
+
+def test_c5_full_size_nonzero_quadratic_modes(O, G):
+    """BASELINE configs[4] with all six modes populated offshore (the recipe starts with zero quadratic modes)."""
+    w = perturbed(c5(), amp_z=0.2)
+    assert np.abs(w.ze[3:]).max() > 1e-3
+    full_size_case(O, G, w, 2)
 
 
 def test_c4_full_size(O, G):

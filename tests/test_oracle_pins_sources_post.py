@@ -1,0 +1,390 @@
+"""Pins for the parts of the oracle that round 1 left unpinned: the bottom-friction term
+(eq. (1) tau_b; R-6), the wiring of limiter_all / wetdry_all (
+R-7, R-8), the depth ramp of the wind stress (R-9) and the p = 2 wet/dry pre-step with its threshold H1 = 10 H0
+(R-8).  Every expected value is computed here in numpy from the closed forms of SURVEY.md 8(c) and from the
+mesh's own tables, never from the oracle's intermediate results."""
+import math
+
+import numpy as np
+import pytest
+
+from helpers import G, brute_force_rhs, eval_basis, l2_project, small_mesh
+from workloads import default_params
+from workloads.mesh import rect_mesh
+
+
+def make_oracle(O, mesh, bathy, **kw):
+    prm = default_params(**kw)
+    return O.Oracle(prm, mesh.xy, bathy, mesh.tri, mesh.edge_elem, mesh.edge_local, mesh.edge_bc, mesh.elem_edge)
+
+
+# ------------------------------------------------------------------ (a) bottom friction
+@pytest.mark.parametrize("p", [1, 2])
+def test_friction_uniform_flow_closed_form(O, p):
+    """Uniform flow (zeta, Qx, Qy) = const over a flat bottom: in an element without a wall edge the flux terms cancel
+    (divergence theorem, exact quadrature of a constant), so d(mean Q)/dt is the source alone:
+        rhs(Qx)_00 = -C_f |Q| Qx / H^2 + f Qy,   rhs(Qy)_00 = -C_f |Q| Qy / H^2 - f Qx      (eq. (1), R-6)
+    and every other mode of every variable is 0 (a constant source has no projection on phi_k, k >= 1)."""
+    mesh = small_mesh(nq=5)
+    ndof = (p + 1) * (p + 2) // 2
+    hb, z, qx, qy, cf, f = 12.0, 0.7, 3.0, -2.0, 0.04, 3e-3
+    o = make_oracle(O, mesh, np.full(mesh.n_nodes, hb), p=p, cf=cf, coriolis_f=f)
+    st = np.zeros((3, ndof, mesh.n_elem)); st[0, 0] = z; st[1, 0] = qx; st[2, 0] = qy
+    o.set_state(0.0, *st)
+    r = np.stack(o.eval_rhs())
+    interior = ~(mesh.edge_bc[mesh.elem_edge] != 0).any(axis=1)
+    assert interior.sum() > 10
+    H = z + hb
+    tau = cf * math.hypot(qx, qy) / H ** 2
+    ex_x, ex_y = -tau * qx + f * qy, -tau * qy - f * qx
+    assert abs(tau * qx) > 1e-3 and abs(tau * qx) > 0.1 * abs(f * qy)   # the friction term is not negligible
+    scale = max(abs(ex_x), abs(ex_y))
+    # the edge and volume flux terms cancel to round-off of THEIR size, (g H^2/2) L/A ~ 30: absolute floor of the comparison
+    lfmax = np.abs(o.get_geometry()[2]).max()
+    cancel = 2e-15 * (G * H * H) * lfmax
+    assert cancel < 1e-9 * scale
+    assert np.abs(r[1, 0, interior] - ex_x).max() <= 1e-13 * scale + cancel
+    assert np.abs(r[2, 0, interior] - ex_y).max() <= 1e-13 * scale + cancel
+    assert np.abs(r[0][:, interior]).max() <= cancel
+    assert np.abs(r[1:, 1:][:, :, interior]).max() <= cancel
+    # the law itself: quadratic in |Q|, inverse square in H (a wrong power of H_c or a missing |Q| fails here)
+    for zz, s in ((0.7, 2.0), (6.0, 1.0)):
+        st2 = np.zeros_like(st); st2[0, 0] = zz; st2[1, 0] = s * qx; st2[2, 0] = s * qy
+        o.set_state(0.0, *st2)
+        r2 = np.stack(o.eval_rhs())
+        H2 = zz + hb
+        tau2 = cf * s * math.hypot(qx, qy) / H2 ** 2
+        assert np.abs(r2[1, 0, interior] - (-tau2 * s * qx + f * s * qy)).max() <= 1e-13 * scale * 4 + 2e-15 * G * H2 * H2 * lfmax
+
+
+def test_friction_off_in_dry_flagged_elements_and_cf_zero(O):
+    """R-6: friction acts only where the wet flag is 1; C_f = 0 leaves the Coriolis source alone."""
+    mesh = small_mesh(nq=5)
+    hb = 12.0
+    o = make_oracle(O, mesh, np.full(mesh.n_nodes, hb), p=1, cf=0.04)
+    st = np.zeros((3, 3, mesh.n_elem)); st[0, 0] = 0.7; st[1, 0] = 3.0; st[2, 0] = -2.0
+    interior = np.flatnonzero(~(mesh.edge_bc[mesh.elem_edge] != 0).any(axis=1))
+    wet = np.ones(mesh.n_elem, dtype=np.uint8); wet[interior[::2]] = 0
+    o.set_state_raw(0.0, *st, wet)
+    r = np.stack(o.eval_rhs())
+    tau = 0.04 * math.hypot(3.0, 2.0) / 12.7 ** 2
+    assert np.abs(r[1, 0, interior[1::2]] + tau * 3.0).max() <= 1e-15
+    assert np.abs(r[1, 0, interior[::2]]).max() <= 1e-12          # flagged dry: no friction at all
+    o0 = make_oracle(O, mesh, np.full(mesh.n_nodes, hb), p=1, cf=0.0, coriolis_f=2e-3)
+    o0.set_state(0.0, *st)
+    r0 = np.stack(o0.eval_rhs())
+    assert np.abs(r0[1, 0, interior] - 2e-3 * (-2.0)).max() <= 1e-12
+    assert np.abs(r0[2, 0, interior] + 2e-3 * 3.0).max() <= 1e-12
+
+
+@pytest.mark.parametrize("p", [1, 2])
+def test_bruteforce_with_strong_friction(O, p):
+    """Brute-force weak form (dense mass solve, 12x12 rule) with C_f = 0.25, where friction is the same size as the
+    pressure terms: the oracle agrees within its quadrature error, and the same comparison against a friction-free
+    brute force misses that tolerance by more than 10x -- i.e. this pin fails if the friction term is dropped
+    (round 1's C_f = 0.0025 case passed with the term deleted)."""
+    mesh = small_mesh(nq=2, L=1000.0, ocean=True)
+    rng = np.random.default_rng(8)
+    bathy = 3.0 + 0.5 * rng.uniform(-1, 1, mesh.n_nodes)
+    ndof = (p + 1) * (p + 2) // 2
+    W = [l2_project(O, mesh, lambda x, y: 0.1 * np.sin(2e-3 * x) * np.cos(1e-3 * y), p),
+         l2_project(O, mesh, lambda x, y: 3.0 + 1.0 * np.cos(1e-3 * x + 2e-3 * y), p),
+         l2_project(O, mesh, lambda x, y: -2.0 + 0.5 * np.sin(2e-3 * x - 1e-3 * y), p)]
+    for c in range(3):
+        W[c] = W[c] + (0.01 if c == 0 else 0.05) * rng.uniform(-1, 1, (ndof, mesh.n_elem)) * (np.arange(ndof)[:, None] < 3)
+    cf = 0.25
+    o = make_oracle(O, mesh, bathy, p=p, cf=cf, coriolis_f=1e-2)
+    o.set_tide(0.1, 0.0, np.pi / 2)
+    o.set_state(0.0, *W)
+    r = np.stack(o.eval_rhs())
+    bf = brute_force_rhs(O, mesh, bathy, p, *W, cf=cf, fcor=1e-2, zeta_b=0.1)
+    bf0 = brute_force_rhs(O, mesh, bathy, p, *W, cf=0.0, fcor=1e-2, zeta_b=0.1)
+    tol = 5e-3 if p == 1 else 2e-3
+    for c in (1, 2):
+        sc = np.abs(bf[c]).max()
+        assert np.abs(r[c] - bf[c]).max() < tol * sc
+        assert np.abs(r[c] - bf0[c]).max() > 10 * tol * sc           # dropping friction would be seen
+    # a wrong power of H_c (|Q|/H instead of |Q|/H^2: a factor H ~ 3) or a missing |Q| (~ 3.6) would be seen as well
+    mean_tau = cf * math.hypot(3.0, 2.0) / 3.0 ** 2
+    assert np.abs((bf - bf0)[1, 0]).mean() > 0.5 * mean_tau * 3.0
+
+
+# ------------------------------------------------------------------ (b) limiter_all / wetdry_all wiring
+def _np_limit(w3, nb_means):
+    """SURVEY.md 8(c.2) in numpy: edge-neighbour Barth-Jespersen on (a, b, c); returns alpha."""
+    a, b, c = w3
+    umin, umax = min([a] + nb_means), max([a] + nb_means)
+    alpha = 1.0
+    for d in (-b - c, -b + c, 2 * b):
+        if d > 0:
+            alpha = min(alpha, (umax - a) / d)
+        elif d < 0:
+            alpha = min(alpha, (umin - a) / d)
+    return alpha
+
+
+def _neighbours(mesh, e):
+    """Edge neighbours of element e from the mesh's own tables (NEDEL/LED)."""
+    out = []
+    for l in range(3):
+        d = mesh.elem_edge[e, l]
+        ep, em = mesh.edge_elem[d]
+        out.append(int(em if ep == e else ep))
+    return out          # -1 across a boundary edge
+
+
+def _post_case(O, p=1, seed=21):
+    mesh = small_mesh(nq=2, L=1000.0, seed=seed)                       # 8 elements, jittered, permuted
+    rng = np.random.default_rng(seed)
+    bathy = 5.0 + 1.0 * rng.uniform(-1, 1, mesh.n_nodes)
+    ndof = (p + 1) * (p + 2) // 2
+    st = np.zeros((3, ndof, mesh.n_elem))
+    st[0, 0] = 0.3 + 0.2 * rng.uniform(-1, 1, mesh.n_elem)
+    st[1, 0] = 1.0 + 0.8 * rng.uniform(-1, 1, mesh.n_elem)
+    st[2, 0] = -0.5 + 0.8 * rng.uniform(-1, 1, mesh.n_elem)
+    st[:, 1:3] = 0.3 * rng.uniform(-1, 1, (3, 2, mesh.n_elem))          # slopes large enough that the limiter binds
+    if p == 2:
+        st[:, 3:] = 0.05 * rng.uniform(-1, 1, (3, 3, mesh.n_elem))
+    return mesh, bathy, st
+
+
+@pytest.mark.parametrize("p", [1, 2])
+def test_limiter_all_neighbour_wiring_wet_gate_and_means(O, p):
+    """limiter_all on a hand-built 8-element state: alpha of every (element, variable) recomputed here from the mesh's
+    own edge tables and the pre-limit means; an element flagged dry must be skipped (its slopes survive); means are
+    never changed (so the in-place sweep is the Jacobi sweep: there is no pre-/post-limit distinction to get wrong);
+    boundary sides contribute no neighbour."""
+    mesh, bathy, st = _post_case(O, p)
+    o = make_oracle(O, mesh, bathy, p=p, limiter=1, wetdry=1)
+    wet = np.ones(mesh.n_elem, dtype=np.uint8)
+    dry_e = 3
+    wet[dry_e] = 0
+    o.set_state_raw(0.0, *st, wet)
+    o.apply_post(limiter=True, wetdry=False)
+    _, *out = o.get_state()
+    out = np.stack(out)
+    assert np.array_equal(out[:, 0], st[:, 0])                          # means untouched
+    assert np.array_equal(out[:, :, dry_e], st[:, :, dry_e])            # dry element skipped entirely
+    n_bind = n_bnd = 0
+    for e in range(mesh.n_elem):
+        if e == dry_e:
+            continue
+        nbs = _neighbours(mesh, e)
+        n_bnd += sum(1 for n in nbs if n < 0)
+        for c in range(3):
+            alpha = _np_limit(st[c, :3, e], [st[c, 0, n] for n in nbs if n >= 0])
+            n_bind += alpha < 1.0
+            assert np.abs(out[c, 1:3, e] - alpha * st[c, 1:3, e]).max() <= 1e-15
+            if p == 2:
+                want = np.zeros(3) if alpha < 1.0 else st[c, 3:, e]
+                assert np.array_equal(out[c, 3:, e], want)
+    assert n_bind >= 8 and n_bnd >= 4
+    # a neighbour of the dry element still uses the dry element's mean (the gate is on the element, not the neighbour)
+    assert any(dry_e in _neighbours(mesh, e) for e in range(mesh.n_elem) if e != dry_e)
+    # wrong wiring would be seen: limiting against a rolled neighbour table gives different alphas somewhere
+    diff = 0
+    for e in range(mesh.n_elem):
+        nbs = [n for n in _neighbours(mesh, (e + 1) % mesh.n_elem) if n >= 0 and n != e]
+        a_wrong = _np_limit(st[0, :3, e], [st[0, 0, n] for n in nbs])
+        a_right = _np_limit(st[0, :3, e], [st[0, 0, n] for n in _neighbours(mesh, e) if n >= 0])
+        diff += abs(a_wrong - a_right) > 1e-6
+    assert diff >= 3
+
+
+def test_post_sequence_limiter_reads_means_before_this_stages_wetdry(O):
+    """Order RK -> SLOPELIM (all elements) -> WETDRY (all elements), R-7/R-8: the limiter of element E sees the momentum
+    mean its neighbour N had BEFORE this stage's wet/dry pass empties N; the wet flag that gates the limiter is the
+    previous stage's; the wet/dry pass then runs on the limited state and rewrites the flags."""
+    mesh, bathy, st = _post_case(O, 1, seed=22)
+    h0 = 1e-3
+    N = 5
+    # element N: flagged wet by the previous stage, but its RK-updated depth is below H0 everywhere -> this stage's
+    # wet/dry pass makes it dry and zeroes its momentum (mean included)
+    hvN = bathy[mesh.tri[N]]
+    u = 0.3 * h0 - hvN
+    a = u.sum() / 3
+    st[0, :, N] = [a, 0.5 * (u[2] - a), 0.5 * (u[1] - u[0])]
+    st[1, 0, N] = 40.0                                                  # a large pre-wet/dry momentum mean: it sets u_max
+    o = make_oracle(O, mesh, bathy, p=1, limiter=1, wetdry=1, h0_dry=h0)
+    wet = np.ones(mesh.n_elem, dtype=np.uint8)
+    D = 1                                                               # flagged dry, but deep: limiter skipped, wet/dry re-wets it
+    assert D != N and D not in _neighbours(mesh, N)
+    wet[D] = 0
+    o.set_state_raw(0.0, *st, wet)
+    o.apply_post(limiter=True, wetdry=True)
+    _, *out = o.get_state()
+    out = np.stack(out)
+    wet_out = o.get_wetdry()
+    touched = 0
+    for e in range(mesh.n_elem):
+        nbs = _neighbours(mesh, e)
+        lim = st[:, :, e].copy()
+        if wet[e]:
+            for c in range(3):
+                lim[c, 1:3] *= _np_limit(st[c, :3, e], [st[c, 0, n] for n in nbs if n >= 0])   # PRE-wet/dry means
+        wflag, z2, x2, y2 = O.wetdry_elem(1, h0, bathy[mesh.tri[e]], lim[0], lim[1], lim[2])    # pinned separately
+        assert wet_out[e] == wflag
+        assert np.abs(out[:, :, e] - np.stack([z2, x2, y2])).max() <= 1e-15
+        if N in nbs:
+            # with N's post-wet/dry mean (0) instead of 40 the bound u_max would differ: make sure that matters
+            a_pre = _np_limit(st[1, :3, e], [st[1, 0, n] for n in nbs if n >= 0])
+            a_post = _np_limit(st[1, :3, e], [0.0 if n == N else st[1, 0, n] for n in nbs if n >= 0])
+            touched += abs(a_pre - a_post) > 1e-3
+    assert touched >= 1
+    assert wet_out[N] == 0 and not out[1:, :, N].any()
+    assert wet_out[D] == 1 and np.array_equal(out[0, :, D], st[0, :, D])   # skipped by the limiter, deep: re-flagged wet
+
+
+def test_limiter_in_model_only_wet_elements_and_means_fixed(O):
+    """Through the model (C4 recipe, small): a step with the limiter on differs from a step with it off only in wet
+    elements' higher modes... and conserves every mean that the wet/dry pass does not touch: checked by running the
+    same step with and without limiter from the same state and comparing the stage-1 means through the RHS hook."""
+    from workloads import c4
+    w = c4(nqx=16, nqy=8, nsteps=5)
+    o = O.Oracle.from_workload(w)
+    prm = dict(w.params); prm["limiter"] = 0
+    m = w.mesh
+    o2 = O.Oracle(prm, m.xy, w.bathy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge)
+    o2.set_wind_holland(w.holland)
+    o2.set_state(0.0, w.ze, w.qx, w.qy)
+    # identical states and flags -> identical RHS whatever the limiter switch
+    assert all(np.array_equal(a, b) for a, b in zip(o.eval_rhs(), o2.eval_rhs()))
+    # post sequence on the same non-trivial state: run 3 steps without limiter, hand the state to both
+    o2.step(3, w.dt)
+    t, *s3 = o2.get_state()
+    wet3 = o2.get_wetdry()
+    assert (wet3 == 0).sum() > 5 and (wet3 == 1).sum() > 50
+    o.set_state_raw(t, *s3, wet3)
+    o.apply_post(limiter=True, wetdry=False)
+    _, *lim = o.get_state()
+    s3, lim = np.stack(s3), np.stack(lim)
+    assert np.array_equal(lim[:, 0], s3[:, 0])                          # means fixed
+    assert np.array_equal(lim[:, :, wet3 == 0], s3[:, :, wet3 == 0])    # dry elements untouched
+    changed = (lim != s3).any(axis=(0, 1))
+    assert changed.any() and not changed[wet3 == 0].any()
+    # every limited vertex value lies between the extrema of the element's and its neighbours' means
+    for e in np.flatnonzero(changed)[:40]:
+        nbs = [n for n in _neighbours(m, int(e)) if n >= 0]
+        for c in range(3):
+            a, b, cc = lim[c, :, e]
+            lo = min([s3[c, 0, e]] + [s3[c, 0, n] for n in nbs]); hi = max([s3[c, 0, e]] + [s3[c, 0, n] for n in nbs])
+            v = np.array([a - b - cc, a - b + cc, a + 2 * b])
+            tol = 1e-12 * max(1.0, abs(hi), abs(lo))
+            assert (v <= hi + tol).all() and (v >= lo - tol).all()
+
+
+# ------------------------------------------------------------------ (c) wind depth ramp
+def test_wind_stress_depth_ramp_between_h0_and_10h0(O):
+    """R-9: the wind stress at an area point is the linear interpolant of the nodal stress times
+    ramp = clamp((H - H0)/(9 H0), 0, 1).  One mesh whose elements sit at depths on both sides of and INSIDE the ramp:
+    expected modal contributions  d rhs(Q)_k = sum_i wa_i/M_k phi_k(x_i) ramp(H_i) tau(x_i)  with the 3-point rule
+    (points lambda = (2/3,1/6,1/6) and permutations, wa = 2/3, M = (2, 1, 1/3)); phi from SURVEY 8(c.1) closed forms."""
+    h0 = 1e-3
+    mesh = rect_mesh(6, 4, 6000.0, 4000.0, diag="same")
+    bathy = np.full(mesh.n_nodes, 0.0)
+    # nodal depth field: 0.2 H0 in the first column of cells (no stress), through the ramp, to 30 H0 (full stress)
+    Hn = h0 * np.maximum(0.2, -6.0 + 36.0 * mesh.xy[:, 0] / 6000.0)
+    zn = Hn - bathy
+    tri = mesh.tri
+    u = zn[tri]                                                         # [ne, 3] vertex values
+    a = u.sum(1) / 3
+    ze = np.stack([a, 0.5 * (u[:, 2] - a), 0.5 * (u[:, 1] - u[:, 0])])
+    hol = dict(x0=-20e3, y0=2000.0, vx=0.0, vy=0.0, rmax=40e3, dp=6000.0, B=1.5, rho_air=1.15, rho_water=1025.0, f=5e-5)
+    o = make_oracle(O, mesh, bathy, p=1, wetdry=1, h0_dry=h0)
+    wet = np.ones(mesh.n_elem, dtype=np.uint8)
+    o.set_state_raw(0.0, ze, 0 * ze, 0 * ze, wet)
+    o.set_wind_holland(hol)
+    r1 = np.stack(o.eval_rhs())
+    tau = o.get_wind()                                                  # nodal stress (pinned by test_holland_closed_forms)
+    o.set_wind_holland(None)
+    r0 = np.stack(o.eval_rhs())
+    d = r1 - r0
+    assert not d[0].any()                                               # no wind term in the continuity equation
+    lam = np.array([[2 / 3, 1 / 6, 1 / 6], [1 / 6, 2 / 3, 1 / 6], [1 / 6, 1 / 6, 2 / 3]])
+    phi = np.stack([np.ones(3), 3 * lam[:, 2] - 1, 2 * lam[:, 1] + lam[:, 2] - 1], axis=1)   # [i, k]
+    Mk = np.array([2.0, 1.0, 1.0 / 3.0])
+    Hq = (Hn[tri] @ lam.T)                                              # [ne, i]
+    ramp = np.clip((Hq - h0) / (9 * h0), 0.0, 1.0)
+    inside = ((ramp > 0.05) & (ramp < 0.95)).any(axis=1)
+    assert inside.sum() >= 6 and (ramp == 0).all(axis=1).any() and (ramp == 1).all(axis=1).any()
+    for c in (0, 1):
+        tq = tau[c][tri] @ lam.T                                        # [ne, i]
+        ex = np.einsum("ei,ik->ke", (2 / 3) * ramp * tq, phi) / Mk[:, None]
+        sc = np.abs(ex).max()
+        assert sc > 1e-6
+        assert np.abs(d[1 + c] - ex).max() <= 1e-11 * sc, c
+    # and a dry-flagged element takes none of it whatever its depth
+    wet[:] = 1; wet[inside.argmax()] = 0
+    o.set_state_raw(0.0, ze, 0 * ze, 0 * ze, wet)
+    o.set_wind_holland(hol)
+    r1b = np.stack(o.eval_rhs())
+    assert np.array_equal(r1b[:, :, inside.argmax()], r0[:, :, inside.argmax()])
+
+
+# ------------------------------------------------------------------ (d) p = 2 wet/dry pre-step
+def _p2_modes_with_min_at(O, lam_x, hmin, hv, K=3.0):
+    """zeta modes (6) of the quadratic  H(lambda) = hmin + K |xi - xi_X|^2  over the bathymetry plane hv."""
+    nodes = np.array([[1, 0, 0], [0, 1, 0], [0, 0, 1], [0, .5, .5], [.5, 0, .5], [.5, .5, 0]], dtype=float)
+    xi = lambda l: np.stack([2 * l[..., 1] - 1, 2 * l[..., 2] - 1], -1)
+    d2 = ((xi(nodes) - xi(np.asarray(lam_x, dtype=float))) ** 2).sum(-1)
+    zeta_nodes = hmin + K * d2 - nodes @ hv
+    V = eval_basis(O, nodes)                                            # [6 nodes, 6 modes] (basis pinned in test_oracle_tables)
+    return np.linalg.solve(V, zeta_nodes)
+
+
+def _p2_points(O):
+    T = O.tables(2)
+    la, elam = T.np("la"), T.np("elam")
+    pts = {"vertex": [np.eye(3)[v] for v in range(3)], "edge": [], "area": [la[i] for i in range(6)]}
+    for l in range(3):
+        a, b = (l + 1) % 3, (l + 2) % 3
+        for j in range(3):
+            lam = np.zeros(3); lam[a] = elam[j][0]; lam[b] = elam[j][1]
+            pts["edge"].append(lam)
+    return pts
+
+
+@pytest.mark.parametrize("where,idx", [("vertex", 1), ("edge", 4), ("edge", 7), ("area", 2), ("area", 5)])
+def test_p2_wetdry_prestep_threshold_and_point_sets(O, where, idx):
+    """R-8 pre-step: the full quadratic depth is examined at the 3 vertices, the 9 edge points and the 6 area points;
+    modes 3-5 of ALL variables are zeroed iff some point depth is <= H1 = 10 H0.  A depth of 5 H0 at exactly one
+    point of one set (all 17 others deeper than 60 H0) must trigger it -- with the survey's threshold H0 it would
+    not, and a loop that skipped that point set would miss it; 11 H0 at the same point must not."""
+    h0 = 1e-3
+    hv = np.array([1.0, 1.2, 0.9])
+    pts = _p2_points(O)
+    X = pts[where][idx]
+    q6 = np.array([1.0, 0.1, 0.1, 0.2, 0.2, 0.2])
+    allpts = np.array(pts["vertex"] + pts["edge"] + pts["area"])
+    for hmin, zeroed in ((5 * h0, True), (11 * h0, False)):
+        ze = _p2_modes_with_min_at(O, X, hmin, hv)
+        depth = eval_basis(O, allpts) @ ze + allpts @ hv
+        order = np.sort(depth)
+        assert abs(order[0] - hmin) < 1e-12 and order[1] > 60 * h0      # exactly one low point
+        wet, z2, x2, y2 = O.wetdry_elem(2, h0, hv, ze, q6, q6)
+        if zeroed:
+            assert not z2[3:].any() and not x2[3:].any() and not y2[3:].any()
+            # the rest is the p = 1 operator on the linear part
+            w1, z1, x1, y1 = O.wetdry_elem(1, h0, hv, ze[:3], q6[:3], q6[:3])
+            assert wet == w1 and np.array_equal(z2[:3], z1) and np.array_equal(x2[:3], x1) and np.array_equal(y2[:3], y1)
+        else:
+            assert np.array_equal(z2[3:], ze[3:]) and np.array_equal(x2[3:], q6[3:]) and np.array_equal(y2[3:], q6[3:])
+    # the low point belongs to one set only: its distance to every point of the other sets is macroscopic
+    others = np.array([p for k, v in pts.items() if k != where for p in v])
+    assert np.abs(others - X).sum(1).min() > 0.05
+
+
+def test_p2_prestep_exact_threshold_is_inclusive(O):
+    """Depth exactly H1 at a vertex counts as low (comparison `<=`, SURVEY 8(c.4) tie-breaks)."""
+    h0 = 2.0 ** -10                                                     # exactly representable, so is 10 H0 + 1 - 1
+    hv = np.array([1.0, 1.0, 1.0])
+    # zeta = const + quadratic bubble that vanishes at the vertices: modes from nodal values
+    nodes = np.array([[1, 0, 0], [0, 1, 0], [0, 0, 1], [0, .5, .5], [.5, 0, .5], [.5, .5, 0]], dtype=float)
+    for dv, zeroed in ((0.0, True), (2.0 ** -40, False)):
+        zn = np.array([10 * h0 + dv - 1.0, 0.5, 0.5, 0.7, 0.7, 0.7])
+        ze = np.linalg.solve(eval_basis(O, nodes), zn)
+        z_v0 = eval_basis(O, nodes[:1]) @ ze
+        if abs(z_v0[0] + 1.0 - (10 * h0 + dv)) > 0:
+            pytest.skip("vertex value not exactly representable through the modal solve")
+        wet, z2, _, _ = O.wetdry_elem(2, h0, hv, ze, np.zeros(6), np.zeros(6))
+        assert (not z2[3:].any()) == zeroed

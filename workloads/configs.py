@@ -97,6 +97,35 @@ def hump(xy: np.ndarray, cx: float, cy: float, amp: float, sigma: float) -> np.n
     return amp * np.exp(-r2 / (2.0 * sigma * sigma))
 
 
+def perturbed(w: Workload, amp_z: float = 0.3, amp_q: float = 1.0, seed: int = 0, min_depth: float = 2.0) -> Workload:
+    """The same workload started from a non-trivial state: a smooth wave pattern (amplitude amp_z in zeta,
+    amp_q in Qx, Qy; wavelength ~ 40 cells) plus seeded white noise (10 % of the amplitude) in ALL modes of all
+    three variables, added in every element whose shallowest vertex is deeper than min_depth (dry land and the
+    swash zone keep the recipe's state).  Used by the parity tests so that every gather, permutation and mode is
+    compared on data that is not zero; the bench keeps BASELINE.json's initial states."""
+    rng = np.random.default_rng(SEED0 + 100 + seed)
+    m = w.mesh
+    p = w.params["p"]
+    nd = ndof_of(p)
+    xy = m.xy
+    span = float(max(np.ptp(xy[:, 0]), np.ptp(xy[:, 1])))
+    cell = span / math.sqrt(max(m.n_elem / 2.0, 1.0))
+    k = 2.0 * math.pi / (40.0 * cell)
+    ph = rng.uniform(0.0, 2.0 * math.pi, 6)
+    nodal = [amp_z * np.sin(k * xy[:, 0] + ph[0]) * np.cos(0.7 * k * xy[:, 1] + ph[1]),
+             amp_q * np.cos(0.8 * k * xy[:, 0] + ph[2]) * np.cos(k * xy[:, 1] + ph[3]),
+             amp_q * np.sin(k * xy[:, 0] + ph[4]) * np.sin(0.6 * k * xy[:, 1] + ph[5])]
+    deep = (w.bathy[m.tri].min(axis=1) > min_depth)[None, :]
+    decay = (1.0 / (1.0 + np.arange(nd)))[:, None]            # higher modes carry less
+    out = []
+    for c, base in enumerate((w.ze, w.qx, w.qy)):
+        amp = amp_z if c == 0 else amp_q
+        d = _modal(nodal[c], m, p) + 0.1 * amp * decay * rng.uniform(-1.0, 1.0, (nd, m.n_elem))
+        out.append(base + np.where(deep, d, 0.0))
+    return Workload(w.name + "+perturbed", m, w.bathy, w.params, out[0], out[1], out[2], w.dt, w.nsteps,
+                    tide=w.tide, holland=w.holland, notes=dict(w.notes, perturbed=(amp_z, amp_q, seed)))
+
+
 # --------------------------------------------------------------------------- C1
 def c1(nq: int = 32, nsteps: int = 100, p: int = 1, rk_order: int = 2) -> Workload:
     """Square basin 10 km x 10 km, nq x nq quads (same diagonal), flat 10 m, closed walls,
