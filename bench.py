@@ -92,7 +92,11 @@ def alg_bytes(w, kind: str, stage_first: bool, fused: bool = False) -> float:
             b += ne * 12 + nn * 16
         return b
     if kind == "limwd":
-        return ne * (st + 12 + 24 + 24 + 1 + st + 1)
+        # what a write-if-changed pass must READ: the state rows the two steps look at (p = 2: not the quadratic momentum
+        # modes), neighbour table, the neighbours' means (once per element), vertex bathymetry, wet flag.  What it writes
+        # depends on the data (only values a step changed) and is NOT credited: the fraction is a lower bound.
+        rows = 9 if w.params["p"] == 1 else 12
+        return ne * (rows * 8 + 12 + 24 + 24 + 1)
     if kind == "wind":
         return nn * 32
     raise ValueError(kind)

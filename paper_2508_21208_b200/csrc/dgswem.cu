@@ -403,7 +403,8 @@ int launch_limwd(dgswem* h, double* w) {
   A.h0 = h->prm.h0_dry; A.limiter = h->prm.limiter; A.wetdry = h->prm.wetdry;
   prof_begin(h, PK_LIMWD);
   const int ntiles = grid_for(h->ne, 128);
-  k_limwd<P><<<std::max(1, std::min(ntiles, h->res_limwd > 0 ? h->res_limwd : ntiles)), 128, 0, h->stream>>>(A, ntiles);
+  const int grid = std::max(1, std::min(ntiles, h->res_limwd > 0 ? h->res_limwd : ntiles));
+  k_limwd_tma<P><<<grid, 128, LimTile<P>::kSmem, h->stream>>>(A, ntiles);
   prof_end(h);
   CKL("k_limwd");
   return 0;
@@ -644,7 +645,10 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     h->res_edge[1] = resident_ctas(k_edge_pipe<2>, DGK_EDGE_THREADS, 0, prm->device);
     // tuning / test knob: DGSWEM_PERSISTENT_CTAS=n caps the persistent grid at n CTAs (so that small
     // meshes walk several tiles per CTA); 0 switches the persistent kernel off
-    h->res_limwd = prm->p == 1 ? resident_ctas(k_limwd<1>, 128, 0, prm->device) : resident_ctas(k_limwd<2>, 128, 0, prm->device);
+    CK(cudaFuncSetAttribute(k_limwd_tma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<1>::kSmem));
+    CK(cudaFuncSetAttribute(k_limwd_tma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<2>::kSmem));
+    h->res_limwd = prm->p == 1 ? resident_ctas(k_limwd_tma<1>, 128, LimTile<1>::kSmem, prm->device)
+                               : resident_ctas(k_limwd_tma<2>, 128, LimTile<2>::kSmem, prm->device);
     if (const char* env = std::getenv("DGSWEM_PERSISTENT_CTAS")) {
       const int cap = std::atoi(env);
 
@@ -987,7 +991,8 @@ int dgswem_halo_unpack(dgswem_t* h, int what, const double* buf, int buf_on_devi
     CK(cudaMemcpyAsync(h->halo_buf, buf, (size_t)rows * h->n_recv * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     dbuf = h->halo_buf;
   }
-  k_halo_unpack<<<grid_for(h->n_recv, 256), 256, 0, h->stream>>>(dst, dbuf, h->halo_recv, (int)h->n_recv, rows);
+  if (what == 0) k_halo_unpack<<<grid_for(h->n_recv, 256), 256, 0, h->stream>>>(dst, dbuf, h->halo_recv, (int)h->n_recv, rows);
+  else k_halo_unpack_means<<<grid_for(h->n_recv, 256), 256, 0, h->stream>>>(h->mean, h->last_out, dbuf, h->halo_recv, (int)h->n_recv, h->ndof);
   CKL("k_halo_unpack");
   if (!buf_on_device) CK(cudaStreamSynchronize(h->stream));
   return DGSWEM_OK;
