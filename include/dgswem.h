@@ -133,6 +133,12 @@ int dgswem_get_wind(dgswem_t*, double* tau);
  * Arguments outside the routines' stated range give unspecified values in rows 0 and 1. */
 int dgswem_test_math(dgswem_t*, int64_t n, const double* x, double* out);
 
+/* MEASUREMENT HOOK: the device's double-precision FMA rate (second roof of the stage kernel: "builder
+ * measures it with a DFMA microbenchmark"): 8 independent chains of dependent DFMAs per thread on 8 CTAs of 256 threads
+ * per SM, best of 3 timed launches (CUDA events on the handle's stream); *dfma_per_s = thread-level DFMAs per second
+ * (x 2 = flop/s).  Synchronises. */
+int dgswem_fp64_peak(dgswem_t*, double* dfma_per_s);
+
 /* Which form of the RK stage this handle runs: 0 = edge kernel + element kernel with the per-edge flux
  * buffer, 1 = element-centric stage kernel without it (default for p = 1; DGSWEM_FUSED=0/1 in the environment of
  * dgswem_create overrides).  Both give the same bits. */

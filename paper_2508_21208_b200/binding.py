@@ -44,7 +44,7 @@ class DgswemError(RuntimeError):
 EXPORTS = ["dgswem_create", "dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_step",
            "dgswem_eval_rhs", "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_nodal", "dgswem_get_wind",
            "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_limit", "dgswem_end_step", "dgswem_set_halo",
-           "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_stage_form", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
+           "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_fp64_peak", "dgswem_stage_form", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
 
 _lib = None
 
@@ -81,6 +81,7 @@ def load_library():
     L.dgswem_set_halo.argtypes = [VP, I64, PI32, I64, PI32]
     L.dgswem_halo_pack.argtypes = [VP, C.c_int, C.c_void_p, C.c_int]
     L.dgswem_halo_unpack.argtypes = [VP, C.c_int, C.c_void_p, C.c_int]
+    L.dgswem_fp64_peak.argtypes = [VP, PD]; L.dgswem_fp64_peak.restype = C.c_int
     L.dgswem_stage_form.argtypes = [VP]; L.dgswem_stage_form.restype = C.c_int
     L.dgswem_launch_count.argtypes = [VP]; L.dgswem_launch_count.restype = I64
     L.dgswem_profile.argtypes = [VP, C.c_int]; L.dgswem_profile.restype = C.c_int
@@ -274,6 +275,12 @@ class Dgswem:
         out = np.empty((4, x.size))
         self._check(self.L.dgswem_test_math(self.h, C.c_int64(x.size), _dp(x), _dp(out)))
         return out
+
+    def fp64_peak(self) -> float:
+        """MEASUREMENT HOOK: the device's DFMA rate (thread-level DFMAs per second) from the library's probe kernel."""
+        out = C.c_double()
+        self._check(self.L.dgswem_fp64_peak(self.h, C.byref(out)))
+        return out.value
 
     def stage_form(self) -> int:
         """0: edge kernel + element kernel (flux buffer); 1: element-centric stage kernel."""

@@ -1127,6 +1127,32 @@ int dgswem_test_math(dgswem_t* h, int64_t n, const double* x, double* out) {
   return DGSWEM_OK;   // the two scratch buffers stay with the handle until dgswem_destroy
 }
 
+int dgswem_fp64_peak(dgswem_t* h, double* dfma_per_s) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!dfma_per_s) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
+  CK(cudaSetDevice(h->prm.device));
+  int sms = 0;
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->prm.device));
+  const int grid = sms * 8, threads = 256, rounds = 20000;
+  cudaEvent_t a, b;
+  CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+  double best = 0.0;
+  for (int rep = 0; rep < 4; ++rep) {      // first repetition warms up
+    CK(cudaEventRecord(a, h->stream));
+    k_dfma_probe<<<grid, threads, 0, h->stream>>>(h->stage_buf, rounds, 0.999999, 1e-6);
+    CKL("k_dfma_probe");
+    CK(cudaEventRecord(b, h->stream));
+    CK(cudaEventSynchronize(b));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, a, b));
+    const double rate = (double)grid * threads * 8.0 * rounds / (ms * 1e-3);
+    if (rep > 0 && rate > best) best = rate;
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b);
+  *dfma_per_s = best;
+  return DGSWEM_OK;
+}
+
 int dgswem_stage_form(const dgswem_t* h) { return (h && h->fused) ? 1 : 0; }
 
 int64_t dgswem_launch_count(const dgswem_t* h) { return h ? h->launches : 0; }

@@ -18,7 +18,7 @@ def lib():
 
 def test_header_symbols_are_exported(lib):
     hdr = (ROOT / "include" / "dgswem.h").read_text()
-    declared = set(re.findall(r"\b(dgswem_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(dgswem_[a-z0-9_]+)\s*\(", hdr))
     assert {"dgswem_create", "dgswem_set_state", "dgswem_step", "dgswem_get_state", "dgswem_eval_rhs",
             "dgswem_get_wetdry", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_destroy"} <= declared
     for name in declared:
