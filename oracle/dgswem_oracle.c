@@ -221,12 +221,25 @@ double orc_det_log(double x) {
  * centre (cx, cy), counter-clockwise; Garratt drag; returns kinematic stress tau_s/rho_0. */
 void orc_holland_node(const orc_holland* h, double cx, double cy, double x, double y,
                       double* tsx, double* tsy, double* Vout) {
+  orc_holland_node_p(h, 0.0, cx, cy, x, y, tsx, tsy, Vout, NULL);
+}
+
+/* The same with the Holland (1980) surface pressure p(r) = p_c + dp exp(-(R/r)^B): returns in *etap the pressure
+ * anomaly against the far field as a water column, eta_p = (p - p_n)/(rho_0 g) = -(dp/(rho_0 g)) (1 - exp(-(R/r)^B))
+ * (PAPER.md:65 forcings, :326 "Wind forcing and pressure calculations (WIND)"; [R-15]).  etap may be NULL. */
+void orc_holland_node_p(const orc_holland* h, double g, double cx, double cy, double x, double y,
+                        double* tsx, double* tsy, double* Vout, double* etap) {
   double dx = x - cx, dy = y - cy;
   double r = sqrt(fma(dy, dy, dx * dx));
-  if (r < 1.0) { *tsx = 0.0; *tsy = 0.0; if (Vout) *Vout = 0.0; return; }
+  if (r < 1.0) {
+    *tsx = 0.0; *tsy = 0.0; if (Vout) *Vout = 0.0;
+    if (etap) *etap = -(h->dp / (h->rho_water * g));
+    return;
+  }
   double xb = orc_det_exp(h->B * orc_det_log(h->rmax / r));   /* (R/r)^B */
+  double ee = orc_det_exp(-xb);
   double rf2 = 0.5 * (r * h->f);
-  double V = sqrt(fma((h->B / h->rho_air) * xb, h->dp * orc_det_exp(-xb), rf2 * rf2)) - rf2;
+  double V = sqrt(fma((h->B / h->rho_air) * xb, h->dp * ee, rf2 * rf2)) - rf2;
   double rr = 1.0 / r;
   double wx = (-(dy * rr)) * V;
   double wy = (dx * rr) * V;
@@ -236,6 +249,7 @@ void orc_holland_node(const orc_holland* h, double cx, double cy, double x, doub
   *tsx = k * wx;
   *tsy = k * wy;
   if (Vout) *Vout = V;
+  if (etap) *etap = -((h->dp / (h->rho_water * g)) * (1.0 - ee));
 }
 
 /* ---------------------------------------------------------------- limiter */
@@ -434,9 +448,13 @@ struct orc_model {
   uint8_t* wet;
   double t;
   double tide_amp, tide_omega, tide_phase;
-  int wind_on;
+  int wind_on;        /* a Holland vortex is set */
+  int stress_on;      /* ... its wind stress enters the momentum source (default 1) */
+  int press_on;       /* ... its surface-pressure gradient enters the momentum source (default 0) [R-15] */
   orc_holland hol;
-  double* tau; /*[2][nn]*/
+  double* tau;  /*[2][nn]*/
+  double* etap; /*[nn] pressure anomaly as a water column */
+  double rain;  /* mass source R of eq. (1), m/s, uniform [R-16] */
 };
 
 static void* xmalloc(size_t n) { void* p = malloc(n ? n : 1); if (!p) abort(); return p; }
@@ -506,6 +524,8 @@ orc_model* orc_create(const orc_params* prm, int64_t n_nodes, const double* xy, 
   m->mean = NEW(double, 3 * ne);
   m->wet = NEW(uint8_t, ne); memset(m->wet, 1, ne);
   m->tau = NEW(double, 2 * n_nodes); memset(m->tau, 0, sizeof(double) * 2 * n_nodes);
+  m->etap = NEW(double, n_nodes); memset(m->etap, 0, sizeof(double) * n_nodes);
+  m->stress_on = 1; m->press_on = 0; m->rain = 0.0;
   m->t = 0.0;
   return m;
 }
@@ -515,7 +535,7 @@ void orc_destroy(orc_model* m) {
   free(m->xy); free(m->bathy); free(m->tri); free(m->edge_elem); free(m->edge_local); free(m->edge_bc);
   free(m->elem_edge); free(m->area); free(m->jinv); free(m->lfac); free(m->hv); free(m->enx); free(m->eny);
   free(m->ehb); free(m->nbr); free(m->w); free(m->w0); free(m->rhs); free(m->flux); free(m->mean);
-  free(m->wet); free(m->tau); free(m);
+  free(m->wet); free(m->tau); free(m->etap); free(m);
 }
 
 const orc_tables* orc_get_tables(const orc_model* m) { return &m->T; }
@@ -602,6 +622,15 @@ static void elem_rhs_all(orc_model* m, const double* w, double* rhs, double* sca
     double dhy = 0.5 * fma(hv2 - hv0, x2y, (hv1 - hv0) * x1y);
     int wet = m->wet[e];
     const int32_t* tn = m->tri + 3 * e;
+    /* gradient of the pressure anomaly eta_p, linear per element from its nodal values (as grad h_b) [R-15] */
+    double dpx = 0.0, dpy = 0.0;
+    const int press = wet && m->wind_on && m->press_on;
+    if (press) {
+      double p0 = m->etap[tn[0]], p1 = m->etap[tn[1]], p2 = m->etap[tn[2]];
+      dpx = 0.5 * fma(p2 - p0, x2x, (p1 - p0) * x1x);
+      dpy = 0.5 * fma(p2 - p0, x2y, (p1 - p0) * x1y);
+    }
+    const double rain = m->rain;
     for (int i = 0; i < nqa; ++i) {
       double z = ze[e], u_qx = qx[e], u_qy = qy[e];
       for (int k = 1; k < ndof; ++k) {                              /* Alg. 1 lines 10-15 */
@@ -623,7 +652,7 @@ static void elem_rhs_all(orc_model* m, const double* w, double* rhs, double* sca
       double tau = 0.0, tsx = 0.0, tsy = 0.0;
       if (wet) {                                                    /* friction, wind: wet elements only [R-6] */
         tau = (cf * sqrt(fma(u_qy, u_qy, u_qx * u_qx))) * (rH * rH);
-        if (m->wind_on) {
+        if (m->wind_on && m->stress_on) {
           /* wind stress, linear from the three nodes, ramped by the local depth with the same
            * thin-layer weight as the wet/dry momentum rule: clamp((H-H0)/(H1-H0),0,1), H1=10 H0
            * ([R-9]; a millimetre film must not take the full hurricane stress: tau_s/H is stiff) */
@@ -637,20 +666,27 @@ static void elem_rhs_all(orc_model* m, const double* w, double* rhs, double* sca
         }
       }
       double S[3];
-      S[0] = 0.0;                                                   /* rain R: out of scope */
+      S[0] = rain;                                                  /* mass source R of eq. (1) [R-16] */
       S[1] = fma(fc, u_qy, fma(-tau, u_qx, gz * dhx)) + tsx;
       S[2] = fma(-fc, u_qx, fma(-tau, u_qy, gz * dhy)) + tsy;
+      double gH = 0.0;
+      if (press) {                                                  /* -(H/rho_0) grad p_a = -g H grad eta_p [R-15] */
+        gH = g * H;
+        S[1] = fma(-gH, dpx, S[1]);
+        S[2] = fma(-gH, dpy, S[2]);
+      }
       for (int k = 0; k < ndof; ++k) {                              /* Alg. 1 lines 26-35 */
         double gxk = fma(T->dphiA2[i][k], x2x, T->dphiA1[i][k] * x1x);
         double gyk = fma(T->dphiA2[i][k], x2y, T->dphiA1[i][k] * x1y);
         double xf = T->wfac[i][k] * gxk, yf = T->wfac[i][k] * gyk, sf = T->srfac[i][k];
         r[0][k] = fma(yf, F[0][1], fma(xf, F[0][0], r[0][k]));
+        if (rain != 0.0) r[0][k] = fma(sf, S[0], r[0][k]);
         r[1][k] = fma(sf, S[1], fma(yf, F[1][1], fma(xf, F[1][0], r[1][k])));
         r[2][k] = fma(sf, S[2], fma(yf, F[2][1], fma(xf, F[2][0], r[2][k])));
         for (int c = 0; c < 3; ++c)
           sc[c][k] += fabs(xf * F[c][0]) + fabs(yf * F[c][1]) + (c ? fabs(sf * (gz * (c == 1 ? dhx : dhy))) +
                       fabs(sf * (tau * (c == 1 ? u_qx : u_qy))) + fabs(sf * (fc * (c == 1 ? u_qy : u_qx))) +
-                      fabs(sf * (c == 1 ? tsx : tsy)) : 0.0);
+                      fabs(sf * (c == 1 ? tsx : tsy)) + fabs(sf * (gH * (c == 1 ? dpx : dpy))) : fabs(sf * S[0]));
       }
     }
     for (int c = 0; c < 3; ++c)
@@ -734,7 +770,7 @@ static void wind_all(orc_model* m, double t) {
   const int64_t nn = m->n_nodes;
 #pragma omp parallel for schedule(static)
   for (int64_t i = 0; i < nn; ++i)
-    orc_holland_node(&m->hol, cx, cy, m->xy[2 * i], m->xy[2 * i + 1], &m->tau[i], &m->tau[nn + i], NULL);
+    orc_holland_node_p(&m->hol, m->prm.g, cx, cy, m->xy[2 * i], m->xy[2 * i + 1], &m->tau[i], &m->tau[nn + i], NULL, &m->etap[i]);
 }
 
 void orc_set_state(orc_model* m, double t, const double* ze, const double* qx, const double* qy) {
@@ -771,6 +807,12 @@ void orc_set_tide(orc_model* m, double amp, double omega, double phase) {
 void orc_set_wind_holland(orc_model* m, const orc_holland* h) {
   if (h) { m->hol = *h; m->wind_on = 1; } else { m->wind_on = 0; }
 }
+
+/* which parts of the Holland forcing enter the momentum source (defaults: stress on, pressure gradient off) */
+void orc_set_wind_forcing(orc_model* m, int stress_on, int press_on) { m->stress_on = stress_on != 0; m->press_on = press_on != 0; }
+
+/* uniform mass source R (rain) in m/s */
+void orc_set_rain(orc_model* m, double rate) { m->rain = rate; }
 
 void orc_step(orc_model* m, int64_t nsteps, double dt) {
   const int64_t n = 3 * (int64_t)m->T.ndof * m->n_elem;
@@ -844,6 +886,8 @@ void orc_get_geometry(orc_model* m, double* area, double* jinv, double* lfac, do
 }
 
 void orc_get_wind(orc_model* m, double* tau) { memcpy(tau, m->tau, sizeof(double) * 2 * m->n_nodes); }
+
+void orc_get_pressure(orc_model* m, double* etap) { memcpy(etap, m->etap, sizeof(double) * m->n_nodes); }
 
 int orc_num_threads(void) {
 #ifdef _OPENMP

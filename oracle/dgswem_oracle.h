@@ -62,6 +62,9 @@ void   orc_llf_flux(double g, double h0, double nx, double ny, double hq,
 double orc_det_exp(double x);
 double orc_det_log(double x);
 void   orc_holland_node(const orc_holland* h, double cx, double cy, double x, double y, double* tsx, double* tsy, double* V);
+/* ... with the surface-pressure anomaly as a water column, eta_p = (p - p_n)/(rho_0 g) (etap may be NULL) */
+void   orc_holland_node_p(const orc_holland* h, double g, double cx, double cy, double x, double y,
+                          double* tsx, double* tsy, double* V, double* etap);
 /* limiter on one element, one variable; mean_nb[3] neighbour means, has_nb[3] flags */
 double orc_limit_var(int p, double* w /*[ndof]*/, const double* mean_nb, const int* has_nb);
 /* wet/dry on one element: modes [ndof] of ze,qx,qy, vertex bathymetry hv[3]; returns wet flag */
@@ -86,6 +89,8 @@ void orc_set_state_raw(orc_model*, double t, const double* ze, const double* qx,
 void orc_apply_post(orc_model*, int do_limiter, int do_wetdry);
 void orc_set_tide(orc_model*, double amp, double omega, double phase);
 void orc_set_wind_holland(orc_model*, const orc_holland* /* NULL = off */);
+void orc_set_wind_forcing(orc_model*, int stress_on, int press_on);   /* parts of the Holland forcing in use (default 1, 0) */
+void orc_set_rain(orc_model*, double rate);                           /* uniform mass source R, m/s */
 void orc_step(orc_model*, int64_t nsteps, double dt);
 /* L_h(current state) at t (stage-1 time); scale arrays (may be NULL) receive the sum of
  * absolute values of all contributions to each entry (the error-norm denominator). */
@@ -97,6 +102,7 @@ void orc_get_nodal(orc_model*, double* zn, double* qxn, double* qyn);   /* [n_no
 void orc_get_geometry(orc_model*, double* area /*[n_elem]*/, double* jinv /*[4][n_elem]*/, double* lfac /*[3][n_elem]*/,
                       double* enx /*[n_edge]*/, double* eny /*[n_edge]*/);
 void orc_get_wind(orc_model*, double* tau /*[2][n_nodes]*/);
+void orc_get_pressure(orc_model*, double* etap /*[n_nodes]*/);
 int  orc_num_threads(void);
 
 #ifdef __cplusplus

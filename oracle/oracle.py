@@ -90,6 +90,7 @@ def lib():
     L.orc_det_exp.argtypes = [D]; L.orc_det_exp.restype = D
     L.orc_det_log.argtypes = [D]; L.orc_det_log.restype = D
     L.orc_holland_node.argtypes = [C.POINTER(Holland), D, D, D, D, PD, PD, PD]
+    L.orc_holland_node_p.argtypes = [C.POINTER(Holland), D, D, D, D, D, PD, PD, PD, PD]
     L.orc_limit_var.argtypes = [C.c_int, PD, PD, C.POINTER(C.c_int)]; L.orc_limit_var.restype = D
     L.orc_wetdry_elem.argtypes = [C.POINTER(Tables), D, PD, PD, PD, PD]; L.orc_wetdry_elem.restype = C.c_int
     L.orc_ssprk_step.argtypes = [C.c_int, I64, PD, PD, PD, D, D, RHS_FN, POST_FN, VP]; L.orc_ssprk_step.restype = C.c_int
@@ -103,6 +104,9 @@ def lib():
     L.orc_apply_post.argtypes = [VP, C.c_int, C.c_int]
     L.orc_set_tide.argtypes = [VP, D, D, D]
     L.orc_set_wind_holland.argtypes = [VP, C.POINTER(Holland)]
+    L.orc_set_wind_forcing.argtypes = [VP, C.c_int, C.c_int]
+    L.orc_set_rain.argtypes = [VP, D]
+    L.orc_get_pressure.argtypes = [VP, PD]
     L.orc_step.argtypes = [VP, I64, D]
     L.orc_eval_rhs.argtypes = [VP, PD, PD, PD, PD, PD, PD]
     L.orc_get_flux.argtypes = [VP, PD]
@@ -150,6 +154,13 @@ def holland_node(hol: dict, cx, cy, x, y):
     out = [C.c_double() for _ in range(3)]
     lib().orc_holland_node(C.byref(h), cx, cy, x, y, *[C.byref(o) for o in out])
     return tuple(o.value for o in out)   # tsx, tsy, V
+
+
+def holland_node_p(hol: dict, g, cx, cy, x, y):
+    h = Holland(**hol)
+    out = [C.c_double() for _ in range(4)]
+    lib().orc_holland_node_p(C.byref(h), g, cx, cy, x, y, *[C.byref(o) for o in out])
+    return tuple(o.value for o in out)   # tsx, tsy, V, eta_p
 
 
 def limit_var(p, w, mean_nb, has_nb):
@@ -223,6 +234,10 @@ class Oracle:
             o.set_tide(*w.tide)
         if w.holland is not None:
             o.set_wind_holland(w.holland)
+            if w.notes.get("pressure"):
+                o.set_wind_forcing(True, True)
+        if w.notes.get("rain"):
+            o.set_rain(w.notes["rain"])
         o.set_state(0.0, w.ze, w.qx, w.qy)
         return o
 
@@ -268,6 +283,17 @@ class Oracle:
             self.L.orc_set_wind_holland(self.h, None)
         else:
             self.L.orc_set_wind_holland(self.h, C.byref(Holland(**hol)))
+
+    def set_wind_forcing(self, stress=True, pressure=False):
+        self.L.orc_set_wind_forcing(self.h, int(bool(stress)), int(bool(pressure)))
+
+    def set_rain(self, rate):
+        self.L.orc_set_rain(self.h, float(rate))
+
+    def get_pressure(self):
+        p = np.zeros(self.n_nodes)
+        self.L.orc_get_pressure(self.h, _dp(p))
+        return p
 
     def step(self, nsteps, dt):
         self.L.orc_step(self.h, int(nsteps), float(dt))
