@@ -84,6 +84,15 @@ int dgswem_set_tide(dgswem_t*, double amp, double omega, double phase);
 /* Moving Holland vortex wind stress (R-9); NULL switches the wind off. */
 int dgswem_set_wind_holland(dgswem_t*, const dgswem_holland*);
 
+/* Which parts of the Holland forcing enter the momentum source while a vortex is set: the wind stress (R-9; default
+ * on) and the surface-pressure gradient -(H/rho_0) grad p_a = -g H grad eta_p with the Holland pressure profile
+ * p(r) = p_c + dp exp(-(R/r)^B) evaluated at the nodes by the WIND kernel ("Wind forcing and pressure
+ * calculations"; R-15; default off). */
+int dgswem_set_wind_forcing(dgswem_t*, int stress_on, int pressure_on);
+
+/* Uniform mass source R in the continuity equation ("such as rain"; R-16), in m/s; 0 = off. */
+int dgswem_set_rain(dgswem_t*, double rate);
+
 /* Advance nsteps time steps of size dt: per step WIND at the nodes, then per
  * stage EDGE -> GATHER+AREA+RK update -> limiter -> wet/dry.  Asynchronous on the stream. */
 int dgswem_step(dgswem_t*, int64_t nsteps, double dt);
@@ -127,6 +136,9 @@ int dgswem_get_nodal(dgswem_t*, double* zn, double* qxn, double* qyn);
 
 /* Nodal kinematic wind stress tau_s/rho_0 of the last WIND evaluation, [2][n_nodes] (test hook). */
 int dgswem_get_wind(dgswem_t*, double* tau);
+
+/* Nodal surface-pressure anomaly as a water column, eta_p = (p - p_n)/(rho_0 g), of the last WIND evaluation, [n_nodes] (test hook). */
+int dgswem_get_pressure(dgswem_t*, double* etap);
 
 /* TEST HOOK: the kernels' reciprocal and square-root routines next to the IEEE
  * operators, on n caller-supplied arguments x (host): out (host, [4][n]) = rcp_rn(x), sqrt_rn(x), 1.0/x, sqrt(x).

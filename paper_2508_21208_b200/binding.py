@@ -41,7 +41,7 @@ class DgswemError(RuntimeError):
         self.code = code
 
 
-EXPORTS = ["dgswem_create", "dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_step",
+EXPORTS = ["dgswem_create", "dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_set_wind_forcing", "dgswem_set_rain", "dgswem_get_pressure", "dgswem_step",
            "dgswem_eval_rhs", "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_nodal", "dgswem_get_wind",
            "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_limit", "dgswem_end_step", "dgswem_set_halo",
            "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_fp64_peak", "dgswem_stage_form", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
@@ -66,6 +66,9 @@ def load_library():
     L.dgswem_set_state.argtypes = [VP, D, PD, PD, PD]
     L.dgswem_set_tide.argtypes = [VP, D, D, D]
     L.dgswem_set_wind_holland.argtypes = [VP, C.POINTER(Holland)]
+    L.dgswem_set_wind_forcing.argtypes = [VP, C.c_int, C.c_int]
+    L.dgswem_set_rain.argtypes = [VP, D]
+    L.dgswem_get_pressure.argtypes = [VP, PD]
     L.dgswem_step.argtypes = [VP, I64, D]
     L.dgswem_eval_rhs.argtypes = [VP, PD, PD, PD]
     L.dgswem_get_flux.argtypes = [VP, PD]
@@ -89,7 +92,8 @@ def load_library():
     L.dgswem_sync.argtypes = [VP]
     L.dgswem_last_error.argtypes = [VP]; L.dgswem_last_error.restype = C.c_char_p
     L.dgswem_destroy.argtypes = [VP]; L.dgswem_destroy.restype = None
-    for name in ("dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_step", "dgswem_eval_rhs",
+    for name in ("dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_set_wind_forcing", "dgswem_set_rain",
+                 "dgswem_get_pressure", "dgswem_step", "dgswem_eval_rhs",
                  "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_wind", "dgswem_sync",
                  "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_limit", "dgswem_end_step", "dgswem_set_halo",
                  "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_get_nodal"):
@@ -169,6 +173,10 @@ class Dgswem:
             o.set_tide(*w.tide)
         if w.holland is not None:
             o.set_wind_holland(w.holland)
+            if w.notes.get("pressure"):
+                o.set_wind_forcing(True, True)
+        if w.notes.get("rain"):
+            o.set_rain(w.notes["rain"])
         o.set_state(0.0, w.ze, w.qx, w.qy)
         return o
 
@@ -196,6 +204,12 @@ class Dgswem:
             self._check(self.L.dgswem_set_wind_holland(self.h, None))
         else:
             self._check(self.L.dgswem_set_wind_holland(self.h, C.byref(Holland(**hol))))
+
+    def set_wind_forcing(self, stress=True, pressure=False):
+        self._check(self.L.dgswem_set_wind_forcing(self.h, int(bool(stress)), int(bool(pressure))))
+
+    def set_rain(self, rate):
+        self._check(self.L.dgswem_set_rain(self.h, float(rate)))
 
     def step(self, nsteps, dt):
         self._check(self.L.dgswem_step(self.h, int(nsteps), float(dt)))
@@ -232,6 +246,11 @@ class Dgswem:
         tau = np.empty((2, self.n_nodes))
         self._check(self.L.dgswem_get_wind(self.h, _dp(tau)))
         return tau
+
+    def get_pressure(self):
+        ep = np.empty(self.n_nodes)
+        self._check(self.L.dgswem_get_pressure(self.h, _dp(ep)))
+        return ep
 
     # ---- stage-granular stepping and halo lists (domain decomposition building blocks)
     def begin_step(self, dt):

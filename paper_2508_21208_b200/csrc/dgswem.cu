@@ -168,7 +168,7 @@ struct dgswem {
   // device
   double* W[3] = {nullptr, nullptr, nullptr};
   double *flux = nullptr, *mean = nullptr, *jinv = nullptr, *lfac = nullptr, *hv = nullptr;
-  double *en = nullptr, *ehb = nullptr, *tau = nullptr, *nxy = nullptr, *stage_buf = nullptr;
+  double *en = nullptr, *ehb = nullptr, *tau = nullptr, *etap = nullptr, *nxy = nullptr, *stage_buf = nullptr;
   int2* edge_elem = nullptr;
   int *einfo = nullptr, *elem_edge = nullptr, *nbr = nullptr, *tri = nullptr, *nbinfo = nullptr;
   double* enl = nullptr;
@@ -201,6 +201,8 @@ struct dgswem {
   double t = 0.0;
   double tide_amp = 0.0, tide_omega = 0.0, tide_phase = 0.0;
   bool wind_on = false;
+  bool stress_on = true, press_on = false;   // parts of the Holland forcing in the momentum source (R-9, R-15)
+  double rain = 0.0;                         // uniform mass source (R-16)
   dgswem_holland hol{};
 
   int fail(int code, const char* fmt, ...) {
@@ -334,12 +336,20 @@ int launch_edge(dgswem* h, const double* w, ScalRef zeta_b) {
   return 0;
 }
 
+// compile-time specialisation of the element / stage kernels: bit 0 first RK stage, bit 1 Holland forcing, bit 2 its
+// pressure gradient; -1 (flags read from the arguments) when a rarely used option is on (rain)
+inline int stage_variant(const dgswem* h, int first) {
+  if (h->rain != 0.0) return -1;
+  return (first ? 1 : 0) | (h->wind_on ? 2 : 0) | ((h->wind_on && h->press_on) ? 4 : 0);
+}
+
 template <int P, int MODE>
 int launch_elem(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b,
                 int first, bool fuse_wd, bool write_mean) {
   ElemArgs A;
   A.win = win; A.w0 = w0; A.wout = wout; A.flux = h->flux; A.elem_edge = h->elem_edge; A.jinv = h->jinv;
   A.lfac = h->lfac; A.hv = h->hv; A.tri = h->tri; A.tau = h->tau; A.wet = h->wet;
+  A.etap = h->etap; A.stress = h->stress_on ? 1 : 0; A.press = h->press_on ? 1 : 0; A.rain = h->rain;
   A.nbinfo = nullptr; A.enl = nullptr; A.zeta = scal(h, 0, 0.0);
   A.mean = write_mean ? h->mean : nullptr;
   A.ne = (int)h->ne; A.ld = h->ld; A.ldd = h->ldd; A.ldn = h->ldn;
@@ -350,11 +360,14 @@ int launch_elem(dgswem* h, const double* win, const double* w0, double* wout, do
   prof_begin(h, PK_ELEM);
   const int grid = grid_for(h->ne, DGK_ELEM_THREADS);
   if constexpr (MODE == MODE_UPDATE) {
-    switch ((first ? 1 : 0) | (h->wind_on ? 2 : 0)) {   // specialised on (first stage, wind), as k_stage
+    switch (stage_variant(h, first)) {   // specialised on (first stage, wind, pressure), as k_stage
       case 0: k_elem<P, MODE, 0><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
       case 1: k_elem<P, MODE, 1><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
       case 2: k_elem<P, MODE, 2><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
-      default: k_elem<P, MODE, 3><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
+      case 3: k_elem<P, MODE, 3><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
+      case 6: k_elem<P, MODE, 6><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
+      case 7: k_elem<P, MODE, 7><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
+      default: k_elem<P, MODE, -1><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
     }
   } else {
     k_elem<P, MODE, -1><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A);
@@ -371,6 +384,7 @@ int launch_stage(dgswem* h, const double* win, const double* w0, double* wout, d
   ElemArgs A;
   A.win = win; A.w0 = w0; A.wout = wout; A.flux = h->flux; A.elem_edge = h->elem_edge; A.jinv = h->jinv;
   A.lfac = h->lfac; A.hv = h->hv; A.tri = h->tri; A.tau = h->tau; A.wet = h->wet;
+  A.etap = h->etap; A.stress = h->stress_on ? 1 : 0; A.press = h->press_on ? 1 : 0; A.rain = h->rain;
   A.nbinfo = h->nbinfo; A.enl = h->enl; A.zeta = zeta_b;
   A.mean = write_mean ? h->mean : nullptr;
   A.ne = (int)h->ne; A.ld = h->ld; A.ldd = h->ldd; A.ldn = h->ldn;
@@ -382,11 +396,14 @@ int launch_stage(dgswem* h, const double* win, const double* w0, double* wout, d
   const int grid = grid_for(h->ne, DGK_STAGE_THREADS);
   if constexpr (MODE == MODE_UPDATE) {
     // specialised on (first stage, wind): no w^n registers in stage 1, no wind registers without wind
-    switch ((first ? 1 : 0) | (h->wind_on ? 2 : 0)) {
+    switch (stage_variant(h, first)) {
       case 0: k_stage<P, MODE, 0><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
       case 1: k_stage<P, MODE, 1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
       case 2: k_stage<P, MODE, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      default: k_stage<P, MODE, 3><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      case 3: k_stage<P, MODE, 3><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      case 6: k_stage<P, MODE, 6><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      case 7: k_stage<P, MODE, 7><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      default: k_stage<P, MODE, -1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
     }
   } else {
     k_stage<P, MODE, -1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A);
@@ -412,7 +429,7 @@ int launch_limwd(dgswem* h, double* w) {
 
 int launch_wind(dgswem* h, double t) {
   WindArgs A;
-  A.nxy = h->nxy; A.tau = h->tau; A.nn = (int)h->nn; A.ldn = h->ldn;
+  A.nxy = h->nxy; A.tau = h->tau; A.etap = h->etap; A.g = h->prm.g; A.nn = (int)h->nn; A.ldn = h->ldn;
   A.cx = scal(h, 4, h->hol.x0 + h->hol.vx * t); A.cy = scal(h, 5, h->hol.y0 + h->hol.vy * t);
   A.rmax = h->hol.rmax; A.dp = h->hol.dp; A.B = h->hol.B; A.rho_air = h->hol.rho_air; A.rho_water = h->hol.rho_water;
   A.f = h->hol.f;
@@ -796,6 +813,7 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     h->flux = (double*)h->dalloc(fbytes);
     h->mean = (double*)h->dalloc((size_t)3 * ld * sizeof(double));
     h->tau = (double*)h->dalloc((size_t)2 * ldn * sizeof(double));
+    h->etap = (double*)h->dalloc((size_t)ldn * sizeof(double));
     h->stage_buf = (double*)h->dalloc(h->stage_bytes);
     h->wet = (unsigned char*)h->dalloc((size_t)ld);
     h->wet_stage = (unsigned char*)h->dalloc((size_t)ld);
@@ -803,11 +821,12 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     h->step_ctr = (int*)h->dalloc(256);
     h->last_out = h->W[0];
     if (const char* env = std::getenv("DGSWEM_GRAPH")) h->graphs_on = std::atoi(env) != 0;
-    if (!h->flux || !h->mean || !h->tau || !h->stage_buf || !h->wet || !h->wet_stage || !h->nf_flag || !h->step_ctr)
+    if (!h->flux || !h->mean || !h->tau || !h->etap || !h->stage_buf || !h->wet || !h->wet_stage || !h->nf_flag || !h->step_ctr)
       return h->fail(DGSWEM_E_CUDA, "device allocation failed");
     CK(cudaMemsetAsync(h->flux, 0, fbytes, h->stream));
     CK(cudaMemsetAsync(h->mean, 0, (size_t)3 * ld * sizeof(double), h->stream));
     CK(cudaMemsetAsync(h->tau, 0, (size_t)2 * ldn * sizeof(double), h->stream));
+    CK(cudaMemsetAsync(h->etap, 0, (size_t)ldn * sizeof(double), h->stream));
     CK(cudaMemsetAsync(h->wet, 1, (size_t)ld, h->stream));
     CK(cudaStreamSynchronize(h->stream));
     return 0;
@@ -861,6 +880,21 @@ int dgswem_set_wind_holland(dgswem_t* h, const dgswem_holland* hol) {
   } else {
     h->wind_on = false;
   }
+  return DGSWEM_OK;
+}
+
+int dgswem_set_wind_forcing(dgswem_t* h, int stress_on, int pressure_on) {
+  if (!h) return DGSWEM_E_ARG;
+  drop_graphs(h);   // frozen kernel arguments
+  h->stress_on = stress_on != 0; h->press_on = pressure_on != 0;
+  return DGSWEM_OK;
+}
+
+int dgswem_set_rain(dgswem_t* h, double rate) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!std::isfinite(rate)) return h->fail(DGSWEM_E_ARG, "rain rate must be finite");
+  drop_graphs(h);
+  h->rain = rate;
   return DGSWEM_OK;
 }
 
@@ -1108,6 +1142,15 @@ int dgswem_get_wind(dgswem_t* h, double* tau) {
   CK(cudaSetDevice(h->prm.device));
   const size_t row = (size_t)h->nn * sizeof(double);
   CK(cudaMemcpy2DAsync(tau, row, h->tau, (size_t)h->ldn * sizeof(double), row, 2, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return DGSWEM_OK;
+}
+
+int dgswem_get_pressure(dgswem_t* h, double* etap) {
+  if (!h) return DGSWEM_E_ARG;
+  if (!etap) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
+  CK(cudaSetDevice(h->prm.device));
+  CK(cudaMemcpyAsync(etap, h->etap, (size_t)h->nn * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
   return DGSWEM_OK;
 }

@@ -126,6 +126,18 @@ def perturbed(w: Workload, amp_z: float = 0.3, amp_q: float = 1.0, seed: int = 0
                     tide=w.tide, holland=w.holland, notes=dict(w.notes, perturbed=(amp_z, amp_q, seed)))
 
 
+def with_forcing(w: Workload, pressure: bool = False, rain: float = 0.0) -> Workload:
+    """The same workload with the surface-pressure gradient of its Holland vortex switched on and / or a uniform rain
+    rate (m/s) -- SURVEY.md 8(f) NEXT-4; both sides' from_workload read these notes."""
+    notes = dict(w.notes)
+    if pressure:
+        notes["pressure"] = True
+    if rain:
+        notes["rain"] = float(rain)
+    return Workload(w.name + ("+pressure" if pressure else "") + ("+rain" if rain else ""), w.mesh, w.bathy, w.params,
+                    w.ze, w.qx, w.qy, w.dt, w.nsteps, tide=w.tide, holland=w.holland, notes=notes)
+
+
 # --------------------------------------------------------------------------- C1
 def c1(nq: int = 32, nsteps: int = 100, p: int = 1, rk_order: int = 2) -> Workload:
     """Square basin 10 km x 10 km, nq x nq quads (same diagonal), flat 10 m, closed walls,
