@@ -161,6 +161,58 @@ void orc_llf_flux(double g, double h0, double nx, double ny, double hq,
   *fqy = fma(fn, ny, ft * nx);
 }
 
+/* Roe flux [R-17] ("e.g., Local Lax-Friedrichs or Roe"), same frame, boundary states and depth floor as the
+ * LLF flux above.  Roe state of the two traces: un~ = (s+ un+ + s- un-)/(s+ + s-), ut~ likewise, s = sqrt(H_c),
+ * c~ = sqrt(g (H_c+ + H_c-)/2); jumps dH = zeta- - zeta+ (same bed on both sides), dqn, dqt; wave strengths
+ * a1,3 = (dH -+ (dqn - un~ dH)/c~)/2 on lambda1,3 = un~ -+ c~ with r1,3 = (1, lambda1,3, ut~), a2 = dqt - ut~ dH on
+ * lambda2 = un~ with r2 = (0, 0, 1);  F^ = (F(w+) + F(w-))/2 . n - (1/2) sum_k |lambda_k| a_k r_k.  No entropy fix.
+ * Every two-term sum pairs a "+"-side with a "-"-side product (or wave 1 with wave 3) and is written without fma, so
+ * that swapping the sides and negating n negates the flux bit for bit (as for LLF), and a wall has exactly zero mass flux. */
+void orc_roe_flux(double g, double h0, double nx, double ny, double hq,
+                  double zp, double qxp, double qyp, double zm, double qxm, double qym,
+                  int bc, double zeta_b, double* fz, double* fqx, double* fqy) {
+  double qnp = fma(qyp, ny, qxp * nx);
+  double qtp = fma(qyp, nx, -(qxp * ny));
+  double qnm, qtm;
+  if (bc == 0) {
+    qnm = fma(qym, ny, qxm * nx);
+    qtm = fma(qym, nx, -(qxm * ny));
+  } else if (bc == 1) {
+    zm = zp; qnm = -qnp; qtm = qtp;
+  } else {
+    zm = zeta_b; qnm = qnp; qtm = qtp;
+  }
+  double Hp = zp + hq, Hm = zm + hq;
+  double Hcp = (Hp > h0) ? Hp : h0;
+  double Hcm = (Hm > h0) ? Hm : h0;
+  double rHp = 1.0 / Hcp, rHm = 1.0 / Hcm;
+  double unp = qnp * rHp, unm = qnm * rHm;
+  double utp = qtp * rHp, utm = qtm * rHm;
+  double sp = sqrt(Hcp), sm = sqrt(Hcm);
+  double rS = 1.0 / (sp + sm);
+  double un = (sp * unp + sm * unm) * rS;
+  double ut = (sp * utp + sm * utm) * rS;
+  double ct = sqrt(g * (0.5 * (Hcp + Hcm)));
+  double rc = 1.0 / ct;
+  double dH = zm - zp, dqn = qnm - qnp, dqt = qtm - qtp;
+  double y = (dqn - un * dH) * rc;
+  double a1 = 0.5 * (dH - y), a3 = 0.5 * (dH + y);
+  double a2 = dqt - ut * dH;
+  double l1 = un - ct, l3 = un + ct;
+  double p1 = fabs(l1) * a1, p3 = fabs(l3) * a3;
+  double D0 = p1 + p3;
+  double Dn = p1 * l1 + p3 * l3;
+  double Dt = fma(fabs(un), a2, D0 * ut);
+  double Pp = (g * zp) * fma(0.5, zp, hq);
+  double Pm = (g * zm) * fma(0.5, zm, hq);
+  double f0 = 0.5 * ((qnp + qnm) - D0);
+  double fn = 0.5 * ((fma(qnp, unp, Pp) + fma(qnm, unm, Pm)) - Dn);
+  double ft = 0.5 * ((qtp * unp + qtm * unm) - Dt);
+  *fz = f0;
+  *fqx = fma(fn, nx, -(ft * ny));
+  *fqy = fma(fn, ny, ft * nx);
+}
+
 /* ------------------------------------------------- deterministic exp / log */
 /* Used only by the Holland wind: the same short algorithm is implemented independently
  * on the CUDA side so that the nodal wind stress is bit-identical.  Accuracy
@@ -577,7 +629,8 @@ static void edge_flux_all(orc_model* m, const double* w, double zeta_b) {
       }
       double hq = hba * T->elam[j][0] + hbb * T->elam[j][1];   /* symmetric in (a,b): same value from either side */
       double fz, fx, fy;
-      orc_llf_flux(m->prm.g, m->prm.h0_dry, nx, ny, hq, zp, qxp, qyp, zm, qxm, qym, bc, zeta_b, &fz, &fx, &fy);
+      if (m->prm.flux == 1) orc_roe_flux(m->prm.g, m->prm.h0_dry, nx, ny, hq, zp, qxp, qyp, zm, qxm, qym, bc, zeta_b, &fz, &fx, &fy);
+      else orc_llf_flux(m->prm.g, m->prm.h0_dry, nx, ny, hq, zp, qxp, qyp, zm, qxm, qym, bc, zeta_b, &fz, &fx, &fy);
       m->flux[(0 * nqe + j) * nd + d] = fz;
       m->flux[(1 * nqe + j) * nd + d] = fx;
       m->flux[(2 * nqe + j) * nd + d] = fy;

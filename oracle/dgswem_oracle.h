@@ -29,7 +29,9 @@ typedef struct {
   int32_t p;          /* 1 or 2 */
   int32_t rk_order;   /* 2: SSP(2,2), 3: SSP(3,3) */
   double g, cf, coriolis_f, h0_dry;
-  int32_t limiter, wetdry;
+  int32_t limiter;    /* 0 off, 1 edge-neighbour Barth-Jespersen [R-7], 2 vertex-neighbourhood Barth-Jespersen [R-18] */
+  int32_t wetdry;
+  int32_t flux;       /* 0 local Lax-Friedrichs [R-3], 1 Roe [R-17] */
 } orc_params;
 
 typedef struct { double x0, y0, vx, vy, rmax, dp, B, rho_air, rho_water, f; } orc_holland;
@@ -57,6 +59,9 @@ typedef struct orc_model orc_model;
 void   orc_basis(double lam0, double lam1, double lam2, double* phi /*[6]*/, double* d1 /*[6]*/, double* d2 /*[6]*/);
 int    orc_make_tables(int p, orc_tables* T);
 void   orc_llf_flux(double g, double h0, double nx, double ny, double hq,
+                    double zp, double qxp, double qyp, double zm, double qxm, double qym,
+                    int bc, double zeta_b, double* fz, double* fqx, double* fqy);
+void   orc_roe_flux(double g, double h0, double nx, double ny, double hq,
                     double zp, double qxp, double qyp, double zm, double qxm, double qym,
                     int bc, double zeta_b, double* fz, double* fqx, double* fqy);
 double orc_det_exp(double x);

@@ -41,7 +41,8 @@ def build(force: bool = False) -> Path:
 
 class Params(C.Structure):
     _fields_ = [("p", C.c_int32), ("rk_order", C.c_int32), ("g", C.c_double), ("cf", C.c_double),
-                ("coriolis_f", C.c_double), ("h0_dry", C.c_double), ("limiter", C.c_int32), ("wetdry", C.c_int32)]
+                ("coriolis_f", C.c_double), ("h0_dry", C.c_double), ("limiter", C.c_int32), ("wetdry", C.c_int32),
+                ("flux", C.c_int32)]
 
 
 class Holland(C.Structure):
@@ -87,6 +88,7 @@ def lib():
     L.orc_basis.argtypes = [D, D, D, PD, PD, PD]
     L.orc_make_tables.argtypes = [C.c_int, C.POINTER(Tables)]
     L.orc_llf_flux.argtypes = [D] * 11 + [C.c_int, D, PD, PD, PD]
+    L.orc_roe_flux.argtypes = [D] * 11 + [C.c_int, D, PD, PD, PD]
     L.orc_det_exp.argtypes = [D]; L.orc_det_exp.restype = D
     L.orc_det_log.argtypes = [D]; L.orc_det_log.restype = D
     L.orc_holland_node.argtypes = [C.POINTER(Holland), D, D, D, D, PD, PD, PD]
@@ -137,6 +139,13 @@ def tables(p: int) -> Tables:
 def llf_flux(g, h0, nx, ny, hq, wp, wm, bc=0, zeta_b=0.0):
     out = [C.c_double() for _ in range(3)]
     lib().orc_llf_flux(g, h0, nx, ny, hq, wp[0], wp[1], wp[2], wm[0], wm[1], wm[2], bc, zeta_b,
+                       *[C.byref(o) for o in out])
+    return np.array([o.value for o in out])
+
+
+def roe_flux(g, h0, nx, ny, hq, wp, wm, bc=0, zeta_b=0.0):
+    out = [C.c_double() for _ in range(3)]
+    lib().orc_roe_flux(g, h0, nx, ny, hq, wp[0], wp[1], wp[2], wm[0], wm[1], wm[2], bc, zeta_b,
                        *[C.byref(o) for o in out])
     return np.array([o.value for o in out])
 
@@ -207,7 +216,8 @@ class Oracle:
     def __init__(self, params: dict, xy, bathy, tri, edge_elem, edge_local, edge_bc, elem_edge):
         L = lib()
         self.L = L
-        self.prm = Params(**{k: params[k] for k in ("p", "rk_order", "g", "cf", "coriolis_f", "h0_dry", "limiter", "wetdry")})
+        self.prm = Params(**{k: params[k] for k in ("p", "rk_order", "g", "cf", "coriolis_f", "h0_dry", "limiter", "wetdry")},
+                          flux=int(params.get("flux", 0)))
         self.p = params["p"]
         self.ndof = (self.p + 1) * (self.p + 2) // 2
         self.nqe = self.p + 1

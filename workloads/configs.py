@@ -60,7 +60,7 @@ def ndof_of(p: int) -> int:
 
 
 def default_params(**kw) -> dict:
-    d = dict(p=1, rk_order=2, g=G, cf=0.0, coriolis_f=0.0, h0_dry=1e-3, limiter=0, wetdry=0)
+    d = dict(p=1, rk_order=2, g=G, cf=0.0, coriolis_f=0.0, h0_dry=1e-3, limiter=0, wetdry=0, flux=0)
     d.update(kw)
     return d
 
