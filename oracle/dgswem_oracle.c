@@ -335,6 +335,31 @@ double orc_limit_var(int p, double* w, const double* mean_nb, const int* has_nb)
   return alpha;
 }
 
+/* Vertex-neighbourhood Barth-Jespersen (the linearity-preserving variant, SURVEY.md 8(c.2) "known weakness" / 8(f)
+ * NEXT-3) [R-18]: the value at vertex v is bounded by the extrema of the means of ALL elements that share that vertex
+ * (vmin[v], vmax[v], the element itself included), not by the three edge neighbours.  Same quotient rule and same
+ * treatment of the quadratic modes as orc_limit_var. */
+double orc_limit_var_vertex(int p, double* w, const double* vmin, const double* vmax) {
+  double ubar = w[0];
+  double b = w[1], c = w[2];
+  double d[3];
+  d[0] = (-b) - c;
+  d[1] = (-b) + c;
+  d[2] = 2.0 * b;
+  double alpha = 1.0;
+  for (int v = 0; v < 3; ++v) {
+    double a;
+    if (d[v] > 0.0) a = (vmax[v] - ubar) / d[v];
+    else if (d[v] < 0.0) a = (vmin[v] - ubar) / d[v];
+    else a = 1.0;
+    if (a < alpha) alpha = a;
+  }
+  w[1] = alpha * b;
+  w[2] = alpha * c;
+  if (p == 2 && alpha < 1.0) { w[3] = 0.0; w[4] = 0.0; w[5] = 0.0; }
+  return alpha;
+}
+
 /* ---------------------------------------------------------------- wet/dry */
 static void vertex_values(const double* w, double* u) {
   /* u(v) = w0 + w1 phi01(v) + w2 phi10(v), phi01 = (-1,-1,2), phi10 = (-1,1,0) */
@@ -504,6 +529,7 @@ struct orc_model {
   int stress_on;      /* ... its wind stress enters the momentum source (default 1) */
   int press_on;       /* ... its surface-pressure gradient enters the momentum source (default 0) [R-15] */
   orc_holland hol;
+  double *nmin, *nmax; /*[3][nn] extrema of the element means around every node (limiter = 2) */
   double* tau;  /*[2][nn]*/
   double* etap; /*[nn] pressure anomaly as a water column */
   double rain;  /* mass source R of eq. (1), m/s, uniform [R-16] */
@@ -577,6 +603,7 @@ orc_model* orc_create(const orc_params* prm, int64_t n_nodes, const double* xy, 
   m->wet = NEW(uint8_t, ne); memset(m->wet, 1, ne);
   m->tau = NEW(double, 2 * n_nodes); memset(m->tau, 0, sizeof(double) * 2 * n_nodes);
   m->etap = NEW(double, n_nodes); memset(m->etap, 0, sizeof(double) * n_nodes);
+  m->nmin = NEW(double, 3 * n_nodes); m->nmax = NEW(double, 3 * n_nodes);
   m->stress_on = 1; m->press_on = 0; m->rain = 0.0;
   m->t = 0.0;
   return m;
@@ -587,7 +614,7 @@ void orc_destroy(orc_model* m) {
   free(m->xy); free(m->bathy); free(m->tri); free(m->edge_elem); free(m->edge_local); free(m->edge_bc);
   free(m->elem_edge); free(m->area); free(m->jinv); free(m->lfac); free(m->hv); free(m->enx); free(m->eny);
   free(m->ehb); free(m->nbr); free(m->w); free(m->w0); free(m->rhs); free(m->flux); free(m->mean);
-  free(m->wet); free(m->tau); free(m->etap); free(m);
+  free(m->wet); free(m->tau); free(m->etap); free(m->nmin); free(m->nmax); free(m);
 }
 
 const orc_tables* orc_get_tables(const orc_model* m) { return &m->T; }
@@ -771,6 +798,37 @@ static void limiter_all(orc_model* m, double* w) {
   const int ndof = m->T.ndof, p = m->T.p;
 #pragma omp parallel for schedule(static)
   for (int64_t e = 0; e < ne; ++e) for (int c = 0; c < 3; ++c) m->mean[c * ne + e] = w[((int64_t)c * ndof) * ne + e];
+  if (m->prm.limiter == 2) {
+    /* extrema of the means of the elements around every node (every incident element counts, wet or dry);
+     * min / max do not depend on the order of the sweep */
+    const int64_t nn = m->n_nodes;
+    for (int c = 0; c < 3; ++c)
+      for (int64_t n = 0; n < nn; ++n) { m->nmin[c * nn + n] = INFINITY; m->nmax[c * nn + n] = -INFINITY; }
+    for (int64_t e = 0; e < ne; ++e)
+      for (int v = 0; v < 3; ++v) {
+        const int64_t n = m->tri[3 * e + v];
+        for (int c = 0; c < 3; ++c) {
+          const double mu = m->mean[c * ne + e];
+          if (mu < m->nmin[c * nn + n]) m->nmin[c * nn + n] = mu;
+          if (mu > m->nmax[c * nn + n]) m->nmax[c * nn + n] = mu;
+        }
+      }
+#pragma omp parallel for schedule(static)
+    for (int64_t e = 0; e < ne; ++e) {
+      if (!m->wet[e]) continue;
+      for (int c = 0; c < 3; ++c) {
+        double wl[ORC_MAXDOF], lo[3], hi[3];
+        for (int k = 0; k < ndof; ++k) wl[k] = w[((int64_t)c * ndof + k) * ne + e];
+        for (int v = 0; v < 3; ++v) {
+          const int64_t n = m->tri[3 * e + v];
+          lo[v] = m->nmin[c * nn + n]; hi[v] = m->nmax[c * nn + n];
+        }
+        orc_limit_var_vertex(p, wl, lo, hi);
+        for (int k = 1; k < ndof; ++k) w[((int64_t)c * ndof + k) * ne + e] = wl[k];
+      }
+    }
+    return;
+  }
 #pragma omp parallel for schedule(static)
   for (int64_t e = 0; e < ne; ++e) {
     if (!m->wet[e]) continue;

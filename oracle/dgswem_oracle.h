@@ -72,6 +72,8 @@ void   orc_holland_node_p(const orc_holland* h, double g, double cx, double cy, 
                           double* tsx, double* tsy, double* V, double* etap);
 /* limiter on one element, one variable; mean_nb[3] neighbour means, has_nb[3] flags */
 double orc_limit_var(int p, double* w /*[ndof]*/, const double* mean_nb, const int* has_nb);
+/* vertex-neighbourhood variant: vmin[3], vmax[3] = extrema of the means of all elements sharing vertex v */
+double orc_limit_var_vertex(int p, double* w /*[ndof]*/, const double* vmin, const double* vmax);
 /* wet/dry on one element: modes [ndof] of ze,qx,qy, vertex bathymetry hv[3]; returns wet flag */
 int    orc_wetdry_elem(const orc_tables* T, double h0, const double* hv, double* ze, double* qx, double* qy);
 /* generic SSP-RK step: w <- one step of size dt, with user RHS and post-stage hooks */

@@ -94,6 +94,7 @@ def lib():
     L.orc_holland_node.argtypes = [C.POINTER(Holland), D, D, D, D, PD, PD, PD]
     L.orc_holland_node_p.argtypes = [C.POINTER(Holland), D, D, D, D, D, PD, PD, PD, PD]
     L.orc_limit_var.argtypes = [C.c_int, PD, PD, C.POINTER(C.c_int)]; L.orc_limit_var.restype = D
+    L.orc_limit_var_vertex.argtypes = [C.c_int, PD, PD, PD]; L.orc_limit_var_vertex.restype = D
     L.orc_wetdry_elem.argtypes = [C.POINTER(Tables), D, PD, PD, PD, PD]; L.orc_wetdry_elem.restype = C.c_int
     L.orc_ssprk_step.argtypes = [C.c_int, I64, PD, PD, PD, D, D, RHS_FN, POST_FN, VP]; L.orc_ssprk_step.restype = C.c_int
     L.orc_create.argtypes = [C.POINTER(Params), I64, PD, PD, I64, C.POINTER(I32), I64, C.POINTER(I32),
@@ -177,6 +178,13 @@ def limit_var(p, w, mean_nb, has_nb):
     mn = np.array(mean_nb, dtype=np.float64)
     hs = (C.c_int * 3)(*[int(h) for h in has_nb])
     alpha = lib().orc_limit_var(p, _dp(w), _dp(mn), hs)
+    return alpha, w
+
+
+def limit_var_vertex(p, w, vmin, vmax):
+    w = np.array(w, dtype=np.float64)
+    lo = np.array(vmin, dtype=np.float64); hi = np.array(vmax, dtype=np.float64)
+    alpha = lib().orc_limit_var_vertex(p, _dp(w), _dp(lo), _dp(hi))
     return alpha, w
 
 
