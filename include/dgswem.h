@@ -44,10 +44,12 @@ typedef struct {
   double  cf;           /* quadratic bottom friction coefficient, 0 = off (R-6)        */
   double  coriolis_f;   /* Coriolis parameter, 0 = off                             */
   double  h0_dry;       /* dry tolerance H0 > 0; also the depth floor in denominators (R-6, R-8) */
-  int32_t limiter;      /* 0/1: slope limiter after every stage (R-7)              */
+  int32_t limiter;      /* slope limiter after every stage: 0 off, 1 edge-neighbour
+                           Barth-Jespersen (R-7), 2 vertex-neighbourhood Barth-Jespersen (R-18)   */
   int32_t wetdry;       /* 0/1: wet/dry pass after every stage (R-8)               */
   int32_t reorder;      /* 0: keep caller's numbering internally; 1: Hilbert-curve renumbering   */
   int32_t device;       /* CUDA device ordinal                                                   */
+  int32_t flux;         /* numerical flux: 0 local Lax-Friedrichs (R-3), 1 Roe (R-17)      */
 } dgswem_params;
 
 /* Holland (1980) vortex, R-9: centre (x0+vx t, y0+vy t), radius of max wind rmax [m],

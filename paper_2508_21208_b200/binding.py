@@ -20,7 +20,7 @@ E_NONFINITE = -4
 class Params(C.Structure):
     _fields_ = [("p", C.c_int32), ("rk_order", C.c_int32), ("g", C.c_double), ("cf", C.c_double),
                 ("coriolis_f", C.c_double), ("h0_dry", C.c_double), ("limiter", C.c_int32), ("wetdry", C.c_int32),
-                ("reorder", C.c_int32), ("device", C.c_int32)]
+                ("reorder", C.c_int32), ("device", C.c_int32), ("flux", C.c_int32)]
 
 
 class Holland(C.Structure):
@@ -133,7 +133,7 @@ class Dgswem:
         assert edge_bc.shape == (self.n_edge,) and elem_edge.shape == (self.n_elem, 3)
         prm = Params(p=self.p, rk_order=self.n_stage, g=params["g"], cf=params["cf"], coriolis_f=params["coriolis_f"],
                      h0_dry=params["h0_dry"], limiter=int(params["limiter"]), wetdry=int(params["wetdry"]),
-                     reorder=int(reorder), device=int(device))
+                     reorder=int(reorder), device=int(device), flux=int(params.get("flux", 0)))
         self.device = torch.device("cuda", device)
         self._tensors = {}
         self.stream = None

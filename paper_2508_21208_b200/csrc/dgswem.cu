@@ -167,6 +167,7 @@ struct dgswem {
 
   // device
   double* W[3] = {nullptr, nullptr, nullptr};
+  double* nmm = nullptr;   // [6][ldn] node extrema of the means (vertex-neighbourhood limiter)
   double *flux = nullptr, *mean = nullptr, *jinv = nullptr, *lfac = nullptr, *hv = nullptr;
   double *en = nullptr, *ehb = nullptr, *tau = nullptr, *etap = nullptr, *nxy = nullptr, *stage_buf = nullptr;
   int2* edge_elem = nullptr;
@@ -327,10 +328,14 @@ int launch_edge(dgswem* h, const double* w, ScalRef zeta_b) {
   const int ntiles = grid_for(h->nd, DGK_EDGE_THREADS);
   const int resident = h->res_edge[P - 1];
   prof_begin(h, PK_EDGE);
-  if (DGK_PIPE_EDGE && resident > 0 && ntiles > resident)
-    k_edge_pipe<P><<<resident, DGK_EDGE_THREADS, 0, h->stream>>>(a, ntiles);
-  else
-    k_edge<P><<<ntiles, DGK_EDGE_THREADS, 0, h->stream>>>(a);
+  const bool pipe = DGK_PIPE_EDGE && resident > 0 && ntiles > resident;
+  if (h->prm.flux == 1) {
+    if (pipe) k_edge_pipe<P, 1><<<resident, DGK_EDGE_THREADS, 0, h->stream>>>(a, ntiles);
+    else k_edge<P, 1><<<ntiles, DGK_EDGE_THREADS, 0, h->stream>>>(a);
+  } else {
+    if (pipe) k_edge_pipe<P, 0><<<resident, DGK_EDGE_THREADS, 0, h->stream>>>(a, ntiles);
+    else k_edge<P, 0><<<ntiles, DGK_EDGE_THREADS, 0, h->stream>>>(a);
+  }
   prof_end(h);
   CKL("k_edge");
   return 0;
@@ -394,7 +399,9 @@ int launch_stage(dgswem* h, const double* win, const double* w0, double* wout, d
   // staging of the next tile's rows in shared memory 445 us, against 374 us)
   prof_begin(h, PK_ELEM);
   const int grid = grid_for(h->ne, DGK_STAGE_THREADS);
-  if constexpr (MODE == MODE_UPDATE) {
+  if (h->prm.flux == 1) {   // Roe: the generic-flag kernel only
+    k_stage<P, MODE, -1, 1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A);
+  } else if constexpr (MODE == MODE_UPDATE) {
     // specialised on (first stage, wind): no w^n registers in stage 1, no wind registers without wind
     switch (stage_variant(h, first)) {
       case 0: k_stage<P, MODE, 0><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
@@ -417,11 +424,18 @@ template <int P>
 int launch_limwd(dgswem* h, double* w) {
   LimArgs A;
   A.w = w; A.mean = h->mean; A.nbr = h->nbr; A.hv = h->hv; A.wet = h->wet; A.ne = (int)h->ne; A.ld = h->ld;
+  A.tri = h->tri; A.nmm = h->nmm; A.ldn = h->ldn;
   A.h0 = h->prm.h0_dry; A.limiter = h->prm.limiter; A.wetdry = h->prm.wetdry;
   prof_begin(h, PK_LIMWD);
   const int ntiles = grid_for(h->ne, 128);
   const int grid = std::max(1, std::min(ntiles, h->res_limwd > 0 ? h->res_limwd : ntiles));
-  k_limwd_tma<P><<<grid, 128, LimTile<P>::kSmem, h->stream>>>(A, ntiles);
+  if (h->prm.limiter == 2) {   // vertex neighbourhood: extrema of the means around every node first
+    k_node_minmax<<<grid_for(h->nn, 256), 256, 0, h->stream>>>(h->nmm, h->ldn, h->mean, h->node_ptr, h->node_ev, (int)h->nn);
+    if (cudaGetLastError() == cudaSuccess) h->launches++;
+    k_limwd_tma<P, 2><<<grid, 128, LimTile<P>::kSmem, h->stream>>>(A, ntiles);
+  } else {
+    k_limwd_tma<P, 1><<<grid, 128, LimTile<P>::kSmem, h->stream>>>(A, ntiles);
+  }
   prof_end(h);
   CKL("k_limwd");
   return 0;
@@ -625,6 +639,8 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     return bail(h->fail(DGSWEM_E_ARG, "bad sizes"));
   if ((prm->p != 1 && prm->p != 2) || (prm->rk_order != 2 && prm->rk_order != 3))
     return bail(h->fail(DGSWEM_E_ARG, "p must be 1 or 2, rk_order 2 or 3"));
+  if (prm->flux < 0 || prm->flux > 1 || prm->limiter < 0 || prm->limiter > 2)
+    return bail(h->fail(DGSWEM_E_ARG, "flux must be 0 (LLF) or 1 (Roe), limiter 0, 1 (edge neighbours) or 2 (vertex neighbourhood)"));
   if (!(prm->h0_dry > 0.0) || !(prm->g > 0.0) || prm->cf < 0.0)
     return bail(h->fail(DGSWEM_E_ARG, "need h0_dry > 0, g > 0, cf >= 0"));
   // range of the kernels' reciprocal / square-root routines (rcp_rn, sqrt_rn): arguments are H_c >= h0_dry and g * H_c
@@ -662,10 +678,16 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     h->res_edge[1] = resident_ctas(k_edge_pipe<2>, DGK_EDGE_THREADS, 0, prm->device);
     // tuning / test knob: DGSWEM_PERSISTENT_CTAS=n caps the persistent grid at n CTAs (so that small
     // meshes walk several tiles per CTA); 0 switches the persistent kernel off
-    CK(cudaFuncSetAttribute(k_limwd_tma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<1>::kSmem));
-    CK(cudaFuncSetAttribute(k_limwd_tma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<2>::kSmem));
-    h->res_limwd = prm->p == 1 ? resident_ctas(k_limwd_tma<1>, 128, LimTile<1>::kSmem, prm->device)
-                               : resident_ctas(k_limwd_tma<2>, 128, LimTile<2>::kSmem, prm->device);
+    CK(cudaFuncSetAttribute(k_limwd_tma<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<1>::kSmem));
+    CK(cudaFuncSetAttribute(k_limwd_tma<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<2>::kSmem));
+    CK(cudaFuncSetAttribute(k_limwd_tma<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<1>::kSmem));
+    CK(cudaFuncSetAttribute(k_limwd_tma<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<2>::kSmem));
+    if (prm->limiter == 2)
+      h->res_limwd = prm->p == 1 ? resident_ctas(k_limwd_tma<1, 2>, 128, LimTile<1>::kSmem, prm->device)
+                                 : resident_ctas(k_limwd_tma<2, 2>, 128, LimTile<2>::kSmem, prm->device);
+    else
+      h->res_limwd = prm->p == 1 ? resident_ctas(k_limwd_tma<1, 1>, 128, LimTile<1>::kSmem, prm->device)
+                                 : resident_ctas(k_limwd_tma<2, 1>, 128, LimTile<2>::kSmem, prm->device);
     if (const char* env = std::getenv("DGSWEM_PERSISTENT_CTAS")) {
       const int cap = std::atoi(env);
 
@@ -814,6 +836,10 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
     h->mean = (double*)h->dalloc((size_t)3 * ld * sizeof(double));
     h->tau = (double*)h->dalloc((size_t)2 * ldn * sizeof(double));
     h->etap = (double*)h->dalloc((size_t)ldn * sizeof(double));
+    if (prm->limiter == 2) {
+      h->nmm = (double*)h->dalloc((size_t)6 * ldn * sizeof(double));
+      if (!h->nmm) return h->fail(DGSWEM_E_CUDA, "device allocation failed");
+    }
     h->stage_buf = (double*)h->dalloc(h->stage_bytes);
     h->wet = (unsigned char*)h->dalloc((size_t)ld);
     h->wet_stage = (unsigned char*)h->dalloc((size_t)ld);
@@ -966,6 +992,8 @@ int dgswem_end_step(dgswem_t* h) {
 
 int dgswem_set_halo(dgswem_t* h, int64_t n_send, const int32_t* send_ids, int64_t n_recv, const int32_t* recv_ids) {
   if (!h) return DGSWEM_E_ARG;
+  if (h->prm.limiter == 2)
+    return h->fail(DGSWEM_E_ARG, "the vertex-neighbourhood limiter needs the elements around every vertex: one layer of edge-neighbour ghosts is not enough");
   if (n_send < 0 || n_recv < 0 || (n_send > 0 && !send_ids) || (n_recv > 0 && !recv_ids)) return h->fail(DGSWEM_E_ARG, "bad halo lists");
   CK(cudaSetDevice(h->prm.device));
   // caller numbering -> internal numbering (host copy of inv_e)

@@ -85,6 +85,9 @@ class PartitionedDgswem:
                  reorder=1, device=0, parts=None, transport=None, part_of_element=None):
         import torch
         from .binding import Dgswem
+        if int(params["limiter"]) == 2:
+            raise ValueError("the vertex-neighbourhood limiter (limiter = 2) needs every element around a vertex; the "
+                             "partitions carry one layer of edge-neighbour ghosts only: use limiter 0 or 1")
         self.torch = torch
         self.subs = partition(xy, tri, edge_elem, edge_local, edge_bc, elem_edge, n_parts, part=part_of_element)
         self.mine = list(range(n_parts)) if parts is None else list(parts)
