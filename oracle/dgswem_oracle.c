@@ -23,6 +23,20 @@
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
+
+/* binary32 build (dgswem_oracle.h): the <math.h> routines called below in their single-precision forms; the tide's
+ * sin() stays binary64 (its arguments are) */
+#ifdef ORC_F32
+#define fma fmaf
+#define sqrt sqrtf
+#define fabs fabsf
+#define rint rintf
+#define ldexp ldexpf
+#define frexp frexpf
+#define ORC_EXP_MAX 80.0f     /* exp arguments beyond +-80 saturate (binary32 range), +-700 in binary64 */
+#else
+#define ORC_EXP_MAX 700.0
+#endif
 #ifdef _OPENMP
 #include <omp.h>
 #endif
@@ -31,24 +45,24 @@
 /* Dubiner orthogonal modal basis on the reference triangle (-1,-1),(1,-1),(-1,1),
  * PAPER.md:97-103 eq. (4); mode order 00, 01, 10, then 02, 11, 20.
  * Input barycentrics; xi_1 = 2 lam_1 - 1, xi_2 = 2 lam_2 - 1.  d1, d2 = d/dxi_1, d/dxi_2. */
-void orc_basis(double lam0, double lam1, double lam2, double* phi, double* d1, double* d2) {
+void orc_basis(real lam0, real lam1, real lam2, real* phi, real* d1, real* d2) {
   (void)lam0;
-  double xi1 = 2.0 * lam1 - 1.0;
-  double xi2 = 2.0 * lam2 - 1.0;
-  double s = 0.5 * (1.0 - xi2);
-  double r = 0.5 * (5.0 * xi2 + 3.0);
-  phi[0] = 1.0;
-  phi[1] = 0.5 * (3.0 * xi2 + 1.0);
-  phi[2] = xi1 + 0.5 * (1.0 + xi2);
-  phi[3] = 0.5 * (((5.0 * xi2) * xi2 + 2.0 * xi2) - 1.0);
+  real xi1 = RL(2.0) * lam1 - RL(1.0);
+  real xi2 = RL(2.0) * lam2 - RL(1.0);
+  real s = RL(0.5) * (RL(1.0) - xi2);
+  real r = RL(0.5) * (RL(5.0) * xi2 + RL(3.0));
+  phi[0] = RL(1.0);
+  phi[1] = RL(0.5) * (RL(3.0) * xi2 + RL(1.0));
+  phi[2] = xi1 + RL(0.5) * (RL(1.0) + xi2);
+  phi[3] = RL(0.5) * (((RL(5.0) * xi2) * xi2 + RL(2.0) * xi2) - RL(1.0));
   phi[4] = phi[2] * r;
-  phi[5] = 0.5 * ((3.0 * phi[2]) * phi[2] - s * s);
-  d1[0] = 0.0;            d2[0] = 0.0;
-  d1[1] = 0.0;            d2[1] = 1.5;
-  d1[2] = 1.0;            d2[2] = 0.5;
-  d1[3] = 0.0;            d2[3] = 5.0 * xi2 + 1.0;
-  d1[4] = r;              d2[4] = 0.5 * r + 2.5 * phi[2];
-  d1[5] = 3.0 * phi[2];   d2[5] = 0.5 * (3.0 * phi[2] + s);
+  phi[5] = RL(0.5) * ((RL(3.0) * phi[2]) * phi[2] - s * s);
+  d1[0] = RL(0.0);            d2[0] = RL(0.0);
+  d1[1] = RL(0.0);            d2[1] = RL(1.5);
+  d1[2] = RL(1.0);            d2[2] = RL(0.5);
+  d1[3] = RL(0.0);            d2[3] = RL(5.0) * xi2 + RL(1.0);
+  d1[4] = r;              d2[4] = RL(0.5) * r + RL(2.5) * phi[2];
+  d1[5] = RL(3.0) * phi[2];   d2[5] = RL(0.5) * (RL(3.0) * phi[2] + s);
 }
 
 /* Quadrature [R-5] (paper: "Gauss-Lobatto", no orders): edges Gauss-Legendre
@@ -61,31 +75,31 @@ int orc_make_tables(int p, orc_tables* T) {
   T->ndof = (p + 1) * (p + 2) / 2;
   T->nqe = p + 1;
   if (p == 1) {
-    T->ge[0] = -0.57735026918962576; T->ge[1] = 0.57735026918962576;
-    T->we[0] = 1.0; T->we[1] = 1.0;
+    T->ge[0] = -RL(0.57735026918962576); T->ge[1] = RL(0.57735026918962576);
+    T->we[0] = RL(1.0); T->we[1] = RL(1.0);
     T->nqa = 3;
     for (int i = 0; i < 3; ++i) {
-      for (int v = 0; v < 3; ++v) T->la[i][v] = (v == i) ? 2.0 / 3.0 : 1.0 / 6.0;
-      T->wa[i] = 2.0 / 3.0;
+      for (int v = 0; v < 3; ++v) T->la[i][v] = (v == i) ? RL(2.0) / RL(3.0) : RL(1.0) / RL(6.0);
+      T->wa[i] = RL(2.0) / RL(3.0);
     }
   } else {
-    T->ge[0] = -0.77459666924148338; T->ge[1] = 0.0; T->ge[2] = 0.77459666924148338;
-    T->we[0] = 5.0 / 9.0; T->we[1] = 8.0 / 9.0; T->we[2] = 5.0 / 9.0;
+    T->ge[0] = -RL(0.77459666924148338); T->ge[1] = RL(0.0); T->ge[2] = RL(0.77459666924148338);
+    T->we[0] = RL(5.0) / RL(9.0); T->we[1] = RL(8.0) / RL(9.0); T->we[2] = RL(5.0) / RL(9.0);
     T->nqa = 6;
-    const double a1 = 0.445948490915965, w1 = 0.223381589678011;
-    const double a2 = 0.091576213509771, w2 = 0.109951743655322;
+    const real a1 = RL(0.445948490915965), w1 = RL(0.223381589678011);
+    const real a2 = RL(0.091576213509771), w2 = RL(0.109951743655322);
     for (int i = 0; i < 3; ++i) {
       for (int v = 0; v < 3; ++v) {
-        T->la[i][v]     = (v == i) ? 1.0 - 2.0 * a1 : a1;
-        T->la[3 + i][v] = (v == i) ? 1.0 - 2.0 * a2 : a2;
+        T->la[i][v]     = (v == i) ? RL(1.0) - RL(2.0) * a1 : a1;
+        T->la[3 + i][v] = (v == i) ? RL(1.0) - RL(2.0) * a2 : a2;
       }
-      T->wa[i] = 2.0 * w1;
-      T->wa[3 + i] = 2.0 * w2;
+      T->wa[i] = RL(2.0) * w1;
+      T->wa[3 + i] = RL(2.0) * w2;
     }
   }
-  const double M[6] = {2.0, 1.0, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 9.0, 2.0 / 15.0};
-  for (int k = 0; k < T->ndof; ++k) T->invM[k] = 1.0 / M[k];
-  double phi[6], d1[6], d2[6];
+  const real M[6] = {RL(2.0), RL(1.0), RL(1.0) / RL(3.0), RL(2.0) / RL(3.0), RL(2.0) / RL(9.0), RL(2.0) / RL(15.0)};
+  for (int k = 0; k < T->ndof; ++k) T->invM[k] = RL(1.0) / M[k];
+  real phi[6], d1[6], d2[6];
   for (int i = 0; i < T->nqa; ++i) {
     orc_basis(T->la[i][0], T->la[i][1], T->la[i][2], phi, d1, d2);
     for (int k = 0; k < T->ndof; ++k) {
@@ -95,14 +109,14 @@ int orc_make_tables(int p, orc_tables* T) {
     }
   }
   for (int j = 0; j < T->nqe; ++j) {
-    T->elam[j][0] = 0.5 * (1.0 - T->ge[j]);
-    T->elam[j][1] = 0.5 * (1.0 + T->ge[j]);
+    T->elam[j][0] = RL(0.5) * (RL(1.0) - T->ge[j]);
+    T->elam[j][1] = RL(0.5) * (RL(1.0) + T->ge[j]);
   }
   /* local edge l runs from local vertex a=(l+1)%3 to b=(l+2)%3 */
   for (int l = 0; l < 3; ++l) {
     int a = (l + 1) % 3, b = (l + 2) % 3;
     for (int j = 0; j < T->nqe; ++j) {
-      double lam[3] = {0.0, 0.0, 0.0};
+      real lam[3] = {RL(0.0), RL(0.0), RL(0.0)};
       lam[a] = T->elam[j][0]; lam[b] = T->elam[j][1];
       orc_basis(lam[0], lam[1], lam[2], phi, d1, d2);
       for (int k = 0; k < T->ndof; ++k) {
@@ -112,8 +126,8 @@ int orc_make_tables(int p, orc_tables* T) {
     }
   }
   for (int v = 0; v < 3; ++v) {
-    double lam[3] = {0.0, 0.0, 0.0};
-    lam[v] = 1.0;
+    real lam[3] = {RL(0.0), RL(0.0), RL(0.0)};
+    lam[v] = RL(1.0);
     orc_basis(lam[0], lam[1], lam[2], phi, d1, d2);
     for (int k = 0; k < T->ndof; ++k) T->phiV[v][k] = phi[k];
   }
@@ -127,12 +141,12 @@ int orc_make_tables(int p, orc_tables* T) {
  * bc: 0 interior, 1 land/wall (mirror: zeta-=zeta+, Qn-=-Qn+, Qt-=Qt+ => mass flux exactly 0),
  *     2 ocean (zeta- = zeta_b, Q- = Q+)   [R-4] (PAPER.md:67 names the boundary types only).
  * Depth floor H_c = max(H, H0) in every denominator and square root [R-6]. */
-void orc_llf_flux(double g, double h0, double nx, double ny, double hq,
-                  double zp, double qxp, double qyp, double zm, double qxm, double qym,
-                  int bc, double zeta_b, double* fz, double* fqx, double* fqy) {
-  double qnp = fma(qyp, ny, qxp * nx);
-  double qtp = fma(qyp, nx, -(qxp * ny));
-  double qnm, qtm;
+void orc_llf_flux(real g, real h0, real nx, real ny, real hq,
+                  real zp, real qxp, real qyp, real zm, real qxm, real qym,
+                  int bc, real zeta_b, real* fz, real* fqx, real* fqy) {
+  real qnp = fma(qyp, ny, qxp * nx);
+  real qtp = fma(qyp, nx, -(qxp * ny));
+  real qnm, qtm;
   if (bc == 0) {
     qnm = fma(qym, ny, qxm * nx);
     qtm = fma(qym, nx, -(qxm * ny));
@@ -141,21 +155,21 @@ void orc_llf_flux(double g, double h0, double nx, double ny, double hq,
   } else {
     zm = zeta_b; qnm = qnp; qtm = qtp;
   }
-  double Hp = zp + hq, Hm = zm + hq;
-  double Hcp = (Hp > h0) ? Hp : h0;
-  double Hcm = (Hm > h0) ? Hm : h0;
-  double rHp = 1.0 / Hcp, rHm = 1.0 / Hcm;
-  double unp = qnp * rHp, unm = qnm * rHm;
-  double cp = sqrt(g * Hcp), cm = sqrt(g * Hcm);
-  double lp = fabs(unp) + cp, lm = fabs(unm) + cm;
-  double lam = (lp > lm) ? lp : lm;
-  double hl = 0.5 * lam;
-  double Pp = (g * zp) * fma(0.5, zp, hq);
-  double Pm = (g * zm) * fma(0.5, zm, hq);
+  real Hp = zp + hq, Hm = zm + hq;
+  real Hcp = (Hp > h0) ? Hp : h0;
+  real Hcm = (Hm > h0) ? Hm : h0;
+  real rHp = RL(1.0) / Hcp, rHm = RL(1.0) / Hcm;
+  real unp = qnp * rHp, unm = qnm * rHm;
+  real cp = sqrt(g * Hcp), cm = sqrt(g * Hcm);
+  real lp = fabs(unp) + cp, lm = fabs(unm) + cm;
+  real lam = (lp > lm) ? lp : lm;
+  real hl = RL(0.5) * lam;
+  real Pp = (g * zp) * fma(RL(0.5), zp, hq);
+  real Pm = (g * zm) * fma(RL(0.5), zm, hq);
   /* each bracket is symmetric in (+,-), so swapping the sides and negating n negates the flux bit for bit */
-  double f0 = fma(-hl, zm - zp, 0.5 * (qnp + qnm));
-  double fn = fma(-hl, qnm - qnp, 0.5 * (fma(qnp, unp, Pp) + fma(qnm, unm, Pm)));
-  double ft = fma(-hl, qtm - qtp, 0.5 * (qtp * unp + qtm * unm));
+  real f0 = fma(-hl, zm - zp, RL(0.5) * (qnp + qnm));
+  real fn = fma(-hl, qnm - qnp, RL(0.5) * (fma(qnp, unp, Pp) + fma(qnm, unm, Pm)));
+  real ft = fma(-hl, qtm - qtp, RL(0.5) * (qtp * unp + qtm * unm));
   *fz = f0;
   *fqx = fma(fn, nx, -(ft * ny));
   *fqy = fma(fn, ny, ft * nx);
@@ -168,12 +182,12 @@ void orc_llf_flux(double g, double h0, double nx, double ny, double hq,
  * lambda2 = un~ with r2 = (0, 0, 1);  F^ = (F(w+) + F(w-))/2 . n - (1/2) sum_k |lambda_k| a_k r_k.  No entropy fix.
  * Every two-term sum pairs a "+"-side with a "-"-side product (or wave 1 with wave 3) and is written without fma, so
  * that swapping the sides and negating n negates the flux bit for bit (as for LLF), and a wall has exactly zero mass flux. */
-void orc_roe_flux(double g, double h0, double nx, double ny, double hq,
-                  double zp, double qxp, double qyp, double zm, double qxm, double qym,
-                  int bc, double zeta_b, double* fz, double* fqx, double* fqy) {
-  double qnp = fma(qyp, ny, qxp * nx);
-  double qtp = fma(qyp, nx, -(qxp * ny));
-  double qnm, qtm;
+void orc_roe_flux(real g, real h0, real nx, real ny, real hq,
+                  real zp, real qxp, real qyp, real zm, real qxm, real qym,
+                  int bc, real zeta_b, real* fz, real* fqx, real* fqy) {
+  real qnp = fma(qyp, ny, qxp * nx);
+  real qtp = fma(qyp, nx, -(qxp * ny));
+  real qnm, qtm;
   if (bc == 0) {
     qnm = fma(qym, ny, qxm * nx);
     qtm = fma(qym, nx, -(qxm * ny));
@@ -182,32 +196,32 @@ void orc_roe_flux(double g, double h0, double nx, double ny, double hq,
   } else {
     zm = zeta_b; qnm = qnp; qtm = qtp;
   }
-  double Hp = zp + hq, Hm = zm + hq;
-  double Hcp = (Hp > h0) ? Hp : h0;
-  double Hcm = (Hm > h0) ? Hm : h0;
-  double rHp = 1.0 / Hcp, rHm = 1.0 / Hcm;
-  double unp = qnp * rHp, unm = qnm * rHm;
-  double utp = qtp * rHp, utm = qtm * rHm;
-  double sp = sqrt(Hcp), sm = sqrt(Hcm);
-  double rS = 1.0 / (sp + sm);
-  double un = (sp * unp + sm * unm) * rS;
-  double ut = (sp * utp + sm * utm) * rS;
-  double ct = sqrt(g * (0.5 * (Hcp + Hcm)));
-  double rc = 1.0 / ct;
-  double dH = zm - zp, dqn = qnm - qnp, dqt = qtm - qtp;
-  double y = (dqn - un * dH) * rc;
-  double a1 = 0.5 * (dH - y), a3 = 0.5 * (dH + y);
-  double a2 = dqt - ut * dH;
-  double l1 = un - ct, l3 = un + ct;
-  double p1 = fabs(l1) * a1, p3 = fabs(l3) * a3;
-  double D0 = p1 + p3;
-  double Dn = p1 * l1 + p3 * l3;
-  double Dt = fma(fabs(un), a2, D0 * ut);
-  double Pp = (g * zp) * fma(0.5, zp, hq);
-  double Pm = (g * zm) * fma(0.5, zm, hq);
-  double f0 = 0.5 * ((qnp + qnm) - D0);
-  double fn = 0.5 * ((fma(qnp, unp, Pp) + fma(qnm, unm, Pm)) - Dn);
-  double ft = 0.5 * ((qtp * unp + qtm * unm) - Dt);
+  real Hp = zp + hq, Hm = zm + hq;
+  real Hcp = (Hp > h0) ? Hp : h0;
+  real Hcm = (Hm > h0) ? Hm : h0;
+  real rHp = RL(1.0) / Hcp, rHm = RL(1.0) / Hcm;
+  real unp = qnp * rHp, unm = qnm * rHm;
+  real utp = qtp * rHp, utm = qtm * rHm;
+  real sp = sqrt(Hcp), sm = sqrt(Hcm);
+  real rS = RL(1.0) / (sp + sm);
+  real un = (sp * unp + sm * unm) * rS;
+  real ut = (sp * utp + sm * utm) * rS;
+  real ct = sqrt(g * (RL(0.5) * (Hcp + Hcm)));
+  real rc = RL(1.0) / ct;
+  real dH = zm - zp, dqn = qnm - qnp, dqt = qtm - qtp;
+  real y = (dqn - un * dH) * rc;
+  real a1 = RL(0.5) * (dH - y), a3 = RL(0.5) * (dH + y);
+  real a2 = dqt - ut * dH;
+  real l1 = un - ct, l3 = un + ct;
+  real p1 = fabs(l1) * a1, p3 = fabs(l3) * a3;
+  real D0 = p1 + p3;
+  real Dn = p1 * l1 + p3 * l3;
+  real Dt = fma(fabs(un), a2, D0 * ut);
+  real Pp = (g * zp) * fma(RL(0.5), zp, hq);
+  real Pm = (g * zm) * fma(RL(0.5), zm, hq);
+  real f0 = RL(0.5) * ((qnp + qnm) - D0);
+  real fn = RL(0.5) * ((fma(qnp, unp, Pp) + fma(qnm, unm, Pm)) - Dn);
+  real ft = RL(0.5) * ((qtp * unp + qtm * unm) - Dt);
   *fz = f0;
   *fqx = fma(fn, nx, -(ft * ny));
   *fqy = fma(fn, ny, ft * nx);
@@ -217,121 +231,123 @@ void orc_roe_flux(double g, double h0, double nx, double ny, double hq,
 /* Used only by the Holland wind: the same short algorithm is implemented independently
  * on the CUDA side so that the nodal wind stress is bit-identical.  Accuracy
  * ~1e-15 relative (pinned against libm in the tests). */
-static const double LN2_HI = 6.93147180369123816490e-01;
-static const double LN2_LO = 1.90821492927058770002e-10;
-static const double INV_LN2 = 1.44269504088896338700e+00;
+static const real LN2_HI = RL(6.93147180369123816490e-01);
+static const real LN2_LO = RL(1.90821492927058770002e-10);
+static const real INV_LN2 = RL(1.44269504088896338700e+00);
 
-double orc_det_exp(double x) {
-  if (x < -700.0) return 0.0;
-  if (x > 700.0) x = 700.0;
-  double kf = rint(x * INV_LN2);
-  double r = fma(-kf, LN2_LO, fma(-kf, LN2_HI, x));
+real orc_det_exp(real x) {
+  if (x < -ORC_EXP_MAX) return RL(0.0);
+  if (x > ORC_EXP_MAX) x = ORC_EXP_MAX;
+  real kf = rint(x * INV_LN2);
+  real r = fma(-kf, LN2_LO, fma(-kf, LN2_HI, x));
   /* Taylor series of e^r, |r| <= 0.35, degree 13, Horner */
-  double q = 1.0 / 6227020800.0;
-  q = fma(q, r, 1.0 / 479001600.0);
-  q = fma(q, r, 1.0 / 39916800.0);
-  q = fma(q, r, 1.0 / 3628800.0);
-  q = fma(q, r, 1.0 / 362880.0);
-  q = fma(q, r, 1.0 / 40320.0);
-  q = fma(q, r, 1.0 / 5040.0);
-  q = fma(q, r, 1.0 / 720.0);
-  q = fma(q, r, 1.0 / 120.0);
-  q = fma(q, r, 1.0 / 24.0);
-  q = fma(q, r, 1.0 / 6.0);
-  q = fma(q, r, 0.5);
-  q = fma(q, r, 1.0);
-  q = fma(q, r, 1.0);
+  real q = RL(1.0) / RL(6227020800.0);
+  q = fma(q, r, RL(1.0) / RL(479001600.0));
+  q = fma(q, r, RL(1.0) / RL(39916800.0));
+  q = fma(q, r, RL(1.0) / RL(3628800.0));
+  q = fma(q, r, RL(1.0) / RL(362880.0));
+  q = fma(q, r, RL(1.0) / RL(40320.0));
+  q = fma(q, r, RL(1.0) / RL(5040.0));
+  q = fma(q, r, RL(1.0) / RL(720.0));
+  q = fma(q, r, RL(1.0) / RL(120.0));
+  q = fma(q, r, RL(1.0) / RL(24.0));
+  q = fma(q, r, RL(1.0) / RL(6.0));
+  q = fma(q, r, RL(0.5));
+  q = fma(q, r, RL(1.0));
+  q = fma(q, r, RL(1.0));
   return ldexp(q, (int)kf);
 }
 
-double orc_det_log(double x) {
+real orc_det_log(real x) {
   /* x > 0, finite, normal.  x = m 2^e, m in [sqrt(1/2), sqrt(2)); log m = 2 atanh(s), s=(m-1)/(m+1) */
   int e;
-  double m = frexp(x, &e);                 /* m in [0.5, 1) */
-  if (m < 0.70710678118654752) { m = 2.0 * m; e = e - 1; }
-  double f = m - 1.0;
-  double s = f / (2.0 + f);
-  double z = s * s;
-  double q = 1.0 / 23.0;
-  q = fma(q, z, 1.0 / 21.0);
-  q = fma(q, z, 1.0 / 19.0);
-  q = fma(q, z, 1.0 / 17.0);
-  q = fma(q, z, 1.0 / 15.0);
-  q = fma(q, z, 1.0 / 13.0);
-  q = fma(q, z, 1.0 / 11.0);
-  q = fma(q, z, 1.0 / 9.0);
-  q = fma(q, z, 1.0 / 7.0);
-  q = fma(q, z, 1.0 / 5.0);
-  q = fma(q, z, 1.0 / 3.0);
-  q = fma(q, z, 1.0);
-  double ef = (double)e;
-  return fma(ef, LN2_LO, fma(ef, LN2_HI, (2.0 * s) * q));
+  real m = frexp(x, &e);                 /* m in [0.5, 1) */
+  if (m < RL(0.70710678118654752)) { m = RL(2.0) * m; e = e - 1; }
+  real f = m - RL(1.0);
+  real s = f / (RL(2.0) + f);
+  real z = s * s;
+  real q = RL(1.0) / RL(23.0);
+  q = fma(q, z, RL(1.0) / RL(21.0));
+  q = fma(q, z, RL(1.0) / RL(19.0));
+  q = fma(q, z, RL(1.0) / RL(17.0));
+  q = fma(q, z, RL(1.0) / RL(15.0));
+  q = fma(q, z, RL(1.0) / RL(13.0));
+  q = fma(q, z, RL(1.0) / RL(11.0));
+  q = fma(q, z, RL(1.0) / RL(9.0));
+  q = fma(q, z, RL(1.0) / RL(7.0));
+  q = fma(q, z, RL(1.0) / RL(5.0));
+  q = fma(q, z, RL(1.0) / RL(3.0));
+  q = fma(q, z, RL(1.0));
+  real ef = (real)e;
+  return fma(ef, LN2_LO, fma(ef, LN2_HI, (RL(2.0) * s) * q));
 }
 
 /* ------------------------------------------------------------------- wind */
 /* WIND (node loops).  [R-9]: analytic Holland (1980) gradient wind about the
  * centre (cx, cy), counter-clockwise; Garratt drag; returns kinematic stress tau_s/rho_0. */
-void orc_holland_node(const orc_holland* h, double cx, double cy, double x, double y,
-                      double* tsx, double* tsy, double* Vout) {
-  orc_holland_node_p(h, 0.0, cx, cy, x, y, tsx, tsy, Vout, NULL);
+void orc_holland_node(const orc_holland* h, double cx, double cy, real x, real y,
+                      real* tsx, real* tsy, real* Vout) {
+  orc_holland_node_p(h, RL(0.0), cx, cy, x, y, tsx, tsy, Vout, NULL);
 }
 
 /* The same with the Holland (1980) surface pressure p(r) = p_c + dp exp(-(R/r)^B): returns in *etap the pressure
  * anomaly against the far field as a water column, eta_p = (p - p_n)/(rho_0 g) = -(dp/(rho_0 g)) (1 - exp(-(R/r)^B))
  * (PAPER.md:65 forcings, :326 "Wind forcing and pressure calculations (WIND)"; [R-15]).  etap may be NULL. */
-void orc_holland_node_p(const orc_holland* h, double g, double cx, double cy, double x, double y,
-                        double* tsx, double* tsy, double* Vout, double* etap) {
-  double dx = x - cx, dy = y - cy;
-  double r = sqrt(fma(dy, dy, dx * dx));
-  if (r < 1.0) {
-    *tsx = 0.0; *tsy = 0.0; if (Vout) *Vout = 0.0;
-    if (etap) *etap = -(h->dp / (h->rho_water * g));
+void orc_holland_node_p(const orc_holland* h, real g, double cx, double cy, real x, real y,
+                        real* tsx, real* tsy, real* Vout, real* etap) {
+  /* the vortex parameters arrive as binary64 (API) and are rounded to the working precision once, here */
+  const real hB = (real)h->B, hrmax = (real)h->rmax, hdp = (real)h->dp, hra = (real)h->rho_air, hrw = (real)h->rho_water, hf = (real)h->f;
+  real dx = x - (real)cx, dy = y - (real)cy;
+  real r = sqrt(fma(dy, dy, dx * dx));
+  if (r < RL(1.0)) {
+    *tsx = RL(0.0); *tsy = RL(0.0); if (Vout) *Vout = RL(0.0);
+    if (etap) *etap = -(hdp / (hrw * g));
     return;
   }
-  double xb = orc_det_exp(h->B * orc_det_log(h->rmax / r));   /* (R/r)^B */
-  double ee = orc_det_exp(-xb);
-  double rf2 = 0.5 * (r * h->f);
-  double V = sqrt(fma((h->B / h->rho_air) * xb, h->dp * ee, rf2 * rf2)) - rf2;
-  double rr = 1.0 / r;
-  double wx = (-(dy * rr)) * V;
-  double wy = (dx * rr) * V;
-  double cd = fma(0.067, V, 0.75) * 1.0e-3;
-  if (cd > 0.0035) cd = 0.0035;
-  double k = ((h->rho_air / h->rho_water) * cd) * V;
+  real xb = orc_det_exp(hB * orc_det_log(hrmax / r));   /* (R/r)^B */
+  real ee = orc_det_exp(-xb);
+  real rf2 = RL(0.5) * (r * hf);
+  real V = sqrt(fma((hB / hra) * xb, hdp * ee, rf2 * rf2)) - rf2;
+  real rr = RL(1.0) / r;
+  real wx = (-(dy * rr)) * V;
+  real wy = (dx * rr) * V;
+  real cd = fma(RL(0.067), V, RL(0.75)) * RL(1.0e-3);
+  if (cd > RL(0.0035)) cd = RL(0.0035);
+  real k = ((hra / hrw) * cd) * V;
   *tsx = k * wx;
   *tsy = k * wy;
   if (Vout) *Vout = V;
-  if (etap) *etap = -((h->dp / (h->rho_water * g)) * (1.0 - ee));
+  if (etap) *etap = -((hdp / (hrw * g)) * (RL(1.0) - ee));
 }
 
 /* ---------------------------------------------------------------- limiter */
 /* SLOPELIM (PAPER.md:109, :326 -- no algorithm given) [R-7]: edge-neighbour Barth-Jespersen
  * on the linear part of one variable.  w[0]=mean; returns alpha in [0,1]. */
-double orc_limit_var(int p, double* w, const double* mean_nb, const int* has_nb) {
-  double ubar = w[0];
-  double umin = ubar, umax = ubar;
+real orc_limit_var(int p, real* w, const real* mean_nb, const int* has_nb) {
+  real ubar = w[0];
+  real umin = ubar, umax = ubar;
   for (int l = 0; l < 3; ++l) {
     if (!has_nb[l]) continue;
-    double m = mean_nb[l];
+    real m = mean_nb[l];
     if (m < umin) umin = m;
     if (m > umax) umax = m;
   }
-  double b = w[1], c = w[2];
-  double d[3];
+  real b = w[1], c = w[2];
+  real d[3];
   d[0] = (-b) - c;
   d[1] = (-b) + c;
-  d[2] = 2.0 * b;
-  double alpha = 1.0;
+  d[2] = RL(2.0) * b;
+  real alpha = RL(1.0);
   for (int v = 0; v < 3; ++v) {
-    double a;
-    if (d[v] > 0.0) a = (umax - ubar) / d[v];
-    else if (d[v] < 0.0) a = (umin - ubar) / d[v];
-    else a = 1.0;
+    real a;
+    if (d[v] > RL(0.0)) a = (umax - ubar) / d[v];
+    else if (d[v] < RL(0.0)) a = (umin - ubar) / d[v];
+    else a = RL(1.0);
     if (a < alpha) alpha = a;
   }
   w[1] = alpha * b;
   w[2] = alpha * c;
-  if (p == 2 && alpha < 1.0) { w[3] = 0.0; w[4] = 0.0; w[5] = 0.0; }
+  if (p == 2 && alpha < RL(1.0)) { w[3] = RL(0.0); w[4] = RL(0.0); w[5] = RL(0.0); }
   return alpha;
 }
 
@@ -339,40 +355,40 @@ double orc_limit_var(int p, double* w, const double* mean_nb, const int* has_nb)
  * NEXT-3) [R-18]: the value at vertex v is bounded by the extrema of the means of ALL elements that share that vertex
  * (vmin[v], vmax[v], the element itself included), not by the three edge neighbours.  Same quotient rule and same
  * treatment of the quadratic modes as orc_limit_var. */
-double orc_limit_var_vertex(int p, double* w, const double* vmin, const double* vmax) {
-  double ubar = w[0];
-  double b = w[1], c = w[2];
-  double d[3];
+real orc_limit_var_vertex(int p, real* w, const real* vmin, const real* vmax) {
+  real ubar = w[0];
+  real b = w[1], c = w[2];
+  real d[3];
   d[0] = (-b) - c;
   d[1] = (-b) + c;
-  d[2] = 2.0 * b;
-  double alpha = 1.0;
+  d[2] = RL(2.0) * b;
+  real alpha = RL(1.0);
   for (int v = 0; v < 3; ++v) {
-    double a;
-    if (d[v] > 0.0) a = (vmax[v] - ubar) / d[v];
-    else if (d[v] < 0.0) a = (vmin[v] - ubar) / d[v];
-    else a = 1.0;
+    real a;
+    if (d[v] > RL(0.0)) a = (vmax[v] - ubar) / d[v];
+    else if (d[v] < RL(0.0)) a = (vmin[v] - ubar) / d[v];
+    else a = RL(1.0);
     if (a < alpha) alpha = a;
   }
   w[1] = alpha * b;
   w[2] = alpha * c;
-  if (p == 2 && alpha < 1.0) { w[3] = 0.0; w[4] = 0.0; w[5] = 0.0; }
+  if (p == 2 && alpha < RL(1.0)) { w[3] = RL(0.0); w[4] = RL(0.0); w[5] = RL(0.0); }
   return alpha;
 }
 
 /* ---------------------------------------------------------------- wet/dry */
-static void vertex_values(const double* w, double* u) {
+static void vertex_values(const real* w, real* u) {
   /* u(v) = w0 + w1 phi01(v) + w2 phi10(v), phi01 = (-1,-1,2), phi10 = (-1,1,0) */
-  double amb = w[0] - w[1];
+  real amb = w[0] - w[1];
   u[0] = amb - w[2];
   u[1] = amb + w[2];
-  u[2] = fma(2.0, w[1], w[0]);
+  u[2] = fma(RL(2.0), w[1], w[0]);
 }
-static void modes_from_vertices(const double* u, double* w) {
-  double a = ((u[0] + u[1]) + u[2]) / 3.0;
+static void modes_from_vertices(const real* u, real* w) {
+  real a = ((u[0] + u[1]) + u[2]) / RL(3.0);
   w[0] = a;
-  w[1] = 0.5 * (u[2] - a);
-  w[2] = 0.5 * (u[1] - u[0]);
+  w[1] = RL(0.5) * (u[2] - a);
+  w[2] = RL(0.5) * (u[1] - u[0]);
 }
 
 /* thin-layer momentum re-assignment (part of [R-8]): vertex weights
@@ -380,30 +396,30 @@ static void modes_from_vertices(const double* u, double* w) {
  * removed momentum R = sum_v (Q_v - w_v Q_v) is handed back in proportion to w_v, so the
  * element total is conserved (unless every w_v = 0: the momentum is dropped).  Identity when
  * every vertex is deeper than H1. */
-static void thin_layer_momentum(double h0, const double* Hh, double* qx, double* qy) {
-  const double h1 = 10.0 * h0;
-  const double rden = 1.0 / (h1 - h0);
-  double wv[3], W = 0.0;
+static void thin_layer_momentum(real h0, const real* Hh, real* qx, real* qy) {
+  const real h1 = RL(10.0) * h0;
+  const real rden = RL(1.0) / (h1 - h0);
+  real wv[3], W = RL(0.0);
   int all_one = 1;
   for (int v = 0; v < 3; ++v) {
-    if (Hh[v] <= h0) wv[v] = 0.0;
-    else if (Hh[v] >= h1) wv[v] = 1.0;
+    if (Hh[v] <= h0) wv[v] = RL(0.0);
+    else if (Hh[v] >= h1) wv[v] = RL(1.0);
     else wv[v] = (Hh[v] - h0) * rden;
-    if (wv[v] != 1.0) all_one = 0;
+    if (wv[v] != RL(1.0)) all_one = 0;
     W = W + wv[v];
   }
   if (all_one) return;
-  double* qq[2] = {qx, qy};
+  real* qq[2] = {qx, qy};
   for (int c = 0; c < 2; ++c) {
-    double qv[3], kept[3];
+    real qv[3], kept[3];
     vertex_values(qq[c], qv);
-    double R = 0.0;
+    real R = RL(0.0);
     for (int v = 0; v < 3; ++v) { kept[v] = wv[v] * qv[v]; R = R + (qv[v] - kept[v]); }
-    if (W > 0.0) {
-      double share = R / W;
+    if (W > RL(0.0)) {
+      real share = R / W;
       for (int v = 0; v < 3; ++v) qv[v] = fma(share, wv[v], kept[v]);
     } else {
-      for (int v = 0; v < 3; ++v) qv[v] = 0.0;
+      for (int v = 0; v < 3; ++v) qv[v] = RL(0.0);
     }
     modes_from_vertices(qv, qq[c]);
   }
@@ -413,49 +429,49 @@ static void thin_layer_momentum(double h0, const double* Hh, double* qx, double*
  * redistribution, SURVEY.md §8(c.3) with the momentum rule replaced by thin_layer_momentum
  * (the survey's equal-share rule pumps momentum into vertices that are
  * barely deeper than H0 and the C4 workload goes non-finite). */
-int orc_wetdry_elem(const orc_tables* T, double h0, const double* hv, double* ze, double* qx, double* qy) {
+int orc_wetdry_elem(const orc_tables* T, real h0, const real* hv, real* ze, real* qx, real* qy) {
   const int ndof = T->ndof;
   if (T->p == 2) {
     /* pre-step: full polynomial depth at the vertices, all edge points, all area points;
      * threshold H1 = 10 H0 so that the linear part below governs every thin element */
-    const double h1 = 10.0 * h0;
+    const real h1 = RL(10.0) * h0;
     int low = 0;
     for (int v = 0; v < 3 && !low; ++v) {
-      double z = ze[0];
+      real z = ze[0];
       for (int k = 1; k < ndof; ++k) z = fma(ze[k], T->phiV[v][k], z);
       if (z + hv[v] <= h1) low = 1;
     }
     for (int l = 0; l < 3 && !low; ++l) {
       int a = (l + 1) % 3, b = (l + 2) % 3;
       for (int j = 0; j < T->nqe && !low; ++j) {
-        double z = ze[0];
+        real z = ze[0];
         for (int k = 1; k < ndof; ++k) z = fma(ze[k], T->phiE[l][j][k], z);
-        double hq = hv[a] * T->elam[j][0] + hv[b] * T->elam[j][1];
+        real hq = hv[a] * T->elam[j][0] + hv[b] * T->elam[j][1];
         if (z + hq <= h1) low = 1;
       }
     }
     for (int i = 0; i < T->nqa && !low; ++i) {
-      double z = ze[0];
+      real z = ze[0];
       for (int k = 1; k < ndof; ++k) z = fma(ze[k], T->phiA[i][k], z);
-      double hq = fma(hv[2], T->la[i][2], fma(hv[1], T->la[i][1], hv[0] * T->la[i][0]));
+      real hq = fma(hv[2], T->la[i][2], fma(hv[1], T->la[i][1], hv[0] * T->la[i][0]));
       if (z + hq <= h1) low = 1;
     }
-    if (low) for (int k = 3; k < 6; ++k) { ze[k] = 0.0; qx[k] = 0.0; qy[k] = 0.0; }
+    if (low) for (int k = 3; k < 6; ++k) { ze[k] = RL(0.0); qx[k] = RL(0.0); qy[k] = RL(0.0); }
   }
-  double zv[3], H[3];
+  real zv[3], H[3];
   vertex_values(ze, zv);
   for (int v = 0; v < 3; ++v) H[v] = zv[v] + hv[v];
   if (H[0] > h0 && H[1] > h0 && H[2] > h0) {                     /* (2) no dry vertex: depths untouched */
     thin_layer_momentum(h0, H, qx, qy);
     return 1;
   }
-  double Hbar = ((H[0] + H[1]) + H[2]) / 3.0;
-  double u[3];
+  real Hbar = ((H[0] + H[1]) + H[2]) / RL(3.0);
+  real u[3];
   if (Hbar <= h0) {                                               /* (3) dry element */
     for (int v = 0; v < 3; ++v) u[v] = Hbar - hv[v];
     modes_from_vertices(u, ze);
-    qx[0] = 0.0; qx[1] = 0.0; qx[2] = 0.0;
-    qy[0] = 0.0; qy[1] = 0.0; qy[2] = 0.0;
+    qx[0] = RL(0.0); qx[1] = RL(0.0); qx[2] = RL(0.0);
+    qy[0] = RL(0.0); qy[1] = RL(0.0); qy[2] = RL(0.0);
     return 0;
   }
   /* (4) partially wet: stable ascending sort of the three vertices by H (ties by index) */
@@ -463,12 +479,12 @@ int orc_wetdry_elem(const orc_tables* T, double h0, const double* hv, double* ze
   if (H[i2] < H[i1]) { tmp = i1; i1 = i2; i2 = tmp; }
   if (H[i3] < H[i2]) { tmp = i2; i2 = i3; i3 = tmp; }
   if (H[i2] < H[i1]) { tmp = i1; i1 = i2; i2 = tmp; }
-  double Hh[3];
+  real Hh[3];
   Hh[i1] = h0;
-  double D1 = h0 - H[i1];
-  double t2 = H[i2] - 0.5 * D1;
+  real D1 = h0 - H[i1];
+  real t2 = H[i2] - RL(0.5) * D1;
   Hh[i2] = (t2 > h0) ? t2 : h0;
-  double D2 = Hh[i2] - H[i2];
+  real D2 = Hh[i2] - H[i2];
   Hh[i3] = (H[i3] - D1) - D2;
   for (int v = 0; v < 3; ++v) u[v] = Hh[v] - hv[v];
   modes_from_vertices(u, ze);
@@ -480,26 +496,26 @@ int orc_wetdry_elem(const orc_tables* T, double h0, const double* hv, double* ze
 /* Shu-Osher SSP(2,2) / SSP(3,3) [R-2] ("optimized SSPRK" whose coefficients the
  * paper does not print; BASELINE configs name SSP-RK2 / RK3).
  *   stage s: u = w^(s-1) + dt L(w^(s-1), t + c_s dt);  w^(s) = u (s=1) or a_s w^0 + b_s u. */
-static const double RK2_A[2] = {0.0, 0.5}, RK2_B[2] = {1.0, 0.5}, RK2_C[2] = {0.0, 1.0};
-static const double RK3_A[3] = {0.0, 0.75, 1.0 / 3.0}, RK3_B[3] = {1.0, 0.25, 2.0 / 3.0}, RK3_C[3] = {0.0, 1.0, 0.5};
+static const real RK2_A[2] = {RL(0.0), RL(0.5)}, RK2_B[2] = {RL(1.0), RL(0.5)}, RK2_C[2] = {RL(0.0), RL(1.0)};
+static const real RK3_A[3] = {RL(0.0), RL(0.75), RL(1.0) / RL(3.0)}, RK3_B[3] = {RL(1.0), RL(0.25), RL(2.0) / RL(3.0)}, RK3_C[3] = {RL(0.0), RL(1.0), RL(0.5)};
 
-int orc_ssprk_step(int order, int64_t n, double* w, double* w0, double* rhs, double t, double dt,
+int orc_ssprk_step(int order, int64_t n, real* w, real* w0, real* rhs, double t, double dt,
                    orc_rhs_fn rhs_fn, orc_post_fn post_fn, void* ctx) {
-  const double *A, *B, *C;
+  const real *A, *B, *C;
   if (order == 2) { A = RK2_A; B = RK2_B; C = RK2_C; }
   else if (order == 3) { A = RK3_A; B = RK3_B; C = RK3_C; }
   else return -1;
-  memcpy(w0, w, (size_t)n * sizeof(double));
+  memcpy(w0, w, (size_t)n * sizeof(real));
   for (int s = 0; s < order; ++s) {
     rhs_fn(ctx, s, t + C[s] * dt, w, rhs);
     if (s == 0) {
 #pragma omp parallel for schedule(static)
       for (int64_t i = 0; i < n; ++i) w[i] = fma(dt, rhs[i], w[i]);
     } else {
-      const double a = A[s], b = B[s];
+      const real a = A[s], b = B[s];
 #pragma omp parallel for schedule(static)
       for (int64_t i = 0; i < n; ++i) {
-        double u = fma(dt, rhs[i], w[i]);
+        real u = fma(dt, rhs[i], w[i]);
         w[i] = fma(b, u, a * w0[i]);
       }
     }
@@ -513,40 +529,40 @@ struct orc_model {
   orc_params prm;
   orc_tables T;
   int64_t n_nodes, n_elem, n_edge;
-  double *xy, *bathy;
+  real *xy, *bathy;
   int32_t *tri, *edge_elem, *edge_bc, *elem_edge;
   int8_t* edge_local;
   /* geometry */
-  double *area, *jinv /*[4][ne]*/, *lfac /*[3][ne]*/, *hv /*[3][ne]*/;
-  double *enx, *eny, *ehb /*[2][nd]*/;
+  real *area, *jinv /*[4][ne]*/, *lfac /*[3][ne]*/, *hv /*[3][ne]*/;
+  real *enx, *eny, *ehb /*[2][nd]*/;
   int32_t* nbr; /*[3][ne]*/
   /* state: w = [3][ndof][ne] contiguous (ze, qx, qy) */
-  double *w, *w0, *rhs, *flux /*[3][nqe][nd]*/, *mean /*[3][ne]*/;
+  real *w, *w0, *rhs, *flux /*[3][nqe][nd]*/, *mean /*[3][ne]*/;
   uint8_t* wet;
-  double t;
+  double t;                                   /* time, tide and storm track stay binary64 in every build */
   double tide_amp, tide_omega, tide_phase;
   int wind_on;        /* a Holland vortex is set */
   int stress_on;      /* ... its wind stress enters the momentum source (default 1) */
   int press_on;       /* ... its surface-pressure gradient enters the momentum source (default 0) [R-15] */
   orc_holland hol;
-  double *nmin, *nmax; /*[3][nn] extrema of the element means around every node (limiter = 2) */
-  double* tau;  /*[2][nn]*/
-  double* etap; /*[nn] pressure anomaly as a water column */
-  double rain;  /* mass source R of eq. (1), m/s, uniform [R-16] */
+  real *nmin, *nmax; /*[3][nn] extrema of the element means around every node (limiter = 2) */
+  real* tau;  /*[2][nn]*/
+  real* etap; /*[nn] pressure anomaly as a water column */
+  real rain;  /* mass source R of eq. (1), m/s, uniform [R-16] */
 };
 
 static void* xmalloc(size_t n) { void* p = malloc(n ? n : 1); if (!p) abort(); return p; }
 #define NEW(T, n) ((T*)xmalloc(sizeof(T) * (size_t)(n)))
 
-orc_model* orc_create(const orc_params* prm, int64_t n_nodes, const double* xy, const double* bathy,
+orc_model* orc_create(const orc_params* prm, int64_t n_nodes, const real* xy, const real* bathy,
                       int64_t n_elem, const int32_t* tri, int64_t n_edge, const int32_t* edge_elem,
                       const int8_t* edge_local, const int32_t* edge_bc, const int32_t* elem_edge) {
   orc_model* m = (orc_model*)calloc(1, sizeof(orc_model));
   m->prm = *prm;
   if (orc_make_tables(prm->p, &m->T) != 0) { free(m); return NULL; }
   m->n_nodes = n_nodes; m->n_elem = n_elem; m->n_edge = n_edge;
-  m->xy = NEW(double, 2 * n_nodes); memcpy(m->xy, xy, sizeof(double) * 2 * n_nodes);
-  m->bathy = NEW(double, n_nodes); memcpy(m->bathy, bathy, sizeof(double) * n_nodes);
+  m->xy = NEW(real, 2 * n_nodes); memcpy(m->xy, xy, sizeof(real) * 2 * n_nodes);
+  m->bathy = NEW(real, n_nodes); memcpy(m->bathy, bathy, sizeof(real) * n_nodes);
   m->tri = NEW(int32_t, 3 * n_elem); memcpy(m->tri, tri, sizeof(int32_t) * 3 * n_elem);
   m->edge_elem = NEW(int32_t, 2 * n_edge); memcpy(m->edge_elem, edge_elem, sizeof(int32_t) * 2 * n_edge);
   m->edge_local = NEW(int8_t, 2 * n_edge); memcpy(m->edge_local, edge_local, 2 * n_edge);
@@ -554,18 +570,18 @@ orc_model* orc_create(const orc_params* prm, int64_t n_nodes, const double* xy, 
   m->elem_edge = NEW(int32_t, 3 * n_elem); memcpy(m->elem_edge, elem_edge, sizeof(int32_t) * 3 * n_elem);
   const int64_t ne = n_elem, nd = n_edge;
   const int ndof = m->T.ndof, nqe = m->T.nqe;
-  m->area = NEW(double, ne); m->jinv = NEW(double, 4 * ne); m->lfac = NEW(double, 3 * ne); m->hv = NEW(double, 3 * ne);
-  m->enx = NEW(double, nd); m->eny = NEW(double, nd); m->ehb = NEW(double, 2 * nd);
+  m->area = NEW(real, ne); m->jinv = NEW(real, 4 * ne); m->lfac = NEW(real, 3 * ne); m->hv = NEW(real, 3 * ne);
+  m->enx = NEW(real, nd); m->eny = NEW(real, nd); m->ehb = NEW(real, 2 * nd);
   m->nbr = NEW(int32_t, 3 * ne);
   /* element geometry (SURVEY.md §8(c.1) "Geometry per element") */
   for (int64_t e = 0; e < ne; ++e) {
     const int32_t* t = tri + 3 * e;
-    double x0 = xy[2 * t[0]], y0 = xy[2 * t[0] + 1];
-    double x1 = xy[2 * t[1]], y1 = xy[2 * t[1] + 1];
-    double x2 = xy[2 * t[2]], y2 = xy[2 * t[2] + 1];
-    double dx1 = x1 - x0, dy1 = y1 - y0, dx2 = x2 - x0, dy2 = y2 - y0;
-    double A = 0.5 * (dx1 * dy2 - dx2 * dy1);
-    double rA = 1.0 / A;
+    real x0 = xy[2 * t[0]], y0 = xy[2 * t[0] + 1];
+    real x1 = xy[2 * t[1]], y1 = xy[2 * t[1] + 1];
+    real x2 = xy[2 * t[2]], y2 = xy[2 * t[2] + 1];
+    real dx1 = x1 - x0, dy1 = y1 - y0, dx2 = x2 - x0, dy2 = y2 - y0;
+    real A = RL(0.5) * (dx1 * dy2 - dx2 * dy1);
+    real rA = RL(1.0) / A;
     m->area[e] = A;
     m->jinv[0 * ne + e] = dy2 * rA;       /* d xi1 / dx */
     m->jinv[1 * ne + e] = (-dx2) * rA;    /* d xi1 / dy */
@@ -573,8 +589,8 @@ orc_model* orc_create(const orc_params* prm, int64_t n_nodes, const double* xy, 
     m->jinv[3 * ne + e] = dx1 * rA;       /* d xi2 / dy */
     for (int l = 0; l < 3; ++l) {
       int a = t[(l + 1) % 3], b = t[(l + 2) % 3];
-      double ex = xy[2 * b] - xy[2 * a], ey = xy[2 * b + 1] - xy[2 * a + 1];
-      double L = sqrt(ex * ex + ey * ey);
+      real ex = xy[2 * b] - xy[2 * a], ey = xy[2 * b + 1] - xy[2 * a + 1];
+      real L = sqrt(ex * ex + ey * ey);
       m->lfac[l * ne + e] = L * rA;
       m->hv[l * ne + e] = bathy[t[l]];
       int32_t d = elem_edge[3 * e + l];
@@ -588,24 +604,24 @@ orc_model* orc_create(const orc_params* prm, int64_t n_nodes, const double* xy, 
     int32_t ep = edge_elem[2 * d];
     int lp = edge_local[2 * d];
     int a = tri[3 * ep + (lp + 1) % 3], b = tri[3 * ep + (lp + 2) % 3];
-    double ex = xy[2 * b] - xy[2 * a], ey = xy[2 * b + 1] - xy[2 * a + 1];
-    double L = sqrt(ex * ex + ey * ey);
-    double rL = 1.0 / L;
+    real ex = xy[2 * b] - xy[2 * a], ey = xy[2 * b + 1] - xy[2 * a + 1];
+    real L = sqrt(ex * ex + ey * ey);
+    real rL = RL(1.0) / L;
     m->enx[d] = ey * rL;
     m->eny[d] = (-ex) * rL;
     m->ehb[0 * nd + d] = bathy[a];
     m->ehb[1 * nd + d] = bathy[b];
   }
-  m->w = NEW(double, 3 * ndof * ne); m->w0 = NEW(double, 3 * ndof * ne); m->rhs = NEW(double, 3 * ndof * ne);
-  memset(m->w, 0, sizeof(double) * 3 * ndof * ne);
-  m->flux = NEW(double, 3 * nqe * nd); memset(m->flux, 0, sizeof(double) * 3 * nqe * nd);
-  m->mean = NEW(double, 3 * ne);
+  m->w = NEW(real, 3 * ndof * ne); m->w0 = NEW(real, 3 * ndof * ne); m->rhs = NEW(real, 3 * ndof * ne);
+  memset(m->w, 0, sizeof(real) * 3 * ndof * ne);
+  m->flux = NEW(real, 3 * nqe * nd); memset(m->flux, 0, sizeof(real) * 3 * nqe * nd);
+  m->mean = NEW(real, 3 * ne);
   m->wet = NEW(uint8_t, ne); memset(m->wet, 1, ne);
-  m->tau = NEW(double, 2 * n_nodes); memset(m->tau, 0, sizeof(double) * 2 * n_nodes);
-  m->etap = NEW(double, n_nodes); memset(m->etap, 0, sizeof(double) * n_nodes);
-  m->nmin = NEW(double, 3 * n_nodes); m->nmax = NEW(double, 3 * n_nodes);
-  m->stress_on = 1; m->press_on = 0; m->rain = 0.0;
-  m->t = 0.0;
+  m->tau = NEW(real, 2 * n_nodes); memset(m->tau, 0, sizeof(real) * 2 * n_nodes);
+  m->etap = NEW(real, n_nodes); memset(m->etap, 0, sizeof(real) * n_nodes);
+  m->nmin = NEW(real, 3 * n_nodes); m->nmax = NEW(real, 3 * n_nodes);
+  m->stress_on = 1; m->press_on = 0; m->rain = RL(0.0);
+  m->t = RL(0.0);
   return m;
 }
 
@@ -624,29 +640,29 @@ const orc_tables* orc_get_tables(const orc_model* m) { return &m->T; }
  * W+- F^ into EDGE_*[e+-, l+-, k] (lines 35-41) the point fluxes are stored per edge and the
  * weights are applied in the gather (north_star: "edge-flux kernel that writes per-edge fluxes
  * to a buffer"); point j is numbered along e+'s local edge, it is point nqe-1-j of e- [R-10]. */
-static void edge_flux_all(orc_model* m, const double* w, double zeta_b) {
+static void edge_flux_all(orc_model* m, const real* w, real zeta_b) {
   const orc_tables* T = &m->T;
   const int64_t ne = m->n_elem, nd = m->n_edge;
   const int ndof = T->ndof, nqe = T->nqe;
-  const double* ze = w; const double* qx = w + (int64_t)ndof * ne; const double* qy = w + 2 * (int64_t)ndof * ne;
+  const real* ze = w; const real* qx = w + (int64_t)ndof * ne; const real* qy = w + 2 * (int64_t)ndof * ne;
 #pragma omp parallel for schedule(static)
   for (int64_t d = 0; d < nd; ++d) {
     int32_t ep = m->edge_elem[2 * d], em = m->edge_elem[2 * d + 1];
     int lp = m->edge_local[2 * d], lm = m->edge_local[2 * d + 1];
     int bc = m->edge_bc[d];
-    double nx = m->enx[d], ny = m->eny[d];
-    double hba = m->ehb[d], hbb = m->ehb[nd + d];
+    real nx = m->enx[d], ny = m->eny[d];
+    real hba = m->ehb[d], hbb = m->ehb[nd + d];
     for (int j = 0; j < nqe; ++j) {
-      const double* php = T->phiE[lp][j];
-      double zp = ze[ep], qxp = qx[ep], qyp = qy[ep];
+      const real* php = T->phiE[lp][j];
+      real zp = ze[ep], qxp = qx[ep], qyp = qy[ep];
       for (int k = 1; k < ndof; ++k) {
         zp = fma(ze[k * ne + ep], php[k], zp);
         qxp = fma(qx[k * ne + ep], php[k], qxp);
         qyp = fma(qy[k * ne + ep], php[k], qyp);
       }
-      double zm = 0.0, qxm = 0.0, qym = 0.0;
+      real zm = RL(0.0), qxm = RL(0.0), qym = RL(0.0);
       if (bc == 0) {
-        const double* phm = T->phiE[lm][nqe - 1 - j];
+        const real* phm = T->phiE[lm][nqe - 1 - j];
         zm = ze[em]; qxm = qx[em]; qym = qy[em];
         for (int k = 1; k < ndof; ++k) {
           zm = fma(ze[k * ne + em], phm[k], zm);
@@ -654,8 +670,8 @@ static void edge_flux_all(orc_model* m, const double* w, double zeta_b) {
           qym = fma(qy[k * ne + em], phm[k], qym);
         }
       }
-      double hq = hba * T->elam[j][0] + hbb * T->elam[j][1];   /* symmetric in (a,b): same value from either side */
-      double fz, fx, fy;
+      real hq = hba * T->elam[j][0] + hbb * T->elam[j][1];   /* symmetric in (a,b): same value from either side */
+      real fz, fx, fy;
       if (m->prm.flux == 1) orc_roe_flux(m->prm.g, m->prm.h0_dry, nx, ny, hq, zp, qxp, qyp, zm, qxm, qym, bc, zeta_b, &fz, &fx, &fy);
       else orc_llf_flux(m->prm.g, m->prm.h0_dry, nx, ny, hq, zp, qxp, qyp, zm, qxm, qym, bc, zeta_b, &fz, &fx, &fy);
       m->flux[(0 * nqe + j) * nd + d] = fz;
@@ -669,25 +685,25 @@ static void edge_flux_all(orc_model* m, const double* w, double zeta_b) {
  * folded into the weights.  rhs_{c,k} =
  *   - sum_l (L_l/A_e) sum_j EDGEFAC[k,j,l] F^_c(l,j) (+ for the e- side)
  *   + sum_i [ XFAC[k,i] F_c,x + YFAC[k,i] F_c,y + SRFAC[k,i] s_c ]      (volume sign + : [R-1]) */
-static void elem_rhs_all(orc_model* m, const double* w, double* rhs, double* scale) {
+static void elem_rhs_all(orc_model* m, const real* w, real* rhs, real* scale) {
   const orc_tables* T = &m->T;
   const int64_t ne = m->n_elem, nd = m->n_edge;
   const int ndof = T->ndof, nqe = T->nqe, nqa = T->nqa;
-  const double g = m->prm.g, h0 = m->prm.h0_dry, cf = m->prm.cf, fc = m->prm.coriolis_f;
-  const double* ze = w; const double* qx = w + (int64_t)ndof * ne; const double* qy = w + 2 * (int64_t)ndof * ne;
+  const real g = m->prm.g, h0 = m->prm.h0_dry, cf = m->prm.cf, fc = m->prm.coriolis_f;
+  const real* ze = w; const real* qx = w + (int64_t)ndof * ne; const real* qy = w + 2 * (int64_t)ndof * ne;
 #pragma omp parallel for schedule(static)
   for (int64_t e = 0; e < ne; ++e) {
-    double r[3][ORC_MAXDOF], sc[3][ORC_MAXDOF];
-    for (int c = 0; c < 3; ++c) for (int k = 0; k < ndof; ++k) { r[c][k] = 0.0; sc[c][k] = 0.0; }
+    real r[3][ORC_MAXDOF], sc[3][ORC_MAXDOF];
+    for (int c = 0; c < 3; ++c) for (int k = 0; k < ndof; ++k) { r[c][k] = RL(0.0); sc[c][k] = RL(0.0); }
     /* ---- GATHER: local edges 0,1,2 in this fixed order (deterministic) ---- */
     for (int l = 0; l < 3; ++l) {
       int32_t d = m->elem_edge[3 * e + l];
       int plus = (m->edge_elem[2 * d] == e && m->edge_local[2 * d] == l);
-      double lf = m->lfac[l * ne + e];
+      real lf = m->lfac[l * ne + e];
       for (int j = 0; j < nqe; ++j) {
         int jj = plus ? j : nqe - 1 - j;
         for (int c = 0; c < 3; ++c) {
-          double t = lf * m->flux[(c * nqe + jj) * nd + d];
+          real t = lf * m->flux[(c * nqe + jj) * nd + d];
           for (int k = 0; k < ndof; ++k) {
             if (plus) r[c][k] = fma(-T->efac[l][j][k], t, r[c][k]); else r[c][k] = fma(T->efac[l][j][k], t, r[c][k]);
             sc[c][k] += fabs(T->efac[l][j][k] * t);
@@ -696,71 +712,71 @@ static void elem_rhs_all(orc_model* m, const double* w, double* rhs, double* sca
       }
     }
     /* ---- AREA ---- */
-    double x1x = m->jinv[e], x1y = m->jinv[ne + e], x2x = m->jinv[2 * ne + e], x2y = m->jinv[3 * ne + e];
-    double hv0 = m->hv[e], hv1 = m->hv[ne + e], hv2 = m->hv[2 * ne + e];
-    double dhx = 0.5 * fma(hv2 - hv0, x2x, (hv1 - hv0) * x1x);   /* grad h_b, constant */
-    double dhy = 0.5 * fma(hv2 - hv0, x2y, (hv1 - hv0) * x1y);
+    real x1x = m->jinv[e], x1y = m->jinv[ne + e], x2x = m->jinv[2 * ne + e], x2y = m->jinv[3 * ne + e];
+    real hv0 = m->hv[e], hv1 = m->hv[ne + e], hv2 = m->hv[2 * ne + e];
+    real dhx = RL(0.5) * fma(hv2 - hv0, x2x, (hv1 - hv0) * x1x);   /* grad h_b, constant */
+    real dhy = RL(0.5) * fma(hv2 - hv0, x2y, (hv1 - hv0) * x1y);
     int wet = m->wet[e];
     const int32_t* tn = m->tri + 3 * e;
     /* gradient of the pressure anomaly eta_p, linear per element from its nodal values (as grad h_b) [R-15] */
-    double dpx = 0.0, dpy = 0.0;
+    real dpx = RL(0.0), dpy = RL(0.0);
     const int press = wet && m->wind_on && m->press_on;
     if (press) {
-      double p0 = m->etap[tn[0]], p1 = m->etap[tn[1]], p2 = m->etap[tn[2]];
-      dpx = 0.5 * fma(p2 - p0, x2x, (p1 - p0) * x1x);
-      dpy = 0.5 * fma(p2 - p0, x2y, (p1 - p0) * x1y);
+      real p0 = m->etap[tn[0]], p1 = m->etap[tn[1]], p2 = m->etap[tn[2]];
+      dpx = RL(0.5) * fma(p2 - p0, x2x, (p1 - p0) * x1x);
+      dpy = RL(0.5) * fma(p2 - p0, x2y, (p1 - p0) * x1y);
     }
-    const double rain = m->rain;
+    const real rain = m->rain;
     for (int i = 0; i < nqa; ++i) {
-      double z = ze[e], u_qx = qx[e], u_qy = qy[e];
+      real z = ze[e], u_qx = qx[e], u_qy = qy[e];
       for (int k = 1; k < ndof; ++k) {                              /* Alg. 1 lines 10-15 */
         z = fma(ze[k * ne + e], T->phiA[i][k], z);
         u_qx = fma(qx[k * ne + e], T->phiA[i][k], u_qx);
         u_qy = fma(qy[k * ne + e], T->phiA[i][k], u_qy);
       }
-      double hq = fma(hv2, T->la[i][2], fma(hv1, T->la[i][1], hv0 * T->la[i][0]));
-      double H = z + hq;
-      double Hc = (H > h0) ? H : h0;
-      double rH = 1.0 / Hc;
-      double u = u_qx * rH, v = u_qy * rH;
-      double gz = g * z;
-      double P = gz * fma(0.5, z, hq);
-      double F[3][2];                                               /* eqs (7)-(9) */
+      real hq = fma(hv2, T->la[i][2], fma(hv1, T->la[i][1], hv0 * T->la[i][0]));
+      real H = z + hq;
+      real Hc = (H > h0) ? H : h0;
+      real rH = RL(1.0) / Hc;
+      real u = u_qx * rH, v = u_qy * rH;
+      real gz = g * z;
+      real P = gz * fma(RL(0.5), z, hq);
+      real F[3][2];                                               /* eqs (7)-(9) */
       F[0][0] = u_qx;         F[0][1] = u_qy;
       F[1][0] = fma(u_qx, u, P); F[1][1] = u_qx * v;
       F[2][0] = F[1][1];         F[2][1] = fma(u_qy, v, P);
-      double tau = 0.0, tsx = 0.0, tsy = 0.0;
+      real tau = RL(0.0), tsx = RL(0.0), tsy = RL(0.0);
       if (wet) {                                                    /* friction, wind: wet elements only [R-6] */
         tau = (cf * sqrt(fma(u_qy, u_qy, u_qx * u_qx))) * (rH * rH);
         if (m->wind_on && m->stress_on) {
           /* wind stress, linear from the three nodes, ramped by the local depth with the same
            * thin-layer weight as the wet/dry momentum rule: clamp((H-H0)/(H1-H0),0,1), H1=10 H0
            * ([R-9]; a millimetre film must not take the full hurricane stress: tau_s/H is stiff) */
-          const double* tx = m->tau; const double* ty = m->tau + m->n_nodes;
-          double ramp;
-          if (H <= h0) ramp = 0.0;
-          else if (H >= 10.0 * h0) ramp = 1.0;
-          else ramp = (H - h0) * (1.0 / (10.0 * h0 - h0));
+          const real* tx = m->tau; const real* ty = m->tau + m->n_nodes;
+          real ramp;
+          if (H <= h0) ramp = RL(0.0);
+          else if (H >= RL(10.0) * h0) ramp = RL(1.0);
+          else ramp = (H - h0) * (RL(1.0) / (RL(10.0) * h0 - h0));
           tsx = ramp * fma(tx[tn[2]], T->la[i][2], fma(tx[tn[1]], T->la[i][1], tx[tn[0]] * T->la[i][0]));
           tsy = ramp * fma(ty[tn[2]], T->la[i][2], fma(ty[tn[1]], T->la[i][1], ty[tn[0]] * T->la[i][0]));
         }
       }
-      double S[3];
+      real S[3];
       S[0] = rain;                                                  /* mass source R of eq. (1) [R-16] */
       S[1] = fma(fc, u_qy, fma(-tau, u_qx, gz * dhx)) + tsx;
       S[2] = fma(-fc, u_qx, fma(-tau, u_qy, gz * dhy)) + tsy;
-      double gH = 0.0;
+      real gH = RL(0.0);
       if (press) {                                                  /* -(H/rho_0) grad p_a = -g H grad eta_p [R-15] */
         gH = g * H;
         S[1] = fma(-gH, dpx, S[1]);
         S[2] = fma(-gH, dpy, S[2]);
       }
       for (int k = 0; k < ndof; ++k) {                              /* Alg. 1 lines 26-35 */
-        double gxk = fma(T->dphiA2[i][k], x2x, T->dphiA1[i][k] * x1x);
-        double gyk = fma(T->dphiA2[i][k], x2y, T->dphiA1[i][k] * x1y);
-        double xf = T->wfac[i][k] * gxk, yf = T->wfac[i][k] * gyk, sf = T->srfac[i][k];
+        real gxk = fma(T->dphiA2[i][k], x2x, T->dphiA1[i][k] * x1x);
+        real gyk = fma(T->dphiA2[i][k], x2y, T->dphiA1[i][k] * x1y);
+        real xf = T->wfac[i][k] * gxk, yf = T->wfac[i][k] * gyk, sf = T->srfac[i][k];
         r[0][k] = fma(yf, F[0][1], fma(xf, F[0][0], r[0][k]));
-        if (rain != 0.0) r[0][k] = fma(sf, S[0], r[0][k]);
+        if (rain != RL(0.0)) r[0][k] = fma(sf, S[0], r[0][k]);
         r[1][k] = fma(sf, S[1], fma(yf, F[1][1], fma(xf, F[1][0], r[1][k])));
         r[2][k] = fma(sf, S[2], fma(yf, F[2][1], fma(xf, F[2][0], r[2][k])));
         for (int c = 0; c < 3; ++c)
@@ -782,7 +798,7 @@ static double tide_value(const orc_model* m, double t) {
   return m->tide_amp * sin(m->tide_omega * t + m->tide_phase);
 }
 
-static void dg_rhs(void* ctx, int stage, double t_stage, const double* w, double* rhs) {
+static void dg_rhs(void* ctx, int stage, double t_stage, const real* w, real* rhs) {
   (void)stage;
   orc_model* m = (orc_model*)ctx;
   edge_flux_all(m, w, tide_value(m, t_stage));
@@ -793,7 +809,7 @@ static void dg_rhs(void* ctx, int stage, double t_stage, const double* w, double
  * wet/dry, [R-7]/[R-8]).  The limiter reads the RK-updated, not yet limited means; it never
  * changes a mean, so the in-place sweep equals the Jacobi sweep.  The wet flag used by the
  * limiter is the one from the end of the previous stage. */
-static void limiter_all(orc_model* m, double* w) {
+static void limiter_all(orc_model* m, real* w) {
   const int64_t ne = m->n_elem;
   const int ndof = m->T.ndof, p = m->T.p;
 #pragma omp parallel for schedule(static)
@@ -808,7 +824,7 @@ static void limiter_all(orc_model* m, double* w) {
       for (int v = 0; v < 3; ++v) {
         const int64_t n = m->tri[3 * e + v];
         for (int c = 0; c < 3; ++c) {
-          const double mu = m->mean[c * ne + e];
+          const real mu = m->mean[c * ne + e];
           if (mu < m->nmin[c * nn + n]) m->nmin[c * nn + n] = mu;
           if (mu > m->nmax[c * nn + n]) m->nmax[c * nn + n] = mu;
         }
@@ -817,7 +833,7 @@ static void limiter_all(orc_model* m, double* w) {
     for (int64_t e = 0; e < ne; ++e) {
       if (!m->wet[e]) continue;
       for (int c = 0; c < 3; ++c) {
-        double wl[ORC_MAXDOF], lo[3], hi[3];
+        real wl[ORC_MAXDOF], lo[3], hi[3];
         for (int k = 0; k < ndof; ++k) wl[k] = w[((int64_t)c * ndof + k) * ne + e];
         for (int v = 0; v < 3; ++v) {
           const int64_t n = m->tri[3 * e + v];
@@ -833,13 +849,13 @@ static void limiter_all(orc_model* m, double* w) {
   for (int64_t e = 0; e < ne; ++e) {
     if (!m->wet[e]) continue;
     for (int c = 0; c < 3; ++c) {
-      double wl[ORC_MAXDOF], mn[3];
+      real wl[ORC_MAXDOF], mn[3];
       int has[3];
       for (int k = 0; k < ndof; ++k) wl[k] = w[((int64_t)c * ndof + k) * ne + e];
       for (int l = 0; l < 3; ++l) {
         int32_t nb = m->nbr[l * ne + e];
         has[l] = nb >= 0;
-        mn[l] = has[l] ? m->mean[c * ne + nb] : 0.0;
+        mn[l] = has[l] ? m->mean[c * ne + nb] : RL(0.0);
       }
       orc_limit_var(p, wl, mn, has);
       for (int k = 1; k < ndof; ++k) w[((int64_t)c * ndof + k) * ne + e] = wl[k];
@@ -847,12 +863,12 @@ static void limiter_all(orc_model* m, double* w) {
   }
 }
 
-static void wetdry_all(orc_model* m, double* w) {
+static void wetdry_all(orc_model* m, real* w) {
   const int64_t ne = m->n_elem;
   const int ndof = m->T.ndof;
 #pragma omp parallel for schedule(static)
   for (int64_t e = 0; e < ne; ++e) {
-    double ze[ORC_MAXDOF], qx[ORC_MAXDOF], qy[ORC_MAXDOF], hv[3];
+    real ze[ORC_MAXDOF], qx[ORC_MAXDOF], qy[ORC_MAXDOF], hv[3];
     for (int k = 0; k < ndof; ++k) {
       ze[k] = w[(0 * (int64_t)ndof + k) * ne + e];
       qx[k] = w[(1 * (int64_t)ndof + k) * ne + e];
@@ -868,7 +884,7 @@ static void wetdry_all(orc_model* m, double* w) {
   }
 }
 
-static void dg_post(void* ctx, int stage, double* w) {
+static void dg_post(void* ctx, int stage, real* w) {
   (void)stage;
   orc_model* m = (orc_model*)ctx;
   if (m->prm.limiter) limiter_all(m, w);
@@ -884,11 +900,11 @@ static void wind_all(orc_model* m, double t) {
     orc_holland_node_p(&m->hol, m->prm.g, cx, cy, m->xy[2 * i], m->xy[2 * i + 1], &m->tau[i], &m->tau[nn + i], NULL, &m->etap[i]);
 }
 
-void orc_set_state(orc_model* m, double t, const double* ze, const double* qx, const double* qy) {
+void orc_set_state(orc_model* m, double t, const real* ze, const real* qx, const real* qy) {
   const int64_t n = (int64_t)m->T.ndof * m->n_elem;
-  memcpy(m->w, ze, sizeof(double) * n);
-  memcpy(m->w + n, qx, sizeof(double) * n);
-  memcpy(m->w + 2 * n, qy, sizeof(double) * n);
+  memcpy(m->w, ze, sizeof(real) * n);
+  memcpy(m->w + n, qx, sizeof(real) * n);
+  memcpy(m->w + 2 * n, qy, sizeof(real) * n);
   m->t = t;
   memset(m->wet, 1, m->n_elem);
   if (m->prm.wetdry) wetdry_all(m, m->w);       /* initialises the wet mask */
@@ -897,11 +913,11 @@ void orc_set_state(orc_model* m, double t, const double* ze, const double* qx, c
 /* TEST HOOKS for the pins of limiter_all / wetdry_all (no arithmetic of their own): load a state and wet flags as
  * given, without the initial wet/dry pass; apply the post-stage sequence SLOPELIM -> WETDRY (either part optional)
  * to the current state exactly as a stage does. */
-void orc_set_state_raw(orc_model* m, double t, const double* ze, const double* qx, const double* qy, const uint8_t* wet) {
+void orc_set_state_raw(orc_model* m, double t, const real* ze, const real* qx, const real* qy, const uint8_t* wet) {
   const int64_t n = (int64_t)m->T.ndof * m->n_elem;
-  memcpy(m->w, ze, sizeof(double) * n);
-  memcpy(m->w + n, qx, sizeof(double) * n);
-  memcpy(m->w + 2 * n, qy, sizeof(double) * n);
+  memcpy(m->w, ze, sizeof(real) * n);
+  memcpy(m->w + n, qx, sizeof(real) * n);
+  memcpy(m->w + 2 * n, qy, sizeof(real) * n);
   m->t = t;
   memcpy(m->wet, wet, (size_t)m->n_elem);
 }
@@ -923,7 +939,7 @@ void orc_set_wind_holland(orc_model* m, const orc_holland* h) {
 void orc_set_wind_forcing(orc_model* m, int stress_on, int press_on) { m->stress_on = stress_on != 0; m->press_on = press_on != 0; }
 
 /* uniform mass source R (rain) in m/s */
-void orc_set_rain(orc_model* m, double rate) { m->rain = rate; }
+void orc_set_rain(orc_model* m, real rate) { m->rain = rate; }
 
 void orc_step(orc_model* m, int64_t nsteps, double dt) {
   const int64_t n = 3 * (int64_t)m->T.ndof * m->n_elem;
@@ -934,71 +950,71 @@ void orc_step(orc_model* m, int64_t nsteps, double dt) {
   }
 }
 
-void orc_eval_rhs(orc_model* m, double* rze, double* rqx, double* rqy, double* sze, double* sqx, double* sqy) {
+void orc_eval_rhs(orc_model* m, real* rze, real* rqx, real* rqy, real* sze, real* sqx, real* sqy) {
   const int64_t n = (int64_t)m->T.ndof * m->n_elem;
   if (m->wind_on) wind_all(m, m->t);
   edge_flux_all(m, m->w, tide_value(m, m->t));
-  double* sc = (sze && sqx && sqy) ? NEW(double, 3 * n) : NULL;
+  real* sc = (sze && sqx && sqy) ? NEW(real, 3 * n) : NULL;
   elem_rhs_all(m, m->w, m->rhs, sc);
-  memcpy(rze, m->rhs, sizeof(double) * n);
-  memcpy(rqx, m->rhs + n, sizeof(double) * n);
-  memcpy(rqy, m->rhs + 2 * n, sizeof(double) * n);
+  memcpy(rze, m->rhs, sizeof(real) * n);
+  memcpy(rqx, m->rhs + n, sizeof(real) * n);
+  memcpy(rqy, m->rhs + 2 * n, sizeof(real) * n);
   if (sc) {
-    memcpy(sze, sc, sizeof(double) * n); memcpy(sqx, sc + n, sizeof(double) * n); memcpy(sqy, sc + 2 * n, sizeof(double) * n);
+    memcpy(sze, sc, sizeof(real) * n); memcpy(sqx, sc + n, sizeof(real) * n); memcpy(sqy, sc + 2 * n, sizeof(real) * n);
     free(sc);
   }
 }
 
-void orc_get_flux(orc_model* m, double* flux) {
-  memcpy(flux, m->flux, sizeof(double) * 3 * (size_t)m->T.nqe * (size_t)m->n_edge);
+void orc_get_flux(orc_model* m, real* flux) {
+  memcpy(flux, m->flux, sizeof(real) * 3 * (size_t)m->T.nqe * (size_t)m->n_edge);
 }
 
-void orc_get_state(orc_model* m, double* t, double* ze, double* qx, double* qy) {
+void orc_get_state(orc_model* m, double* t, real* ze, real* qx, real* qy) {
   const int64_t n = (int64_t)m->T.ndof * m->n_elem;
   if (t) *t = m->t;
-  memcpy(ze, m->w, sizeof(double) * n);
-  memcpy(qx, m->w + n, sizeof(double) * n);
-  memcpy(qy, m->w + 2 * n, sizeof(double) * n);
+  memcpy(ze, m->w, sizeof(real) * n);
+  memcpy(qx, m->w + n, sizeof(real) * n);
+  memcpy(qy, m->w + 2 * n, sizeof(real) * n);
 }
 
 /* Nodal output ("to output the state variables, we convert the modal representation to a nodal
  * representation by averaging the neighboring elements of each node"): value of every incident element's polynomial at
  * the node (basis at the vertices, modes k ascending), summed in ascending element order, divided by the count. */
-void orc_get_nodal(orc_model* m, double* zn, double* qxn, double* qyn) {
+void orc_get_nodal(orc_model* m, real* zn, real* qxn, real* qyn) {
   const int64_t ne = m->n_elem, nn = m->n_nodes;
   const int ndof = m->T.ndof;
-  double* out[3] = {zn, qxn, qyn};
+  real* out[3] = {zn, qxn, qyn};
   int32_t* cnt = (int32_t*)calloc((size_t)nn, sizeof(int32_t));
-  for (int c = 0; c < 3; ++c) for (int64_t n = 0; n < nn; ++n) out[c][n] = 0.0;
+  for (int c = 0; c < 3; ++c) for (int64_t n = 0; n < nn; ++n) out[c][n] = RL(0.0);
   for (int64_t e = 0; e < ne; ++e) {
     for (int v = 0; v < 3; ++v) {
       const int64_t n = m->tri[3 * e + v];
       for (int c = 0; c < 3; ++c) {
-        const double* w = m->w + ((int64_t)c * ndof) * ne;
-        double val = w[e];
+        const real* w = m->w + ((int64_t)c * ndof) * ne;
+        real val = w[e];
         for (int k = 1; k < ndof; ++k) val = fma(w[(int64_t)k * ne + e], m->T.phiV[v][k], val);
         out[c][n] = out[c][n] + val;
       }
       cnt[n] += 1;
     }
   }
-  for (int c = 0; c < 3; ++c) for (int64_t n = 0; n < nn; ++n) if (cnt[n] > 0) out[c][n] = out[c][n] / (double)cnt[n];
+  for (int c = 0; c < 3; ++c) for (int64_t n = 0; n < nn; ++n) if (cnt[n] > 0) out[c][n] = out[c][n] / (real)cnt[n];
   free(cnt);
 }
 
 void orc_get_wetdry(orc_model* m, uint8_t* wet) { memcpy(wet, m->wet, (size_t)m->n_elem); }
 
-void orc_get_geometry(orc_model* m, double* area, double* jinv, double* lfac, double* enx, double* eny) {
-  if (area) memcpy(area, m->area, sizeof(double) * m->n_elem);
-  if (jinv) memcpy(jinv, m->jinv, sizeof(double) * 4 * m->n_elem);
-  if (lfac) memcpy(lfac, m->lfac, sizeof(double) * 3 * m->n_elem);
-  if (enx) memcpy(enx, m->enx, sizeof(double) * m->n_edge);
-  if (eny) memcpy(eny, m->eny, sizeof(double) * m->n_edge);
+void orc_get_geometry(orc_model* m, real* area, real* jinv, real* lfac, real* enx, real* eny) {
+  if (area) memcpy(area, m->area, sizeof(real) * m->n_elem);
+  if (jinv) memcpy(jinv, m->jinv, sizeof(real) * 4 * m->n_elem);
+  if (lfac) memcpy(lfac, m->lfac, sizeof(real) * 3 * m->n_elem);
+  if (enx) memcpy(enx, m->enx, sizeof(real) * m->n_edge);
+  if (eny) memcpy(eny, m->eny, sizeof(real) * m->n_edge);
 }
 
-void orc_get_wind(orc_model* m, double* tau) { memcpy(tau, m->tau, sizeof(double) * 2 * m->n_nodes); }
+void orc_get_wind(orc_model* m, real* tau) { memcpy(tau, m->tau, sizeof(real) * 2 * m->n_nodes); }
 
-void orc_get_pressure(orc_model* m, double* etap) { memcpy(etap, m->etap, sizeof(double) * m->n_nodes); }
+void orc_get_pressure(orc_model* m, real* etap) { memcpy(etap, m->etap, sizeof(real) * m->n_nodes); }
 
 int orc_num_threads(void) {
 #ifdef _OPENMP

@@ -16,7 +16,12 @@ import numpy as np
 HERE = Path(__file__).resolve().parent
 SRC = HERE / "dgswem_oracle.c"
 HDR = HERE / "dgswem_oracle.h"
-LIB = HERE / "liborc.so"
+# working precision of this module instance: binary64, or binary32 when loaded through oracle/oracle32.py (-DORC_F32 build
+# of the same source; arrays in and out are then float32, time / tide / storm-track scalars stay Python floats = binary64)
+F32 = bool(globals().get("_ORC_F32", False))
+REAL = C.c_float if F32 else C.c_double
+NP = np.float32 if F32 else np.float64
+LIB = HERE / ("liborc32.so" if F32 else "liborc.so")
 
 MAXDOF, MAXQA, MAXQE = 6, 6, 3
 
@@ -26,7 +31,7 @@ def build(force: bool = False) -> Path:
     if (not force and LIB.exists() and LIB.stat().st_mtime >= max(SRC.stat().st_mtime, HDR.stat().st_mtime)):
         return LIB
     tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
-    cmd = ["gcc", "-std=c99", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared",
+    cmd = ["gcc", "-std=c99"] + (["-DORC_F32"] if F32 else []) + ["-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared",
            "-Wall", "-Wextra", "-o", str(tmp), str(SRC), "-lm"]
     # fma() calls become one instruction where the CPU has it (same result: fma is correctly rounded either way)
     try:
@@ -40,8 +45,8 @@ def build(force: bool = False) -> Path:
 
 
 class Params(C.Structure):
-    _fields_ = [("p", C.c_int32), ("rk_order", C.c_int32), ("g", C.c_double), ("cf", C.c_double),
-                ("coriolis_f", C.c_double), ("h0_dry", C.c_double), ("limiter", C.c_int32), ("wetdry", C.c_int32),
+    _fields_ = [("p", C.c_int32), ("rk_order", C.c_int32), ("g", REAL), ("cf", REAL),
+                ("coriolis_f", REAL), ("h0_dry", REAL), ("limiter", C.c_int32), ("wetdry", C.c_int32),
                 ("flux", C.c_int32)]
 
 
@@ -51,31 +56,32 @@ class Holland(C.Structure):
 
 class Tables(C.Structure):
     _fields_ = [("p", C.c_int32), ("ndof", C.c_int32), ("nqe", C.c_int32), ("nqa", C.c_int32),
-                ("ge", C.c_double * MAXQE), ("we", C.c_double * MAXQE),
-                ("elam", (C.c_double * 2) * MAXQE),
-                ("la", (C.c_double * 3) * MAXQA), ("wa", C.c_double * MAXQA),
-                ("invM", C.c_double * MAXDOF),
-                ("phiA", (C.c_double * MAXDOF) * MAXQA),
-                ("dphiA1", (C.c_double * MAXDOF) * MAXQA),
-                ("dphiA2", (C.c_double * MAXDOF) * MAXQA),
-                ("phiE", ((C.c_double * MAXDOF) * MAXQE) * 3),
-                ("wfac", (C.c_double * MAXDOF) * MAXQA),
-                ("srfac", (C.c_double * MAXDOF) * MAXQA),
-                ("efac", ((C.c_double * MAXDOF) * MAXQE) * 3),
-                ("phiV", (C.c_double * MAXDOF) * 3)]
+                ("ge", REAL * MAXQE), ("we", REAL * MAXQE),
+                ("elam", (REAL * 2) * MAXQE),
+                ("la", (REAL * 3) * MAXQA), ("wa", REAL * MAXQA),
+                ("invM", REAL * MAXDOF),
+                ("phiA", (REAL * MAXDOF) * MAXQA),
+                ("dphiA1", (REAL * MAXDOF) * MAXQA),
+                ("dphiA2", (REAL * MAXDOF) * MAXQA),
+                ("phiE", ((REAL * MAXDOF) * MAXQE) * 3),
+                ("wfac", (REAL * MAXDOF) * MAXQA),
+                ("srfac", (REAL * MAXDOF) * MAXQA),
+                ("efac", ((REAL * MAXDOF) * MAXQE) * 3),
+                ("phiV", (REAL * MAXDOF) * 3)]
 
     def np(self, name):
         return np.ctypeslib.as_array(getattr(self, name)).copy()
 
 
-RHS_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_int, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double))
-POST_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_int, C.POINTER(C.c_double))
+RHS_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_int, C.c_double, C.POINTER(REAL), C.POINTER(REAL))
+POST_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_int, C.POINTER(REAL))
 
 _lib = None
 
 
 def _dp(a):
-    return a.ctypes.data_as(C.POINTER(C.c_double))
+    assert a.dtype == NP, a.dtype
+    return a.ctypes.data_as(C.POINTER(REAL))
 
 
 def lib():
@@ -83,41 +89,42 @@ def lib():
     if _lib is not None:
         return _lib
     L = C.CDLL(str(build()))
-    D, I32, I64, VP = C.c_double, C.c_int32, C.c_int64, C.c_void_p
-    PD = C.POINTER(C.c_double)
-    L.orc_basis.argtypes = [D, D, D, PD, PD, PD]
+    # R = working precision (`real`), D = binary64 scalars that stay binary64 in every build (time, dt, tide, storm centre)
+    R, D, I32, I64, VP = REAL, C.c_double, C.c_int32, C.c_int64, C.c_void_p
+    PR = C.POINTER(REAL)
+    L.orc_basis.argtypes = [R, R, R, PR, PR, PR]
     L.orc_make_tables.argtypes = [C.c_int, C.POINTER(Tables)]
-    L.orc_llf_flux.argtypes = [D] * 11 + [C.c_int, D, PD, PD, PD]
-    L.orc_roe_flux.argtypes = [D] * 11 + [C.c_int, D, PD, PD, PD]
-    L.orc_det_exp.argtypes = [D]; L.orc_det_exp.restype = D
-    L.orc_det_log.argtypes = [D]; L.orc_det_log.restype = D
-    L.orc_holland_node.argtypes = [C.POINTER(Holland), D, D, D, D, PD, PD, PD]
-    L.orc_holland_node_p.argtypes = [C.POINTER(Holland), D, D, D, D, D, PD, PD, PD, PD]
-    L.orc_limit_var.argtypes = [C.c_int, PD, PD, C.POINTER(C.c_int)]; L.orc_limit_var.restype = D
-    L.orc_limit_var_vertex.argtypes = [C.c_int, PD, PD, PD]; L.orc_limit_var_vertex.restype = D
-    L.orc_wetdry_elem.argtypes = [C.POINTER(Tables), D, PD, PD, PD, PD]; L.orc_wetdry_elem.restype = C.c_int
-    L.orc_ssprk_step.argtypes = [C.c_int, I64, PD, PD, PD, D, D, RHS_FN, POST_FN, VP]; L.orc_ssprk_step.restype = C.c_int
-    L.orc_create.argtypes = [C.POINTER(Params), I64, PD, PD, I64, C.POINTER(I32), I64, C.POINTER(I32),
+    L.orc_llf_flux.argtypes = [R] * 11 + [C.c_int, R, PR, PR, PR]
+    L.orc_roe_flux.argtypes = [R] * 11 + [C.c_int, R, PR, PR, PR]
+    L.orc_det_exp.argtypes = [R]; L.orc_det_exp.restype = R
+    L.orc_det_log.argtypes = [R]; L.orc_det_log.restype = R
+    L.orc_holland_node.argtypes = [C.POINTER(Holland), D, D, R, R, PR, PR, PR]
+    L.orc_holland_node_p.argtypes = [C.POINTER(Holland), R, D, D, R, R, PR, PR, PR, PR]
+    L.orc_limit_var.argtypes = [C.c_int, PR, PR, C.POINTER(C.c_int)]; L.orc_limit_var.restype = R
+    L.orc_limit_var_vertex.argtypes = [C.c_int, PR, PR, PR]; L.orc_limit_var_vertex.restype = R
+    L.orc_wetdry_elem.argtypes = [C.POINTER(Tables), R, PR, PR, PR, PR]; L.orc_wetdry_elem.restype = C.c_int
+    L.orc_ssprk_step.argtypes = [C.c_int, I64, PR, PR, PR, D, D, RHS_FN, POST_FN, VP]; L.orc_ssprk_step.restype = C.c_int
+    L.orc_create.argtypes = [C.POINTER(Params), I64, PR, PR, I64, C.POINTER(I32), I64, C.POINTER(I32),
                              C.POINTER(C.c_int8), C.POINTER(I32), C.POINTER(I32)]
     L.orc_create.restype = VP
     L.orc_destroy.argtypes = [VP]
     L.orc_get_tables.argtypes = [VP]; L.orc_get_tables.restype = C.POINTER(Tables)
-    L.orc_set_state.argtypes = [VP, D, PD, PD, PD]
-    L.orc_set_state_raw.argtypes = [VP, D, PD, PD, PD, C.POINTER(C.c_uint8)]
+    L.orc_set_state.argtypes = [VP, D, PR, PR, PR]
+    L.orc_set_state_raw.argtypes = [VP, D, PR, PR, PR, C.POINTER(C.c_uint8)]
     L.orc_apply_post.argtypes = [VP, C.c_int, C.c_int]
     L.orc_set_tide.argtypes = [VP, D, D, D]
     L.orc_set_wind_holland.argtypes = [VP, C.POINTER(Holland)]
     L.orc_set_wind_forcing.argtypes = [VP, C.c_int, C.c_int]
-    L.orc_set_rain.argtypes = [VP, D]
-    L.orc_get_pressure.argtypes = [VP, PD]
+    L.orc_set_rain.argtypes = [VP, R]
+    L.orc_get_pressure.argtypes = [VP, PR]
     L.orc_step.argtypes = [VP, I64, D]
-    L.orc_eval_rhs.argtypes = [VP, PD, PD, PD, PD, PD, PD]
-    L.orc_get_flux.argtypes = [VP, PD]
-    L.orc_get_state.argtypes = [VP, PD, PD, PD, PD]
+    L.orc_eval_rhs.argtypes = [VP, PR, PR, PR, PR, PR, PR]
+    L.orc_get_flux.argtypes = [VP, PR]
+    L.orc_get_state.argtypes = [VP, C.POINTER(C.c_double), PR, PR, PR]
     L.orc_get_wetdry.argtypes = [VP, C.POINTER(C.c_uint8)]
-    L.orc_get_geometry.argtypes = [VP, PD, PD, PD, PD, PD]
-    L.orc_get_wind.argtypes = [VP, PD]
-    L.orc_get_nodal.argtypes = [VP, PD, PD, PD]
+    L.orc_get_geometry.argtypes = [VP, PR, PR, PR, PR, PR]
+    L.orc_get_wind.argtypes = [VP, PR]
+    L.orc_get_nodal.argtypes = [VP, PR, PR, PR]
     L.orc_get_nodal.restype = None
     L.orc_num_threads.restype = C.c_int
     _lib = L
@@ -126,7 +133,7 @@ def lib():
 
 # ------------------------------------------------------------------ piece-level helpers
 def basis(lam0, lam1, lam2):
-    phi, d1, d2 = (np.zeros(6) for _ in range(3))
+    phi, d1, d2 = (np.zeros(6, dtype=NP) for _ in range(3))
     lib().orc_basis(lam0, lam1, lam2, _dp(phi), _dp(d1), _dp(d2))
     return phi, d1, d2
 
@@ -138,14 +145,14 @@ def tables(p: int) -> Tables:
 
 
 def llf_flux(g, h0, nx, ny, hq, wp, wm, bc=0, zeta_b=0.0):
-    out = [C.c_double() for _ in range(3)]
+    out = [REAL() for _ in range(3)]
     lib().orc_llf_flux(g, h0, nx, ny, hq, wp[0], wp[1], wp[2], wm[0], wm[1], wm[2], bc, zeta_b,
                        *[C.byref(o) for o in out])
     return np.array([o.value for o in out])
 
 
 def roe_flux(g, h0, nx, ny, hq, wp, wm, bc=0, zeta_b=0.0):
-    out = [C.c_double() for _ in range(3)]
+    out = [REAL() for _ in range(3)]
     lib().orc_roe_flux(g, h0, nx, ny, hq, wp[0], wp[1], wp[2], wm[0], wm[1], wm[2], bc, zeta_b,
                        *[C.byref(o) for o in out])
     return np.array([o.value for o in out])
@@ -161,46 +168,46 @@ def det_log(x):
 
 def holland_node(hol: dict, cx, cy, x, y):
     h = Holland(**hol)
-    out = [C.c_double() for _ in range(3)]
+    out = [REAL() for _ in range(3)]
     lib().orc_holland_node(C.byref(h), cx, cy, x, y, *[C.byref(o) for o in out])
     return tuple(o.value for o in out)   # tsx, tsy, V
 
 
 def holland_node_p(hol: dict, g, cx, cy, x, y):
     h = Holland(**hol)
-    out = [C.c_double() for _ in range(4)]
+    out = [REAL() for _ in range(4)]
     lib().orc_holland_node_p(C.byref(h), g, cx, cy, x, y, *[C.byref(o) for o in out])
     return tuple(o.value for o in out)   # tsx, tsy, V, eta_p
 
 
 def limit_var(p, w, mean_nb, has_nb):
-    w = np.array(w, dtype=np.float64)
-    mn = np.array(mean_nb, dtype=np.float64)
+    w = np.array(w, dtype=NP)
+    mn = np.array(mean_nb, dtype=NP)
     hs = (C.c_int * 3)(*[int(h) for h in has_nb])
     alpha = lib().orc_limit_var(p, _dp(w), _dp(mn), hs)
     return alpha, w
 
 
 def limit_var_vertex(p, w, vmin, vmax):
-    w = np.array(w, dtype=np.float64)
-    lo = np.array(vmin, dtype=np.float64); hi = np.array(vmax, dtype=np.float64)
+    w = np.array(w, dtype=NP)
+    lo = np.array(vmin, dtype=NP); hi = np.array(vmax, dtype=NP)
     alpha = lib().orc_limit_var_vertex(p, _dp(w), _dp(lo), _dp(hi))
     return alpha, w
 
 
 def wetdry_elem(p, h0, hv, ze, qx, qy):
     T = tables(p)
-    hv = np.array(hv, dtype=np.float64)
-    ze, qx, qy = (np.array(a, dtype=np.float64) for a in (ze, qx, qy))
+    hv = np.array(hv, dtype=NP)
+    ze, qx, qy = (np.array(a, dtype=NP) for a in (ze, qx, qy))
     wet = lib().orc_wetdry_elem(C.byref(T), h0, _dp(hv), _dp(ze), _dp(qx), _dp(qy))
     return wet, ze, qx, qy
 
 
 def ssprk_step(order, w, t, dt, rhs_py, post_py=None):
     """One SSP-RK step with a Python RHS rhs_py(stage, t_stage, w)->array."""
-    w = np.array(w, dtype=np.float64)
+    w = np.array(w, dtype=NP)
     n = w.size
-    w0, rhs = np.zeros(n), np.zeros(n)
+    w0, rhs = np.zeros(n, dtype=NP), np.zeros(n, dtype=NP)
 
     def _rhs(ctx, stage, ts, wp, rp):
         wa = np.ctypeslib.as_array(wp, shape=(n,))
@@ -229,8 +236,8 @@ class Oracle:
         self.p = params["p"]
         self.ndof = (self.p + 1) * (self.p + 2) // 2
         self.nqe = self.p + 1
-        xy = np.ascontiguousarray(xy, dtype=np.float64)
-        bathy = np.ascontiguousarray(bathy, dtype=np.float64)
+        xy = np.ascontiguousarray(xy, dtype=NP)
+        bathy = np.ascontiguousarray(bathy, dtype=NP)
         tri = np.ascontiguousarray(tri, dtype=np.int32)
         edge_elem = np.ascontiguousarray(edge_elem, dtype=np.int32)
         edge_local = np.ascontiguousarray(edge_local, dtype=np.int8)
@@ -274,7 +281,7 @@ class Oracle:
         return self.L.orc_get_tables(self.h).contents
 
     def _chk(self, a):
-        a = np.ascontiguousarray(a, dtype=np.float64)
+        a = np.ascontiguousarray(a, dtype=NP)
         assert a.shape == (self.ndof, self.n_elem), a.shape
         return a
 
@@ -309,7 +316,7 @@ class Oracle:
         self.L.orc_set_rain(self.h, float(rate))
 
     def get_pressure(self):
-        p = np.zeros(self.n_nodes)
+        p = np.zeros(self.n_nodes, dtype=NP)
         self.L.orc_get_pressure(self.h, _dp(p))
         return p
 
@@ -318,22 +325,22 @@ class Oracle:
 
     def eval_rhs(self, with_scale=False):
         shp = (self.ndof, self.n_elem)
-        r = [np.zeros(shp) for _ in range(3)]
+        r = [np.zeros(shp, dtype=NP) for _ in range(3)]
         if with_scale:
-            s = [np.zeros(shp) for _ in range(3)]
+            s = [np.zeros(shp, dtype=NP) for _ in range(3)]
             self.L.orc_eval_rhs(self.h, *[_dp(a) for a in r], *[_dp(a) for a in s])
             return r, s
         self.L.orc_eval_rhs(self.h, *[_dp(a) for a in r], None, None, None)
         return r
 
     def get_flux(self):
-        f = np.zeros((3, self.nqe, self.n_edge))
+        f = np.zeros((3, self.nqe, self.n_edge), dtype=NP)
         self.L.orc_get_flux(self.h, _dp(f))
         return f
 
     def get_state(self):
         shp = (self.ndof, self.n_elem)
-        ze, qx, qy = np.zeros(shp), np.zeros(shp), np.zeros(shp)
+        ze, qx, qy = np.zeros(shp, dtype=NP), np.zeros(shp, dtype=NP), np.zeros(shp, dtype=NP)
         t = C.c_double()
         self.L.orc_get_state(self.h, C.byref(t), _dp(ze), _dp(qx), _dp(qy))
         return t.value, ze, qx, qy
@@ -344,18 +351,18 @@ class Oracle:
         return wet
 
     def get_geometry(self):
-        area = np.zeros(self.n_elem); jinv = np.zeros((4, self.n_elem)); lfac = np.zeros((3, self.n_elem))
-        enx = np.zeros(self.n_edge); eny = np.zeros(self.n_edge)
+        area = np.zeros(self.n_elem, dtype=NP); jinv = np.zeros((4, self.n_elem), dtype=NP); lfac = np.zeros((3, self.n_elem), dtype=NP)
+        enx = np.zeros(self.n_edge, dtype=NP); eny = np.zeros(self.n_edge, dtype=NP)
         self.L.orc_get_geometry(self.h, _dp(area), _dp(jinv), _dp(lfac), _dp(enx), _dp(eny))
         return area, jinv, lfac, enx, eny
 
     def get_nodal(self):
-        out = [np.zeros(self.n_nodes) for _ in range(3)]
+        out = [np.zeros(self.n_nodes, dtype=NP) for _ in range(3)]
         self.L.orc_get_nodal(self.h, *[_dp(a) for a in out])
         return out
 
     def get_wind(self):
-        tau = np.zeros((2, self.n_nodes))
+        tau = np.zeros((2, self.n_nodes), dtype=NP)
         self.L.orc_get_wind(self.h, _dp(tau))
         return tau
 
