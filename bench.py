@@ -29,7 +29,7 @@ if str(ROOT) not in sys.path:
 
 import numpy as np  # noqa: E402
 
-METRIC = "fp64 DOF-updates/sec per RK stage"
+METRIC = "fp64 DOF-updates/sec per RK stage"          # BASELINE.json metric; with --dtype f32 the line says fp32
 UNIT = "DOF-updates/s"
 
 
@@ -58,57 +58,58 @@ def make_workload(name: str, scale: float = 1.0):
 # algorithmic bytes: what the two-kernel design must move per launch, every
 # array counted once (unique-read assumption: each element's state is read once by EDGE although
 # three edges use it; each flux value once by the element kernel although two elements use it).
-def alg_bytes(w, kind: str, stage_first: bool, fused: bool = False) -> float:
+def alg_bytes(w, kind: str, stage_first: bool, fused: bool = False, rb: int = 8) -> float:
+    """rb = bytes per value of the working precision (8: fp64, 4: fp32); index tables are int32, masks bytes."""
     ne, nd = w.mesh.n_elem, w.mesh.n_edge
     nn = w.mesh.n_nodes
     ndof, nqe = w.ndof, w.params["p"] + 1
     lim, wd, wind = w.params["limiter"], w.params["wetdry"], w.holland is not None
-    st = 3 * ndof * 8
+    st = 3 * ndof * rb
     if kind == "edge":
-        return nd * (8 + 4 + 16 + 16 + 3 * nqe * 8) + ne * st
+        return nd * (8 + 4 + 2 * rb + 2 * rb + 3 * nqe * rb) + ne * st
     if kind == "elem" and fused:
         # element-centric stage kernel (A1-A5, A7): state once (the neighbours' rows are other elements' own
         # rows: unique-read assumption), neighbour table 12, normals 48, L/A 24, Jacobian 32, vertex bathymetry
         # 24, wet flag 1, new state; no flux buffer, no edge records
-        b = ne * (st + 12 + 48 + 24 + 32 + 24 + 1 + st)
+        b = ne * (st + 12 + 6 * rb + 3 * rb + 4 * rb + 3 * rb + 1 + st)
         if not stage_first:
             b += ne * st
         if wd and not lim:
             b += ne * 1
         if lim:
-            b += ne * 24
+            b += ne * 3 * rb
         if wind:
-            b += ne * 12 + nn * 16
+            b += ne * 12 + nn * 2 * rb
         return b
     if kind == "elem":
-        b = nd * 3 * nqe * 8 + ne * (st + 12 + 24 + 32 + 24 + 1 + st)
+        b = nd * 3 * nqe * rb + ne * (st + 12 + 3 * rb + 4 * rb + 3 * rb + 1 + st)
         if not stage_first:
             b += ne * st
         if wd and not lim:
             b += ne * 1
         if lim:
-            b += ne * 24
+            b += ne * 3 * rb
         if wind:
-            b += ne * 12 + nn * 16
+            b += ne * 12 + nn * 2 * rb
         return b
     if kind == "limwd":
         # what a write-if-changed pass must READ: the state rows the two steps look at (p = 2: not the quadratic momentum
         # modes), neighbour table, the neighbours' means (once per element), vertex bathymetry, wet flag.  What it writes
         # depends on the data (only values a step changed) and is NOT credited: the fraction is a lower bound.
         rows = 9 if w.params["p"] == 1 else 12
-        return ne * (rows * 8 + 12 + 24 + 24 + 1)
+        return ne * (rows * rb + 12 + 3 * rb + 3 * rb + 1)
     if kind == "wind":
-        return nn * 32
+        return nn * 4 * rb
     raise ValueError(kind)
 
 
-def stage_bytes_total(w, fused: bool = False) -> float:
+def stage_bytes_total(w, fused: bool = False, rb: int = 8) -> float:
     """Algorithmic bytes of one whole time step (all stages)."""
-    tot = alg_bytes(w, "wind", True) if w.holland is not None else 0.0
+    tot = alg_bytes(w, "wind", True, rb=rb) if w.holland is not None else 0.0
     for s in range(w.n_stage):
-        tot += (0.0 if fused else alg_bytes(w, "edge", s == 0)) + alg_bytes(w, "elem", s == 0, fused)
+        tot += (0.0 if fused else alg_bytes(w, "edge", s == 0, rb=rb)) + alg_bytes(w, "elem", s == 0, fused, rb=rb)
         if w.params["limiter"]:
-            tot += alg_bytes(w, "limwd", s == 0)
+            tot += alg_bytes(w, "limwd", s == 0, rb=rb)
     return tot
 
 
@@ -208,7 +209,10 @@ def run_reference(args, rank: int):
     """The CPU oracle, as it stands, on the host cores (bench contract: reference arm)."""
     if rank != 0:
         return
-    from oracle import oracle as orc
+    if args.dtype == "f32":
+        from oracle import oracle32 as orc
+    else:
+        from oracle import oracle as orc
     orc.build()
     total = args.steps + args.warmup
     # bounded sample: the full mesh if the run stays within a few minutes, else a smaller mesh of the same recipe
@@ -222,9 +226,9 @@ def run_reference(args, rank: int):
     dt = time.perf_counter() - t0
     value = w.dofs * w.n_stage * args.steps / dt
     sample = f"{w.name}: {w.mesh.n_elem} elements, {args.steps} steps after {args.warmup} warm-up"
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+    line = {"impl": "reference", "metric": METRIC.replace("fp64", "fp32") if args.dtype == "f32" else METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
             "config": {"workload": w.name, "n_elem": w.mesh.n_elem, "p": w.params["p"], "rk_order": w.params["rk_order"],
                        "dt": w.dt, "kind": "CPU oracle (oracle/dgswem_oracle.c, gcc -O2 -ffp-contract=off, OpenMP)"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
@@ -299,7 +303,10 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     import paper_2508_21208_b200 as pk
     torch.cuda.set_device(local_rank)
     w = make_workload(args.workload)
-    g = pk.Dgswem.from_workload(w, reorder=args.reorder, device=local_rank)
+    f32 = args.dtype == "f32"
+    rb = 4 if f32 else 8
+    metric = METRIC.replace("fp64", "fp32") if f32 else METRIC
+    g = pk.Dgswem.from_workload(w, reorder=args.reorder, device=local_rank, precision=32 if f32 else 64)
     dofs_stage = w.dofs * w.n_stage
     fused = g.stage_form() == 1
 
@@ -357,7 +364,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     e2e_s = max_over_ranks(e2e_s, world, "cuda")
-    state_bytes = 3 * w.ndof * w.mesh.n_elem * 8
+    state_bytes = 3 * w.ndof * w.mesh.n_elem * 8          # the ABI's host arrays are binary64 in both precisions
     e2e = {"value": whole_job_value(world, dofs_stage, args.steps, e2e_s), "unit": UNIT,
            "h2d_bytes_per_step": state_bytes / args.steps, "d2h_bytes_per_step": (state_bytes + w.mesh.n_elem) / args.steps,
            "call": f"dgswem_set_state + dgswem_step({args.steps}) + dgswem_get_state + dgswem_get_wetdry, pinned host buffers, "
@@ -371,7 +378,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     for k, (tms, cnt) in prof.items():
         if cnt:
             nfirst = cnt // w.n_stage if k in ("edge", "elem", "limwd") else cnt
-            byts = (alg_bytes(w, k, True, fused) * nfirst + alg_bytes(w, k, False, fused) * (cnt - nfirst)) / cnt
+            byts = (alg_bytes(w, k, True, fused, rb) * nfirst + alg_bytes(w, k, False, fused, rb) * (cnt - nfirst)) / cnt
             per_kind[k] = {"launches": cnt, "avg_ms": tms / cnt, "alg_bytes_per_launch": byts,
                            "achieved_gbs": byts / (tms / cnt * 1e-3) / 1e9, "share_of_step": tms / ms_prof}
     dom = max(per_kind, key=lambda k: per_kind[k]["avg_ms"] * per_kind[k]["launches"])
@@ -385,13 +392,13 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             if len(f) >= 3 and f[0] == args.workload and f[1] == ("stage" if (fused and dom == "elem") else dom):
                 traffic = float(f[2])
     kname = "k_stage" if (fused and dom == "elem") else f"k_{dom}"
-    sb = stage_bytes_total(w, fused)
+    sb = stage_bytes_total(w, fused, rb)
     # SURVEY.md section 8(d)'s figure for the flux-buffer design (591 B per element-stage at p = 1), for reference
-    sb_survey = stage_bytes_total(w, False)
+    sb_survey = stage_bytes_total(w, False, rb)
     roofline = {"bound": "hbm", "kernel": f"{kname}<{w.params['p']}>", "achieved": d["achieved_gbs"], "peak": peak, "unit": "GB/s",
                 "frac": d["achieved_gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
                 "alg_bytes_per_launch": d["alg_bytes_per_launch"], "avg_launch_ms": d["avg_ms"], "kernels": per_kind,
-                "fp64_roof": fp64_roof(w, fused, dom, d["avg_ms"], dfma_rate),
+                "fp64_roof": None if f32 else fp64_roof(w, fused, dom, d["avg_ms"], dfma_rate),
                 "whole_step": {"alg_bytes": sb, "achieved_gbs": sb / (ms / args.steps * 1e-3) / 1e9,
                                "frac_of_measured_peak": sb / (ms / args.steps * 1e-3) / 1e9 / peak,
                                "frac_of_8TBs_nominal": sb / (ms / args.steps * 1e-3) / 1e9 / 8000.0,
@@ -401,7 +408,10 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     # ---- CPU baseline: the oracle on a bounded sample of the same workload, on this box's cores
     cpu = None
     if not args.no_cpu:
-        from oracle import oracle as orc
+        if f32:
+            from oracle import oracle32 as orc
+        else:
+            from oracle import oracle as orc
         orc.build()
         o = orc.Oracle.from_workload(w)
         nsamp = max(1, min(args.steps, int(round(12.0 / (w.mesh.n_elem * w.n_stage * 0.28e-6 + 1e-3)))))
@@ -412,8 +422,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         cpu = {"value": dofs_stage * nsamp / cs, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
                "sample": f"{nsamp} steps of {w.name} (full mesh, {w.mesh.n_elem} elements) after 1 warm-up step, {cs:.1f} s"}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": ms / args.steps, "ms_per_step_with_per_launch_events": ms_prof / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+    line = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms / args.steps, "ms_per_step_with_per_launch_events": ms_prof / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
             "data": "synthetic",
             "config": {"workload": w.name, "n_elem": w.mesh.n_elem, "n_edge": w.mesh.n_edge, "n_nodes": w.mesh.n_nodes,
                        "p": w.params["p"], "rk_order": w.params["rk_order"], "dt": w.dt, "limiter": w.params["limiter"],
@@ -435,6 +445,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C3")
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"], help="working precision of the path (f32: SURVEY 8(f) NEXT-2, "
+                    "the paper's own precision; the driver's default line stays C3 / f64)")
     ap.add_argument("--reorder", type=int, default=1)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--decomp", type=int, default=0, help="domain decomposition instead of replicas: one partition per rank "

@@ -1,6 +1,6 @@
 /* dgswem.h -- C ABI of the B200-native DG-SWEM hot path (arxiv 2508.21208).
  *
- * The library evaluates, on ONE sm_100a GPU in fp64, the per-RK-stage discontinuous Galerkin
+ * The library evaluates, on ONE sm_100a GPU in fp64 (or, on request, fp32), the per-RK-stage discontinuous Galerkin
  * right-hand side of the 2-D shallow water equations on an unstructured triangular mesh
  * (eqs (1)-(5); kernels EDGE / GATHER / AREA = PAPER.md Alg. 2 / 3 / 1) and the
  * SSP Runge-Kutta stage update followed by slope limiting and wetting/drying.
@@ -50,6 +50,10 @@ typedef struct {
   int32_t reorder;      /* 0: keep caller's numbering internally; 1: Hilbert-curve renumbering   */
   int32_t device;       /* CUDA device ordinal                                                   */
   int32_t flux;         /* numerical flux: 0 local Lax-Friedrichs (R-3), 1 Roe (R-17)      */
+  int32_t precision;    /* working precision of state, tables and kernels: 64 (or 0; default, the BASELINE
+                           metric) or 32 (the paper's own runs, PAPER.md:158 "-r4", :529).
+                           Every pointer of this ABI stays binary64: values are rounded on the way in and are
+                           exact on the way out; time, time step, tide and storm track stay binary64 inside */
 } dgswem_params;
 
 /* Holland (1980) vortex, R-9: centre (x0+vx t, y0+vy t), radius of max wind rmax [m],
@@ -157,6 +161,9 @@ int dgswem_fp64_peak(dgswem_t*, double* dfma_per_s);
  * buffer, 1 = element-centric stage kernel without it (default for p = 1; DGSWEM_FUSED=0/1 in the environment of
  * dgswem_create overrides).  Both give the same bits. */
 int dgswem_stage_form(const dgswem_t*);
+
+/* Working precision of the handle: 64 or 32 (dgswem_params.precision). */
+int dgswem_precision(const dgswem_t*);
 
 /* Number of kernels launched by this handle so far (for bench.py's gpu_launches). */
 int64_t dgswem_launch_count(const dgswem_t*);

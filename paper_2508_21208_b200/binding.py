@@ -20,7 +20,7 @@ E_NONFINITE = -4
 class Params(C.Structure):
     _fields_ = [("p", C.c_int32), ("rk_order", C.c_int32), ("g", C.c_double), ("cf", C.c_double),
                 ("coriolis_f", C.c_double), ("h0_dry", C.c_double), ("limiter", C.c_int32), ("wetdry", C.c_int32),
-                ("reorder", C.c_int32), ("device", C.c_int32), ("flux", C.c_int32)]
+                ("reorder", C.c_int32), ("device", C.c_int32), ("flux", C.c_int32), ("precision", C.c_int32)]
 
 
 class Holland(C.Structure):
@@ -44,7 +44,7 @@ class DgswemError(RuntimeError):
 EXPORTS = ["dgswem_create", "dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_set_wind_forcing", "dgswem_set_rain", "dgswem_get_pressure", "dgswem_step",
            "dgswem_eval_rhs", "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_nodal", "dgswem_get_wind",
            "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_limit", "dgswem_end_step", "dgswem_set_halo",
-           "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_fp64_peak", "dgswem_stage_form", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
+           "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_fp64_peak", "dgswem_stage_form", "dgswem_precision", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
 
 _lib = None
 
@@ -86,6 +86,7 @@ def load_library():
     L.dgswem_halo_unpack.argtypes = [VP, C.c_int, C.c_void_p, C.c_int]
     L.dgswem_fp64_peak.argtypes = [VP, PD]; L.dgswem_fp64_peak.restype = C.c_int
     L.dgswem_stage_form.argtypes = [VP]; L.dgswem_stage_form.restype = C.c_int
+    L.dgswem_precision.argtypes = [VP]; L.dgswem_precision.restype = C.c_int
     L.dgswem_launch_count.argtypes = [VP]; L.dgswem_launch_count.restype = I64
     L.dgswem_profile.argtypes = [VP, C.c_int]; L.dgswem_profile.restype = C.c_int
     L.dgswem_profile_read.argtypes = [VP, PD, C.POINTER(I64)]; L.dgswem_profile_read.restype = C.c_int
@@ -110,7 +111,7 @@ class Dgswem:
     """One model on one GPU.  Method names mirror the C ABI (dgswem_<name>)."""
 
     def __init__(self, params: dict, xy, bathy, tri, edge_elem, edge_local, edge_bc, elem_edge, *,
-                 reorder: int = 1, device: int = 0, use_torch_alloc: bool = True):
+                 reorder: int = 1, device: int = 0, use_torch_alloc: bool = True, precision: int = 64):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2508_21208_b200 needs a CUDA device (there is no CPU fallback)")
@@ -133,7 +134,8 @@ class Dgswem:
         assert edge_bc.shape == (self.n_edge,) and elem_edge.shape == (self.n_elem, 3)
         prm = Params(p=self.p, rk_order=self.n_stage, g=params["g"], cf=params["cf"], coriolis_f=params["coriolis_f"],
                      h0_dry=params["h0_dry"], limiter=int(params["limiter"]), wetdry=int(params["wetdry"]),
-                     reorder=int(reorder), device=int(device), flux=int(params.get("flux", 0)))
+                     reorder=int(reorder), device=int(device), flux=int(params.get("flux", 0)),
+                     precision=int(precision))
         self.device = torch.device("cuda", device)
         self._tensors = {}
         self.stream = None
@@ -300,6 +302,10 @@ class Dgswem:
         out = C.c_double()
         self._check(self.L.dgswem_fp64_peak(self.h, C.byref(out)))
         return out.value
+
+    def precision(self) -> int:
+        """Working precision of the handle: 64 or 32."""
+        return int(self.L.dgswem_precision(self.h))
 
     def stage_form(self) -> int:
         """0: edge kernel + element kernel (flux buffer); 1: element-centric stage kernel."""

@@ -1,7 +1,8 @@
 """Build paper_2508_21208_b200/libdgswem.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-Flags that matter: -fmad=false and host -ffp-contract=off (no FMA contraction,
-so results agree with the oracle bit for bit), -lineinfo (ncu source page)."""
+Flags that matter: -fmad=false and host -ffp-contract=off (the compilers contract nothing by
+themselves -- fused multiply-adds are the explicit fma() calls of the canonical arithmetic -- so results are reproducible bit
+for bit against the specification), -lineinfo (ncu source page).  csrc/dgswem.cu compiles kernels and host code twice (fp64, fp32)."""
 from __future__ import annotations
 
 import os
@@ -12,7 +13,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 SRC = PKG / "csrc" / "dgswem.cu"
-DEPS = [SRC, PKG / "csrc" / "dgswem_kernels.cuh", ROOT / "include" / "dgswem.h"]
+DEPS = [SRC, PKG / "csrc" / "dgswem_kernels.cuh", PKG / "csrc" / "dgswem_impl.inl", ROOT / "include" / "dgswem.h"]
 LIB = PKG / "libdgswem.so"
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false",

@@ -1,8 +1,10 @@
-// dgswem.cu -- host side of the C ABI (include/dgswem.h): handle, validation, element-independent
-// tables, geometry, Hilbert renumbering, device layout and the per-step launch sequence.
+// dgswem.cu -- the C ABI of include/dgswem.h.  The implementation (handle, validation, element-independent tables,
+// geometry, Hilbert renumbering, device layout, per-step launch sequence: dgswem_impl.inl) and the kernels
+// (dgswem_kernels.cuh) are compiled twice, in binary64 (namespaces imp64 / dgk64; the default, the BASELINE metric) and in
+// binary32 (imp32 / dgk32, the paper's own precision).  dgswem_params.precision
+// picks one at dgswem_create; every other entry point dispatches on the handle.  The ABI itself is binary64 in both.
 // No torch types here; device memory comes from the hooks (or cudaMalloc), work goes to one stream.
 #include "dgswem.h"
-#include "dgswem_kernels.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -14,1246 +16,95 @@
 #include <string>
 #include <vector>
 
-using namespace dgk;
+#include <cuda_runtime.h>
 
-namespace {
-
-thread_local std::string g_create_error;
-
-constexpr double kG_edge1 = 0.57735026918962576;   // 1/sqrt(3)
-constexpr double kG_edge2 = 0.77459666924148338;   // sqrt(3/5)
-
-inline long long round_up(long long n, long long m) { return (n + m - 1) / m * m; }
-
-// ------------------------------------------------------------------------------------ tables
-// Dubiner basis (eq. (4)), mode order 00,01,10,02,11,20, from barycentrics.
-void dubiner(double l1, double l2, double* phi, double* g1, double* g2) {
-  const double xi1 = 2.0 * l1 - 1.0;
-  const double xi2 = 2.0 * l2 - 1.0;
-  const double s = 0.5 * (1.0 - xi2);
-  const double r = 0.5 * (5.0 * xi2 + 3.0);
-  phi[0] = 1.0;
-  phi[1] = 0.5 * (3.0 * xi2 + 1.0);
-  phi[2] = xi1 + 0.5 * (1.0 + xi2);
-  phi[3] = 0.5 * (((5.0 * xi2) * xi2 + 2.0 * xi2) - 1.0);
-  phi[4] = phi[2] * r;
-  phi[5] = 0.5 * ((3.0 * phi[2]) * phi[2] - s * s);
-  g1[0] = 0.0;           g2[0] = 0.0;
-  g1[1] = 0.0;           g2[1] = 1.5;
-  g1[2] = 1.0;           g2[2] = 0.5;
-  g1[3] = 0.0;           g2[3] = 5.0 * xi2 + 1.0;
-  g1[4] = r;             g2[4] = 0.5 * r + 2.5 * phi[2];
-  g1[5] = 3.0 * phi[2];  g2[5] = 0.5 * (3.0 * phi[2] + s);
-}
-
-void make_tables(int p, Tables& T) {
-  std::memset(&T, 0, sizeof(T));
-  const int ndof = (p + 1) * (p + 2) / 2, nqe = p + 1, nqa = (p == 1) ? 3 : 6;
-  double ge[3] = {0, 0, 0}, we[3] = {0, 0, 0}, wa[6] = {0, 0, 0, 0, 0, 0};
-  if (p == 1) {
-    ge[0] = -kG_edge1; ge[1] = kG_edge1; we[0] = 1.0; we[1] = 1.0;
-    for (int i = 0; i < 3; ++i) {
-      for (int v = 0; v < 3; ++v) T.la[i][v] = (v == i) ? 2.0 / 3.0 : 1.0 / 6.0;
-      wa[i] = 2.0 / 3.0;
-    }
-  } else {
-    ge[0] = -kG_edge2; ge[1] = 0.0; ge[2] = kG_edge2;
-    we[0] = 5.0 / 9.0; we[1] = 8.0 / 9.0; we[2] = 5.0 / 9.0;
-    const double a1 = 0.445948490915965, w1 = 0.223381589678011;
-    const double a2 = 0.091576213509771, w2 = 0.109951743655322;
-    for (int i = 0; i < 3; ++i) {
-      for (int v = 0; v < 3; ++v) {
-        T.la[i][v] = (v == i) ? 1.0 - 2.0 * a1 : a1;
-        T.la[3 + i][v] = (v == i) ? 1.0 - 2.0 * a2 : a2;
-      }
-      wa[i] = 2.0 * w1;
-      wa[3 + i] = 2.0 * w2;
-    }
-  }
-  const double mass[6] = {2.0, 1.0, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 9.0, 2.0 / 15.0};
-  double invM[6];
-  for (int k = 0; k < 6; ++k) invM[k] = 1.0 / mass[k];
-  double phi[6], g1[6], g2[6];
-  for (int i = 0; i < nqa; ++i) {
-    dubiner(T.la[i][1], T.la[i][2], phi, g1, g2);
-    for (int k = 0; k < ndof; ++k) {
-      T.phiA[i][k] = phi[k]; T.dA1[i][k] = g1[k]; T.dA2[i][k] = g2[k];
-      T.wfac[i][k] = wa[i] * invM[k];
-      T.srfac[i][k] = T.wfac[i][k] * phi[k];
-    }
-  }
-  for (int j = 0; j < nqe; ++j) {
-    T.elam[j][0] = 0.5 * (1.0 - ge[j]);
-    T.elam[j][1] = 0.5 * (1.0 + ge[j]);
-  }
-  for (int l = 0; l < 3; ++l) {
-    const int va = (l + 1) % 3, vb = (l + 2) % 3;
-    for (int j = 0; j < nqe; ++j) {
-      double lam[3] = {0.0, 0.0, 0.0};
-      lam[va] = T.elam[j][0]; lam[vb] = T.elam[j][1];
-      dubiner(lam[1], lam[2], phi, g1, g2);
-      for (int k = 0; k < ndof; ++k) {
-        T.phiE[l][j][k] = phi[k];
-        T.efac[l][j][k] = (we[j] * invM[k]) * phi[k];
-      }
-    }
-  }
-  for (int v = 0; v < 3; ++v) {
-    double lam[3] = {0.0, 0.0, 0.0};
-    lam[v] = 1.0;
-    dubiner(lam[1], lam[2], phi, g1, g2);
-    for (int k = 0; k < ndof; ++k) T.phiV[v][k] = phi[k];
-  }
-}
-
-// ------------------------------------------------------------------------------------ Hilbert
-// index of (x, y) in [0, 2^16)^2 along the Hilbert curve
-inline uint32_t hilbert_d(uint32_t x, uint32_t y) {
-  const uint32_t n = 1u << 16;
-  uint32_t d = 0;
-  for (uint32_t s = n >> 1; s > 0; s >>= 1) {
-    const uint32_t rx = (x & s) ? 1u : 0u, ry = (y & s) ? 1u : 0u;
-    d += s * s * ((3u * rx) ^ ry);
-    if (ry == 0) {   // rotate / flip the quadrant
-      if (rx == 1) { x = (n - 1u) - x; y = (n - 1u) - y; }
-      const uint32_t t = x; x = y; y = t;
-    }
-  }
-  return d;
-}
-
-std::vector<int> hilbert_order(const std::vector<double>& px, const std::vector<double>& py) {
-  const size_t n = px.size();
-  double x0 = 1e300, x1 = -1e300, y0 = 1e300, y1 = -1e300;
-  for (size_t i = 0; i < n; ++i) {
-    x0 = std::min(x0, px[i]); x1 = std::max(x1, px[i]);
-    y0 = std::min(y0, py[i]); y1 = std::max(y1, py[i]);
-  }
-  const double span = std::max(std::max(x1 - x0, y1 - y0), 1e-300);
-  std::vector<uint64_t> key(n);
-  for (size_t i = 0; i < n; ++i) {
-    const uint32_t ix = (uint32_t)std::min(65535.0, (px[i] - x0) / span * 65535.0);
-    const uint32_t iy = (uint32_t)std::min(65535.0, (py[i] - y0) / span * 65535.0);
-    key[i] = ((uint64_t)hilbert_d(ix, iy) << 32) | (uint64_t)i;
-  }
-  std::sort(key.begin(), key.end());
-  std::vector<int> order(n);
-  for (size_t i = 0; i < n; ++i) order[i] = (int)(key[i] & 0xffffffffu);
-  return order;   // order[new] = old
-}
-
-}  // namespace
-
-// ------------------------------------------------------------------------------------ handle
+// what both precisions' handles share (the opaque dgswem_t of the ABI)
 struct dgswem {
-  dgswem_params prm{};
-  int ndof = 0, nqe = 0, nqa = 0, nstage = 0;
-  long long nn = 0, ne = 0, nd = 0, ld = 0, ldd = 0, ldn = 0;
-  cudaStream_t stream = nullptr;
-  bool own_stream = false;
-  dgswem_devhooks hooks{};
-  bool have_hooks = false;
-  std::vector<void*> allocs;
+  int precision = 64;
   std::string err;
-  long long launches = 0;
-  int res_edge[2] = {0, 0};   // resident grid of the persistent edge kernel [p-1]
-  int res_limwd = 0;          // same for the limiter kernel of this handle's p
-
-  // optional per-kernel timing (dgswem_profile): CUDA events recorded on the stream around every launch
-  struct ProfRec { int kind; cudaEvent_t a, b; };
-  bool profiling = false;
-  std::vector<ProfRec> prof;
-  cudaEvent_t prof_start = nullptr;
-
-  // device
-  double* W[3] = {nullptr, nullptr, nullptr};
-  double* nmm = nullptr;   // [6][ldn] node extrema of the means (vertex-neighbourhood limiter)
-  double *flux = nullptr, *mean = nullptr, *jinv = nullptr, *lfac = nullptr, *hv = nullptr;
-  double *en = nullptr, *ehb = nullptr, *tau = nullptr, *etap = nullptr, *nxy = nullptr, *stage_buf = nullptr;
-  int2* edge_elem = nullptr;
-  int *einfo = nullptr, *elem_edge = nullptr, *nbr = nullptr, *tri = nullptr, *nbinfo = nullptr;
-  double* enl = nullptr;
-  bool fused = false;         // element-centric stage kernel (k_stage) instead of k_edge + k_elem
-  int *node_ptr = nullptr, *node_ev = nullptr;   // node -> (internal element * 4 + vertex), ascending caller element id
-  int *perm_e = nullptr, *inv_e = nullptr, *inv_d = nullptr;   // perm_e[new]=old, inv_e[old]=new, inv_d[old]=new
-  unsigned char *wet = nullptr, *wet_stage = nullptr;
-  int* nf_flag = nullptr;
-  size_t stage_bytes = 0;
-
-  // CUDA-graph replay of whole time steps (dgswem_step): per-call scalar table + device step counter
-  bool graphs_on = true;      // DGSWEM_GRAPH=0 switches to plain stream launches
-  bool capturing = false;     // launch helpers pass table references instead of values
-  double* scal_tab = nullptr; // [cap][kScalStride]
-  double* scal_host = nullptr; // pinned staging copy of the table (so that dgswem_step stays asynchronous)
-  cudaEvent_t scal_ev = nullptr;   // recorded after the table's upload: the staging copy may be rewritten after it
-  long long scal_cap = 0;
-  int* step_ctr = nullptr;
-  struct StepGraph { cudaGraphExec_t exec = nullptr; int steps = 0; long long launches = 0; };
-  StepGraph graph_many, graph_one;
-  double graph_dt = 0.0; bool graph_wind = false; bool graph_tide = false;
-
-  // stage-granular stepping and halo lists (dgswem_begin_step ... dgswem_halo_unpack)
-  double step_dt = 0.0;        // dt of the step in progress (0: none)
-  double* last_out = nullptr;  // stage buffer written by the last dgswem_stage_rhs (W[0] between steps)
-  int *halo_send = nullptr, *halo_recv = nullptr;   // internal element ids
-  long long n_send = 0, n_recv = 0;
-  double* halo_buf = nullptr;  // device staging for host-side pack/unpack, [rows][max(n_send, n_recv)]
-
-  double t = 0.0;
-  double tide_amp = 0.0, tide_omega = 0.0, tide_phase = 0.0;
-  bool wind_on = false;
-  bool stress_on = true, press_on = false;   // parts of the Holland forcing in the momentum source (R-9, R-15)
-  double rain = 0.0;                         // uniform mass source (R-16)
-  dgswem_holland hol{};
-
-  int fail(int code, const char* fmt, ...) {
-    char buf[512];
-    va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof(buf), fmt, ap); va_end(ap);
-    err = buf;
-    return code;
-  }
-  int cuda_fail(cudaError_t e, const char* what) { return fail(DGSWEM_E_CUDA, "%s: %s", what, cudaGetErrorString(e)); }
-
-  void* dalloc(size_t bytes) {
-    void* p = nullptr;
-    if (bytes == 0) bytes = 256;
-    if (have_hooks) {
-      p = hooks.alloc(bytes, hooks.user);
-    } else if (cudaMalloc(&p, bytes) != cudaSuccess) {
-      p = nullptr;
-    }
-    if (p) allocs.push_back(p);
-    return p;
-  }
-  void release_all() {
-    for (void* p : allocs) {
-      if (have_hooks) hooks.free(p, hooks.user); else cudaFree(p);
-    }
-    allocs.clear();
-  }
+  virtual ~dgswem() {}
 };
 
-#define CK(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return h->cuda_fail(e__, #call); } while (0)
-#define CKL(name) do { cudaError_t e__ = cudaGetLastError(); if (e__ != cudaSuccess) return h->cuda_fail(e__, name); h->launches++; } while (0)
-
-enum ProfKind { PK_WIND = 0, PK_EDGE = 1, PK_ELEM = 2, PK_LIMWD = 3, PK_COUNT = 4 };
-constexpr size_t kMaxProfRecords = 1 << 15;
-static inline void prof_begin(dgswem* h, int kind) {
-  if (!h->profiling || h->prof.size() >= kMaxProfRecords) return;
-  dgswem::ProfRec r; r.kind = kind; r.a = nullptr; r.b = nullptr;
-  if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) return;
-  cudaEventRecord(r.a, h->stream);
-  h->prof.push_back(r);
-  h->prof_start = r.a;
-}
-static inline void prof_end(dgswem* h) {
-  if (!h->profiling || h->prof_start == nullptr) return;
-  cudaEventRecord(h->prof.back().b, h->stream);
-  h->prof_start = nullptr;
-}
-
 namespace {
-
-template <typename T>
-int upload(dgswem* h, T*& dptr, const std::vector<T>& host) {
-  dptr = (T*)h->dalloc(host.size() * sizeof(T));
-  if (!dptr) return h->fail(DGSWEM_E_CUDA, "device allocation of %zu bytes failed", host.size() * sizeof(T));
-  CK(cudaMemcpyAsync(dptr, host.data(), host.size() * sizeof(T), cudaMemcpyHostToDevice, h->stream));
-  CK(cudaStreamSynchronize(h->stream));   // host vector may die after return
-  return 0;
+thread_local std::string g_create_error;
 }
 
-inline int grid_for(long long n, int block) { return (int)((n + block - 1) / block); }
+#define DGK_NS dgk64
+#define DGK_REAL double
+#define DGK_F32 0
+#define DGK_IMPL_NS imp64
+#include "dgswem_kernels.cuh"
+#include "dgswem_impl.inl"
+#undef DGK_NS
+#undef DGK_REAL
+#undef DGK_F32
+#undef DGK_IMPL_NS
 
-int validate_mesh(dgswem* h, long long nn, const double* xy, long long ne, const int32_t* tri, long long nd,
-                  const int32_t* edge_elem, const int8_t* edge_local, const int32_t* edge_bc, const int32_t* elem_edge) {
-  for (long long e = 0; e < ne; ++e) {
-    for (int v = 0; v < 3; ++v)
-      if (tri[3 * e + v] < 0 || tri[3 * e + v] >= nn) return h->fail(DGSWEM_E_MESH, "element %lld: node id out of range", e);
-    const double* a = xy + 2 * (long long)tri[3 * e], *b = xy + 2 * (long long)tri[3 * e + 1], *c = xy + 2 * (long long)tri[3 * e + 2];
-    const double A2 = (b[0] - a[0]) * (c[1] - a[1]) - (c[0] - a[0]) * (b[1] - a[1]);
-    if (!(A2 > 0.0)) return h->fail(DGSWEM_E_MESH, "element %lld is not counter-clockwise (or degenerate)", e);
-    for (int l = 0; l < 3; ++l) {
-      const long long d = elem_edge[3 * e + l];
-      if (d < 0 || d >= nd) return h->fail(DGSWEM_E_MESH, "elem_edge[%lld][%d] out of range", e, l);
-      const bool plus = edge_elem[2 * d] == e && edge_local[2 * d] == l;
-      const bool minus = edge_elem[2 * d + 1] == e && edge_local[2 * d + 1] == l;
-      if (plus == minus) return h->fail(DGSWEM_E_MESH, "elem_edge[%lld][%d]=%lld does not point back to the element", e, l, d);
-    }
-  }
-  for (long long d = 0; d < nd; ++d) {
-    const long long ep = edge_elem[2 * d], em = edge_elem[2 * d + 1];
-    const int lp = edge_local[2 * d], lm = edge_local[2 * d + 1];
-    const int bc = edge_bc[d];
-    if (ep < 0 || ep >= ne || lp < 0 || lp > 2) return h->fail(DGSWEM_E_MESH, "edge %lld: bad e+ / local edge", d);
-    if (elem_edge[3 * ep + lp] != d) return h->fail(DGSWEM_E_MESH, "edge %lld: e+ does not list it", d);
-    if (em >= 0) {
-      if (em >= ne || lm < 0 || lm > 2 || em == ep) return h->fail(DGSWEM_E_MESH, "edge %lld: bad e- / local edge", d);
-      if (elem_edge[3 * em + lm] != d) return h->fail(DGSWEM_E_MESH, "edge %lld: e- does not list it", d);
-      if (bc != 0) return h->fail(DGSWEM_E_MESH, "edge %lld: interior edge with boundary code %d", d, bc);
-      // the two sides must share the same two nodes, traversed in opposite directions
-      const int a1 = tri[3 * ep + (lp + 1) % 3], b1 = tri[3 * ep + (lp + 2) % 3];
-      const int a2 = tri[3 * em + (lm + 1) % 3], b2 = tri[3 * em + (lm + 2) % 3];
-      if (a1 != b2 || b1 != a2) return h->fail(DGSWEM_E_MESH, "edge %lld: the two sides do not share the same nodes", d);
-    } else {
-      if (bc != 1 && bc != 2) return h->fail(DGSWEM_E_MESH, "edge %lld: boundary edge needs code 1 or 2, got %d", d, bc);
-    }
-  }
-  return 0;
-}
+#define DGK_NS dgk32
+#define DGK_REAL float
+#define DGK_F32 1
+#define DGK_IMPL_NS imp32
+#include "dgswem_kernels.cuh"
+#include "dgswem_impl.inl"
+#undef DGK_NS
+#undef DGK_REAL
+#undef DGK_F32
+#undef DGK_IMPL_NS
 
-// resident grid of a persistent kernel: CTAs per SM (occupancy API) x SM count
-template <typename K>
-int resident_ctas(K kernel, int threads, size_t smem, int device) {
-  int per_sm = 0, sms = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess) return 0;
-  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return 0;
-  return per_sm * sms;
-}
+// call the implementation of the handle's precision
+#define DISPATCH(h, fn, ...) \
+  ((h)->precision == 32 ? imp32::fn(static_cast<imp32::Handle*>(h), ##__VA_ARGS__) : imp64::fn(static_cast<imp64::Handle*>(h), ##__VA_ARGS__))
+#define DISPATCH_C(h, fn, ...)                                                           \
+  ((h)->precision == 32 ? imp32::fn(static_cast<const imp32::Handle*>(h), ##__VA_ARGS__) \
+                        : imp64::fn(static_cast<const imp64::Handle*>(h), ##__VA_ARGS__))
 
-// a scalar argument: by value on a stream launch, by table reference while a step graph is being captured
-inline ScalRef scal(const dgswem* h, int idx, double val) {
-  ScalRef r;
-  r.tab = h->capturing ? h->scal_tab : nullptr; r.ctr = h->capturing ? h->step_ctr : nullptr; r.idx = idx; r.val = val;
-  return r;
-}
-
-template <int P>
-int launch_edge(dgswem* h, const double* w, ScalRef zeta_b) {
-  EdgeArgs a;
-  a.w = w; a.edge_elem = h->edge_elem; a.einfo = h->einfo; a.en = h->en; a.ehb = h->ehb; a.flux = h->flux;
-  a.nd = (int)h->nd; a.ld = h->ld; a.ldd = h->ldd;
-  a.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
-  a.zeta = zeta_b;
-  const int ntiles = grid_for(h->nd, DGK_EDGE_THREADS);
-  const int resident = h->res_edge[P - 1];
-  prof_begin(h, PK_EDGE);
-  const bool pipe = DGK_PIPE_EDGE && resident > 0 && ntiles > resident;
-  if (h->prm.flux == 1) {
-    if (pipe) k_edge_pipe<P, 1><<<resident, DGK_EDGE_THREADS, 0, h->stream>>>(a, ntiles);
-    else k_edge<P, 1><<<ntiles, DGK_EDGE_THREADS, 0, h->stream>>>(a);
-  } else {
-    if (pipe) k_edge_pipe<P, 0><<<resident, DGK_EDGE_THREADS, 0, h->stream>>>(a, ntiles);
-    else k_edge<P, 0><<<ntiles, DGK_EDGE_THREADS, 0, h->stream>>>(a);
-  }
-  prof_end(h);
-  CKL("k_edge");
-  return 0;
-}
-
-// compile-time specialisation of the element / stage kernels: bit 0 first RK stage, bit 1 Holland forcing, bit 2 its
-// pressure gradient; -1 (flags read from the arguments) when a rarely used option is on (rain)
-inline int stage_variant(const dgswem* h, int first) {
-  if (h->rain != 0.0) return -1;
-  return (first ? 1 : 0) | (h->wind_on ? 2 : 0) | ((h->wind_on && h->press_on) ? 4 : 0);
-}
-
-template <int P, int MODE>
-int launch_elem(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b,
-                int first, bool fuse_wd, bool write_mean) {
-  ElemArgs A;
-  A.win = win; A.w0 = w0; A.wout = wout; A.flux = h->flux; A.elem_edge = h->elem_edge; A.jinv = h->jinv;
-  A.lfac = h->lfac; A.hv = h->hv; A.tri = h->tri; A.tau = h->tau; A.wet = h->wet;
-  A.etap = h->etap; A.stress = h->stress_on ? 1 : 0; A.press = h->press_on ? 1 : 0; A.rain = h->rain;
-  A.nbinfo = nullptr; A.enl = nullptr; A.zeta = scal(h, 0, 0.0);
-  A.mean = write_mean ? h->mean : nullptr;
-  A.ne = (int)h->ne; A.ld = h->ld; A.ldd = h->ldd; A.ldn = h->ldn;
-  A.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
-  A.dt = dt; A.a = a; A.b = b; A.first_stage = first; A.wind = h->wind_on ? 1 : 0; A.fuse_wetdry = fuse_wd ? 1 : 0;
-  // (a persistent form with next-tile index prefetch, as for the edge kernel, was measured slower: it needs
-  // more registers than the 128 the 4-CTA budget leaves, and the spills cost more than the prefetch saves)
-  prof_begin(h, PK_ELEM);
-  const int grid = grid_for(h->ne, DGK_ELEM_THREADS);
-  if constexpr (MODE == MODE_UPDATE) {
-    switch (stage_variant(h, first)) {   // specialised on (first stage, wind, pressure), as k_stage
-      case 0: k_elem<P, MODE, 0><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
-      case 1: k_elem<P, MODE, 1><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
-      case 2: k_elem<P, MODE, 2><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
-      case 3: k_elem<P, MODE, 3><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
-      case 6: k_elem<P, MODE, 6><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
-      case 7: k_elem<P, MODE, 7><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
-      default: k_elem<P, MODE, -1><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A); break;
-    }
-  } else {
-    k_elem<P, MODE, -1><<<grid, DGK_ELEM_THREADS, 0, h->stream>>>(A);
-  }
-  prof_end(h);
-  CKL("k_elem");
-  return 0;
-}
-
-// A1-A5 (+A7) in one launch (element-centric form, no flux buffer)
-template <int P, int MODE>
-int launch_stage(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b,
-                 int first, bool fuse_wd, bool write_mean, ScalRef zeta_b) {
-  ElemArgs A;
-  A.win = win; A.w0 = w0; A.wout = wout; A.flux = h->flux; A.elem_edge = h->elem_edge; A.jinv = h->jinv;
-  A.lfac = h->lfac; A.hv = h->hv; A.tri = h->tri; A.tau = h->tau; A.wet = h->wet;
-  A.etap = h->etap; A.stress = h->stress_on ? 1 : 0; A.press = h->press_on ? 1 : 0; A.rain = h->rain;
-  A.nbinfo = h->nbinfo; A.enl = h->enl; A.zeta = zeta_b;
-  A.mean = write_mean ? h->mean : nullptr;
-  A.ne = (int)h->ne; A.ld = h->ld; A.ldd = h->ldd; A.ldn = h->ldn;
-  A.ph = Phys{h->prm.g, h->prm.h0_dry, h->prm.cf, h->prm.coriolis_f};
-  A.dt = dt; A.a = a; A.b = b; A.first_stage = first; A.wind = h->wind_on ? 1 : 0; A.fuse_wetdry = fuse_wd ? 1 : 0;
-  // (persistent forms were measured slower on C3: next-tile neighbour-table prefetch 425 us, per-warp cp.async
-  // staging of the next tile's rows in shared memory 445 us, against 374 us)
-  prof_begin(h, PK_ELEM);
-  const int grid = grid_for(h->ne, DGK_STAGE_THREADS);
-  if (h->prm.flux == 1) {   // Roe: the generic-flag kernel only
-    k_stage<P, MODE, -1, 1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A);
-  } else if constexpr (MODE == MODE_UPDATE) {
-    // specialised on (first stage, wind): no w^n registers in stage 1, no wind registers without wind
-    switch (stage_variant(h, first)) {
-      case 0: k_stage<P, MODE, 0><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      case 1: k_stage<P, MODE, 1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      case 2: k_stage<P, MODE, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      case 3: k_stage<P, MODE, 3><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      case 6: k_stage<P, MODE, 6><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      case 7: k_stage<P, MODE, 7><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      default: k_stage<P, MODE, -1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-    }
-  } else {
-    k_stage<P, MODE, -1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A);
-  }
-  prof_end(h);
-  CKL("k_stage");
-  return 0;
-}
-
-template <int P>
-int launch_limwd(dgswem* h, double* w) {
-  LimArgs A;
-  A.w = w; A.mean = h->mean; A.nbr = h->nbr; A.hv = h->hv; A.wet = h->wet; A.ne = (int)h->ne; A.ld = h->ld;
-  A.tri = h->tri; A.nmm = h->nmm; A.ldn = h->ldn;
-  A.h0 = h->prm.h0_dry; A.limiter = h->prm.limiter; A.wetdry = h->prm.wetdry;
-  prof_begin(h, PK_LIMWD);
-  const int ntiles = grid_for(h->ne, 128);
-  const int grid = std::max(1, std::min(ntiles, h->res_limwd > 0 ? h->res_limwd : ntiles));
-  if (h->prm.limiter == 2) {   // vertex neighbourhood: extrema of the means around every node first
-    k_node_minmax<<<grid_for(h->nn, 256), 256, 0, h->stream>>>(h->nmm, h->ldn, h->mean, h->node_ptr, h->node_ev, (int)h->nn);
-    if (cudaGetLastError() == cudaSuccess) h->launches++;
-    k_limwd_tma<P, 2><<<grid, 128, LimTile<P>::kSmem, h->stream>>>(A, ntiles);
-  } else {
-    k_limwd_tma<P, 1><<<grid, 128, LimTile<P>::kSmem, h->stream>>>(A, ntiles);
-  }
-  prof_end(h);
-  CKL("k_limwd");
-  return 0;
-}
-
-int launch_wind(dgswem* h, double t) {
-  WindArgs A;
-  A.nxy = h->nxy; A.tau = h->tau; A.etap = h->etap; A.g = h->prm.g; A.nn = (int)h->nn; A.ldn = h->ldn;
-  A.cx = scal(h, 4, h->hol.x0 + h->hol.vx * t); A.cy = scal(h, 5, h->hol.y0 + h->hol.vy * t);
-  A.rmax = h->hol.rmax; A.dp = h->hol.dp; A.B = h->hol.B; A.rho_air = h->hol.rho_air; A.rho_water = h->hol.rho_water;
-  A.f = h->hol.f;
-  prof_begin(h, PK_WIND);
-  k_wind<<<grid_for(h->nn, 256), 256, 0, h->stream>>>(A);
-  prof_end(h);
-  CKL("k_wind");
-  return 0;
-}
-
-double tide_value(const dgswem* h, double t) {
-  if (h->tide_amp == 0.0) return 0.0;
-  return h->tide_amp * std::sin(h->tide_omega * t + h->tide_phase);
-}
-
-// one RK stage, first part: EDGE -> GATHER+AREA+RK (+wet/dry when no limiter follows)
-template <int P>
-int run_stage_rhs(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b, int first,
-                  double t_stage, int stage) {
-  const bool lim = h->prm.limiter != 0;
-  const bool wd = h->prm.wetdry != 0;
-  int rc;
-  if (h->fused) {
-    rc = launch_stage<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim, scal(h, stage, tide_value(h, t_stage)));
-  } else {
-    rc = launch_edge<P>(h, win, scal(h, stage, tide_value(h, t_stage)));
-    if (rc) return rc;
-    rc = launch_elem<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim);
-  }
-  return rc;
-}
-
-// one RK stage: first part, then the limiter + wet/dry pass over the RK-updated means (limiter on)
-template <int P>
-int run_stage(dgswem* h, const double* win, const double* w0, double* wout, double dt, double a, double b, int first,
-              double t_stage, int stage) {
-  int rc = run_stage_rhs<P>(h, win, w0, wout, dt, a, b, first, t_stage, stage);
-  if (rc) return rc;
-  if (h->prm.limiter != 0) rc = launch_limwd<P>(h, wout);
-  return rc;
-}
-
-// Shu-Osher SSP(2,2) / SSP(3,3) (R-2)
-static const double kA2[2] = {0.0, 0.5}, kB2[2] = {1.0, 0.5}, kC2[2] = {0.0, 1.0};
-static const double kA3[3] = {0.0, 0.75, 1.0 / 3.0}, kB3[3] = {1.0, 0.25, 2.0 / 3.0}, kC3[3] = {0.0, 1.0, 0.5};
-
-// enqueue the kernels of one time step starting at time t (values) or at table row *step_ctr (capturing)
-template <int P>
-int enqueue_step(dgswem* h, double dt, double t) {
-  const bool rk3 = h->prm.rk_order == 3;
-  const double* a = rk3 ? kA3 : kA2; const double* b = rk3 ? kB3 : kB2; const double* c = rk3 ? kC3 : kC2;
-  if (h->wind_on) { int rc = launch_wind(h, t); if (rc) return rc; }
-  // current state lives in W[0]; RK2: W0 -> W1 -> W0 ; RK3: W0 -> W1 -> W2 -> W0
-  int rc = run_stage<P>(h, h->W[0], h->W[0], h->W[1], dt, a[0], b[0], 1, t + c[0] * dt, 0);
-  if (rc) return rc;
-  if (!rk3) {
-    rc = run_stage<P>(h, h->W[1], h->W[0], h->W[0], dt, a[1], b[1], 0, t + c[1] * dt, 1);
-  } else {
-    rc = run_stage<P>(h, h->W[1], h->W[0], h->W[2], dt, a[1], b[1], 0, t + c[1] * dt, 1);
-    if (rc) return rc;
-    rc = run_stage<P>(h, h->W[2], h->W[0], h->W[0], dt, a[2], b[2], 0, t + c[2] * dt, 2);
-  }
-  return rc;
-}
-
-void drop_graphs(dgswem* h) {
-  if (h->graph_many.exec) cudaGraphExecDestroy(h->graph_many.exec);
-  if (h->graph_one.exec) cudaGraphExecDestroy(h->graph_one.exec);
-  h->graph_many = dgswem::StepGraph(); h->graph_one = dgswem::StepGraph();
-}
-
-// capture `steps` consecutive time steps (each followed by k_advance when a scalar table is in use) into one graph
-template <int P>
-int capture_steps(dgswem* h, int steps, double dt, bool need_tab, dgswem::StepGraph& out) {
-  const long long l0 = h->launches;
-  CK(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeRelaxed));
-  h->capturing = need_tab;
-  int rc = 0;
-  for (int i = 0; i < steps && rc == 0; ++i) {
-    rc = enqueue_step<P>(h, dt, 0.0);
-    if (rc == 0 && need_tab) { k_advance<<<1, 1, 0, h->stream>>>(h->step_ctr); if (cudaGetLastError() != cudaSuccess) rc = DGSWEM_E_CUDA; else h->launches++; }
-  }
-  h->capturing = false;
-  cudaGraph_t g = nullptr;
-  const cudaError_t e = cudaStreamEndCapture(h->stream, &g);
-  out.launches = h->launches - l0;
-  h->launches = l0;   // nothing has run yet: replays are counted when they are launched
-  if (rc) { if (g) cudaGraphDestroy(g); return rc; }
-  if (e != cudaSuccess) return h->cuda_fail(e, "cudaStreamEndCapture");
-  const cudaError_t e2 = cudaGraphInstantiate(&out.exec, g, 0);
-  cudaGraphDestroy(g);
-  if (e2 != cudaSuccess) { out.exec = nullptr; return h->cuda_fail(e2, "cudaGraphInstantiate"); }
-  out.steps = steps;
-  return 0;
-}
-
-template <int P>
-int run_steps(dgswem* h, long long nsteps, double dt) {
-  const bool rk3 = h->prm.rk_order == 3;
-  const double* c = rk3 ? kC3 : kC2;
-  if (!h->graphs_on || h->profiling || nsteps == 0) {
-    for (long long n = 0; n < nsteps; ++n) {
-      int rc = enqueue_step<P>(h, dt, h->t);
-      if (rc) return rc;
-      h->t = h->t + dt;
-    }
-    return 0;
-  }
-  // ---- graph replay: the step's kernel sequence is captured once per (dt, forcing on/off) and replayed;
-  // the scalars that change from step to step (tidal elevation per stage, storm centre) are tabulated here
-  // on the host exactly as the stream path computes them, and read by row on the device.
-  const bool tide_on = h->tide_amp != 0.0;
-  const bool need_tab = tide_on || h->wind_on;
-  if (h->graph_one.exec && (h->graph_dt != dt || h->graph_wind != h->wind_on || h->graph_tide != tide_on)) drop_graphs(h);
-  constexpr long long kScalRows = 4096;   // steps per table upload (256 KiB); longer calls go in chunks
-  if (need_tab && !h->scal_tab) {
-    h->scal_tab = (double*)h->dalloc((size_t)kScalRows * kScalStride * sizeof(double));
-    if (!h->scal_tab) return h->fail(DGSWEM_E_CUDA, "device allocation failed");
-    CK(cudaMallocHost((void**)&h->scal_host, (size_t)kScalRows * kScalStride * sizeof(double)));
-    CK(cudaEventCreateWithFlags(&h->scal_ev, cudaEventDisableTiming));
-    h->scal_cap = kScalRows;
-  }
-  const int many = h->ne < 65536 ? 8 : (h->ne < 1000000 ? 2 : 1);
-  if (!h->graph_one.exec) {
-    int rc = capture_steps<P>(h, 1, dt, need_tab, h->graph_one);
-    if (rc) return rc;
-    if (many > 1 && (rc = capture_steps<P>(h, many, dt, need_tab, h->graph_many))) return rc;
-    h->graph_dt = dt; h->graph_wind = h->wind_on; h->graph_tide = tide_on;
-  }
-  long long done = 0;
-  while (done < nsteps) {
-    const long long chunk = need_tab ? std::min(nsteps - done, h->scal_cap) : nsteps - done;
-    if (need_tab) {
-      CK(cudaEventSynchronize(h->scal_ev));   // the previous upload has left the pinned staging copy
-      double t = h->t;
-      for (long long n = 0; n < chunk; ++n) {
-        double* row = h->scal_host + (size_t)n * kScalStride;
-        for (int i = 0; i < kScalStride; ++i) row[i] = 0.0;
-        for (int st = 0; st < h->nstage; ++st) row[st] = tide_value(h, t + c[st] * dt);
-        row[4] = h->hol.x0 + h->hol.vx * t; row[5] = h->hol.y0 + h->hol.vy * t;
-        t = t + dt;
-      }
-      // stream order keeps earlier replays' reads of the device table ahead of this overwrite
-      CK(cudaMemcpyAsync(h->scal_tab, h->scal_host, (size_t)chunk * kScalStride * sizeof(double), cudaMemcpyHostToDevice, h->stream));
-      CK(cudaEventRecord(h->scal_ev, h->stream));
-      CK(cudaMemsetAsync(h->step_ctr, 0, sizeof(int), h->stream));
-    }
-    long long left = chunk;
-    while (left > 0) {
-      dgswem::StepGraph& g = (h->graph_many.exec && left >= h->graph_many.steps) ? h->graph_many : h->graph_one;
-      CK(cudaGraphLaunch(g.exec, h->stream));
-      h->launches += g.launches;
-      left -= g.steps;
-    }
-    for (long long n = 0; n < chunk; ++n) h->t = h->t + dt;
-    done += chunk;
-  }
-  return 0;
-}
-
-}  // namespace
-
-// ------------------------------------------------------------------------------------ C ABI
 extern "C" {
 
 const char* dgswem_last_error(const dgswem_t* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
-void dgswem_destroy(dgswem_t* h) {
-  if (!h) return;
-  cudaSetDevice(h->prm.device);
-  if (h->stream) cudaStreamSynchronize(h->stream);
-  for (auto& r : h->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
-  h->prof.clear();
-  if (h->graph_many.exec) cudaGraphExecDestroy(h->graph_many.exec);
-  if (h->graph_one.exec) cudaGraphExecDestroy(h->graph_one.exec);
-  if (h->scal_ev) cudaEventDestroy(h->scal_ev);
-  if (h->scal_host) cudaFreeHost(h->scal_host);
-  h->release_all();
-  if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
-  delete h;
-}
-
-int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* hooks, int64_t n_nodes,
-                  const double* xy, const double* bathy, int64_t n_elem, const int32_t* tri, int64_t n_edge,
-                  const int32_t* edge_elem, const int8_t* edge_local, const int32_t* edge_bc, const int32_t* elem_edge) {
+int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* hooks, int64_t n_nodes, const double* xy,
+                  const double* bathy, int64_t n_elem, const int32_t* tri, int64_t n_edge, const int32_t* edge_elem,
+                  const int8_t* edge_local, const int32_t* edge_bc, const int32_t* elem_edge) {
   if (!out) { g_create_error = "out is NULL"; return DGSWEM_E_ARG; }
   *out = nullptr;
-  dgswem* h = new dgswem();
-  auto bail = [&](int code) { g_create_error = h->err; dgswem_destroy(h); return code; };
-  if (!prm || !xy || !bathy || !tri || !edge_elem || !edge_local || !edge_bc || !elem_edge)
-    return bail(h->fail(DGSWEM_E_ARG, "NULL argument"));
-  if (n_nodes < 3 || n_elem < 1 || n_edge < 3 || n_elem > 0x1fffffff || n_edge > 0x7ffffff0 || n_nodes > 0x7ffffff0)
-    return bail(h->fail(DGSWEM_E_ARG, "bad sizes"));
-  if ((prm->p != 1 && prm->p != 2) || (prm->rk_order != 2 && prm->rk_order != 3))
-    return bail(h->fail(DGSWEM_E_ARG, "p must be 1 or 2, rk_order 2 or 3"));
-  if (prm->flux < 0 || prm->flux > 1 || prm->limiter < 0 || prm->limiter > 2)
-    return bail(h->fail(DGSWEM_E_ARG, "flux must be 0 (LLF) or 1 (Roe), limiter 0, 1 (edge neighbours) or 2 (vertex neighbourhood)"));
-  if (!(prm->h0_dry > 0.0) || !(prm->g > 0.0) || prm->cf < 0.0)
-    return bail(h->fail(DGSWEM_E_ARG, "need h0_dry > 0, g > 0, cf >= 0"));
-  // range of the kernels' reciprocal / square-root routines (rcp_rn, sqrt_rn): arguments are H_c >= h0_dry and g * H_c
-  if (!(prm->h0_dry >= 1e-100) || !(prm->g * prm->h0_dry >= 1e-100) || !(prm->g <= 1e100) || !(prm->h0_dry <= 1e100))
-    return bail(h->fail(DGSWEM_E_ARG, "need 1e-100 <= h0_dry <= 1e100, g <= 1e100 and g*h0_dry >= 1e-100"));
-  h->prm = *prm;
-  h->ndof = (prm->p + 1) * (prm->p + 2) / 2; h->nqe = prm->p + 1; h->nqa = prm->p == 1 ? 3 : 6; h->nstage = prm->rk_order;
-  h->nn = n_nodes; h->ne = n_elem; h->nd = n_edge;
-  h->ld = round_up(n_elem, 256); h->ldd = round_up(n_edge, 256); h->ldn = round_up(n_nodes, 64);
-  int rc = validate_mesh(h, n_nodes, xy, n_elem, tri, n_edge, edge_elem, edge_local, edge_bc, elem_edge);
-  if (rc) return bail(rc);
-
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return bail(h->fail(DGSWEM_E_CUDA, "no CUDA device"));
-  if (prm->device < 0 || prm->device >= ndev) return bail(h->fail(DGSWEM_E_ARG, "device ordinal out of range"));
-  if (cudaSetDevice(prm->device) != cudaSuccess) return bail(h->fail(DGSWEM_E_CUDA, "cudaSetDevice failed"));
-  if (hooks && hooks->alloc && hooks->free) { h->hooks = *hooks; h->have_hooks = true; }
-  if (hooks && hooks->stream) {
-    h->stream = (cudaStream_t)hooks->stream;
-  } else {
-    if (cudaStreamCreateWithFlags(&h->stream, cudaStreamNonBlocking) != cudaSuccess)
-      return bail(h->fail(DGSWEM_E_CUDA, "cudaStreamCreate failed"));
-    h->own_stream = true;
+  if (prm && prm->precision != 0 && prm->precision != 64 && prm->precision != 32) {
+    g_create_error = "precision must be 64 (or 0) or 32";
+    return DGSWEM_E_ARG;
   }
-
-  auto body = [&]() -> int {
-    // ---- tables to constant memory (both degrees; identical for every handle)
-    Tables T1, T2;
-    make_tables(1, T1); make_tables(2, T2);
-    CK(cudaMemcpyToSymbolAsync(c_tab1, &T1, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
-    CK(cudaMemcpyToSymbolAsync(c_tab2, &T2, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
-    CK(cudaStreamSynchronize(h->stream));
-
-    h->res_edge[0] = resident_ctas(k_edge_pipe<1>, DGK_EDGE_THREADS, 0, prm->device);
-    h->res_edge[1] = resident_ctas(k_edge_pipe<2>, DGK_EDGE_THREADS, 0, prm->device);
-    // tuning / test knob: DGSWEM_PERSISTENT_CTAS=n caps the persistent grid at n CTAs (so that small
-    // meshes walk several tiles per CTA); 0 switches the persistent kernel off
-    CK(cudaFuncSetAttribute(k_limwd_tma<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<1>::kSmem));
-    CK(cudaFuncSetAttribute(k_limwd_tma<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<2>::kSmem));
-    CK(cudaFuncSetAttribute(k_limwd_tma<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<1>::kSmem));
-    CK(cudaFuncSetAttribute(k_limwd_tma<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<2>::kSmem));
-    if (prm->limiter == 2)
-      h->res_limwd = prm->p == 1 ? resident_ctas(k_limwd_tma<1, 2>, 128, LimTile<1>::kSmem, prm->device)
-                                 : resident_ctas(k_limwd_tma<2, 2>, 128, LimTile<2>::kSmem, prm->device);
-    else
-      h->res_limwd = prm->p == 1 ? resident_ctas(k_limwd_tma<1, 1>, 128, LimTile<1>::kSmem, prm->device)
-                                 : resident_ctas(k_limwd_tma<2, 1>, 128, LimTile<2>::kSmem, prm->device);
-    if (const char* env = std::getenv("DGSWEM_PERSISTENT_CTAS")) {
-      const int cap = std::atoi(env);
-
-      for (int& r : h->res_edge) r = cap <= 0 ? 0 : std::min(r, cap);
-      h->res_limwd = cap <= 0 ? 0 : std::min(h->res_limwd, cap);
-    }
-
-    // DGSWEM_FUSED=1/0: element-centric stage kernel (no flux buffer) on/off; default: on for p = 1
-    h->fused = prm->p == 1;
-    if (const char* env = std::getenv("DGSWEM_FUSED")) h->fused = std::atoi(env) != 0;
-
-    const long long ne = h->ne, nd = h->nd, nn = h->nn, ld = h->ld, ldd = h->ldd, ldn = h->ldn;
-    // ---- renumbering (internal only): perm_e[new] = old
-    std::vector<int> perm_e(ne), inv_e(ne), perm_d(nd), inv_d(nd);
-    if (prm->reorder == 1) {
-      std::vector<double> cx(ne), cy(ne);
-      for (long long e = 0; e < ne; ++e) {
-        const int* t = tri + 3 * e;
-        cx[e] = (xy[2 * (long long)t[0]] + xy[2 * (long long)t[1]] + xy[2 * (long long)t[2]]) / 3.0;
-        cy[e] = (xy[2 * (long long)t[0] + 1] + xy[2 * (long long)t[1] + 1] + xy[2 * (long long)t[2] + 1]) / 3.0;
-      }
-      perm_e = hilbert_order(cx, cy);
-    } else {
-      std::iota(perm_e.begin(), perm_e.end(), 0);
-      std::iota(perm_d.begin(), perm_d.end(), 0);
-    }
-    for (long long i = 0; i < ne; ++i) inv_e[perm_e[i]] = (int)i;
-    if (prm->reorder == 1) {
-      // edges follow the elements: sorted by (first, second) of their two elements in the new element
-      // numbering, so an edge sits next to the first element that needs it and the
-      // state gather of consecutive edges walks consecutive elements
-      std::vector<uint64_t> key(nd);
-      for (long long d = 0; d < nd; ++d) {
-        const uint32_t ip = (uint32_t)inv_e[edge_elem[2 * d]];
-        const uint32_t im = edge_elem[2 * d + 1] >= 0 ? (uint32_t)inv_e[edge_elem[2 * d + 1]] : ip;
-        key[d] = ((uint64_t)std::min(ip, im) << 32) | (uint64_t)std::max(ip, im);
-      }
-      std::iota(perm_d.begin(), perm_d.end(), 0);
-      std::stable_sort(perm_d.begin(), perm_d.end(), [&](int x, int y) { return key[x] < key[y]; });
-    }
-    for (long long i = 0; i < nd; ++i) inv_d[perm_d[i]] = (int)i;
-
-    // ---- element geometry in internal order (same expression trees as the spec)
-    std::vector<double> jinv(4 * ld, 0.0), lfac(3 * ld, 0.0), hv(3 * ld, 0.0);
-    std::vector<int> ee_packed(3 * ld, 0), nbr(3 * ld, -1), trin(3 * ld, 0), nbinfo(3 * ld, (int)0x80000001);
-    std::vector<double> enl(6 * ld, 0.0);
-    for (long long i = 0; i < ne; ++i) {
-      const long long e = perm_e[i];
-      const int* t = tri + 3 * e;
-      const double x0 = xy[2 * (long long)t[0]], y0 = xy[2 * (long long)t[0] + 1];
-      const double x1 = xy[2 * (long long)t[1]], y1 = xy[2 * (long long)t[1] + 1];
-      const double x2 = xy[2 * (long long)t[2]], y2 = xy[2 * (long long)t[2] + 1];
-      const double dx1 = x1 - x0, dy1 = y1 - y0, dx2 = x2 - x0, dy2 = y2 - y0;
-      const double A = 0.5 * (dx1 * dy2 - dx2 * dy1);
-      const double rA = 1.0 / A;
-      jinv[tix(4, 0, i)] = dy2 * rA;
-      jinv[tix(4, 1, i)] = (-dx2) * rA;
-      jinv[tix(4, 2, i)] = (-dy1) * rA;
-      jinv[tix(4, 3, i)] = dx1 * rA;
-      for (int l = 0; l < 3; ++l) {
-        const long long na = t[(l + 1) % 3], nb = t[(l + 2) % 3];
-        const double ex = xy[2 * nb] - xy[2 * na], ey = xy[2 * nb + 1] - xy[2 * na + 1];
-        const double L = std::sqrt(ex * ex + ey * ey);
-        lfac[tix(3, l, i)] = L * rA;
-        hv[tix(3, l, i)] = bathy[t[l]];
-        trin[tix(3, l, i)] = t[l];
-        const long long d = elem_edge[3 * e + l];
-        const bool plus = edge_elem[2 * d] == e && edge_local[2 * d] == l;
-        ee_packed[tix(3, l, i)] = inv_d[d] | (plus ? 0 : (int)0x80000000);
-        const long long other = plus ? edge_elem[2 * d + 1] : edge_elem[2 * d];
-        nbr[tix(3, l, i)] = other >= 0 ? inv_e[other] : -1;
-        // element-centric form: neighbour id | its local edge << 29 (or bit 31 | boundary code), and the
-        // outward normal: the e+ side's normal (computed from the e+ vertices, as for the edge kernel) or its negative
-        const int lo = plus ? edge_local[2 * d + 1] : edge_local[2 * d];
-        nbinfo[tix(3, l, i)] = other >= 0 ? (inv_e[other] | (lo << 29)) : (int)(0x80000000u | (unsigned)edge_bc[d]);
-        const long long ep = edge_elem[2 * d];
-        const int lp = edge_local[2 * d];
-        const long long pa = tri[3 * ep + (lp + 1) % 3], pb = tri[3 * ep + (lp + 2) % 3];
-        const double px = xy[2 * pb] - xy[2 * pa], py = xy[2 * pb + 1] - xy[2 * pa + 1];
-        const double rL = 1.0 / std::sqrt(px * px + py * py);
-        const double nx = py * rL, ny = (-px) * rL;
-        enl[tix(6, 2 * l, i)] = plus ? nx : -nx;
-        enl[tix(6, 2 * l + 1, i)] = plus ? ny : -ny;
-      }
-    }
-    // ---- edge geometry in internal order, from the e+ side
-    std::vector<int2> ee(ldd, make_int2(0, -1));
-    std::vector<int> einfo(ldd, 1 << 4);
-    std::vector<double> en(2 * ldd, 0.0), ehb(2 * ldd, 0.0);
-    for (long long i = 0; i < nd; ++i) {
-      const long long d = perm_d[i];
-      const long long ep = edge_elem[2 * d], em = edge_elem[2 * d + 1];
-      const int lp = edge_local[2 * d], lm = em >= 0 ? edge_local[2 * d + 1] : 0;
-      const long long na = tri[3 * ep + (lp + 1) % 3], nb = tri[3 * ep + (lp + 2) % 3];
-      const double ex = xy[2 * nb] - xy[2 * na], ey = xy[2 * nb + 1] - xy[2 * na + 1];
-      const double L = std::sqrt(ex * ex + ey * ey);
-      const double rL = 1.0 / L;
-      en[i] = ey * rL;
-      en[ldd + i] = (-ex) * rL;
-      ehb[i] = bathy[na];
-      ehb[ldd + i] = bathy[nb];
-      ee[i] = make_int2(inv_e[ep], em >= 0 ? inv_e[em] : -1);
-      einfo[i] = lp | (lm << 2) | (edge_bc[d] << 4);
-    }
-    // node -> incident (element, vertex) lists for the nodal output, in ascending caller element id
-    std::vector<int> node_ptr(nn + 1, 0), node_ev(3 * ne, 0);
-    for (long long e = 0; e < ne; ++e) for (int v = 0; v < 3; ++v) node_ptr[tri[3 * e + v] + 1]++;
-    for (long long n = 0; n < nn; ++n) node_ptr[n + 1] += node_ptr[n];
-    {
-      std::vector<int> fill(node_ptr.begin(), node_ptr.end() - 1);
-      for (long long e = 0; e < ne; ++e) for (int v = 0; v < 3; ++v) node_ev[fill[tri[3 * e + v]]++] = inv_e[e] * 4 + v;
-    }
-    std::vector<double> nxy(2 * ldn, 0.0);
-    for (long long i = 0; i < nn; ++i) { nxy[i] = xy[2 * i]; nxy[ldn + i] = xy[2 * i + 1]; }
-
-    int r;
-    if ((r = upload(h, h->jinv, jinv))) return r;
-    if ((r = upload(h, h->lfac, lfac))) return r;
-    if ((r = upload(h, h->hv, hv))) return r;
-    if ((r = upload(h, h->elem_edge, ee_packed))) return r;
-    if ((r = upload(h, h->nbr, nbr))) return r;
-    if ((r = upload(h, h->nbinfo, nbinfo))) return r;
-    if ((r = upload(h, h->enl, enl))) return r;
-    if ((r = upload(h, h->tri, trin))) return r;
-    if ((r = upload(h, h->edge_elem, ee))) return r;
-    if ((r = upload(h, h->einfo, einfo))) return r;
-    if ((r = upload(h, h->en, en))) return r;
-    if ((r = upload(h, h->ehb, ehb))) return r;
-    if ((r = upload(h, h->nxy, nxy))) return r;
-    if ((r = upload(h, h->node_ptr, node_ptr))) return r;
-    if ((r = upload(h, h->node_ev, node_ev))) return r;
-    if (prm->reorder == 1) {
-      if ((r = upload(h, h->perm_e, perm_e))) return r;
-      if ((r = upload(h, h->inv_e, inv_e))) return r;
-      if ((r = upload(h, h->inv_d, inv_d))) return r;
-    }
-    const size_t wbytes = (size_t)3 * h->ndof * ld * sizeof(double);
-    for (int i = 0; i < h->nstage; ++i) {
-      h->W[i] = (double*)h->dalloc(wbytes);
-      if (!h->W[i]) return h->fail(DGSWEM_E_CUDA, "device allocation of %zu bytes failed", wbytes);
-      CK(cudaMemsetAsync(h->W[i], 0, wbytes, h->stream));
-    }
-    const size_t fbytes = (size_t)3 * h->nqe * ldd * sizeof(double);
-    h->stage_bytes = std::max(wbytes, fbytes);
-    h->flux = (double*)h->dalloc(fbytes);
-    h->mean = (double*)h->dalloc((size_t)3 * ld * sizeof(double));
-    h->tau = (double*)h->dalloc((size_t)2 * ldn * sizeof(double));
-    h->etap = (double*)h->dalloc((size_t)ldn * sizeof(double));
-    if (prm->limiter == 2) {
-      h->nmm = (double*)h->dalloc((size_t)6 * ldn * sizeof(double));
-      if (!h->nmm) return h->fail(DGSWEM_E_CUDA, "device allocation failed");
-    }
-    h->stage_buf = (double*)h->dalloc(h->stage_bytes);
-    h->wet = (unsigned char*)h->dalloc((size_t)ld);
-    h->wet_stage = (unsigned char*)h->dalloc((size_t)ld);
-    h->nf_flag = (int*)h->dalloc(256);
-    h->step_ctr = (int*)h->dalloc(256);
-    h->last_out = h->W[0];
-    if (const char* env = std::getenv("DGSWEM_GRAPH")) h->graphs_on = std::atoi(env) != 0;
-    if (!h->flux || !h->mean || !h->tau || !h->etap || !h->stage_buf || !h->wet || !h->wet_stage || !h->nf_flag || !h->step_ctr)
-      return h->fail(DGSWEM_E_CUDA, "device allocation failed");
-    CK(cudaMemsetAsync(h->flux, 0, fbytes, h->stream));
-    CK(cudaMemsetAsync(h->mean, 0, (size_t)3 * ld * sizeof(double), h->stream));
-    CK(cudaMemsetAsync(h->tau, 0, (size_t)2 * ldn * sizeof(double), h->stream));
-    CK(cudaMemsetAsync(h->etap, 0, (size_t)ldn * sizeof(double), h->stream));
-    CK(cudaMemsetAsync(h->wet, 1, (size_t)ld, h->stream));
-    CK(cudaStreamSynchronize(h->stream));
-    return 0;
-  };
-  rc = body();
-  if (rc) return bail(rc);
-  *out = h;
-  return DGSWEM_OK;
+  if (prm && prm->precision == 32)
+    return imp32::api_create(out, prm, hooks, n_nodes, xy, bathy, n_elem, tri, n_edge, edge_elem, edge_local, edge_bc, elem_edge);
+  return imp64::api_create(out, prm, hooks, n_nodes, xy, bathy, n_elem, tri, n_edge, edge_elem, edge_local, edge_bc, elem_edge);
 }
 
-int dgswem_set_state(dgswem_t* h, double t, const double* ze, const double* qx, const double* qy) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!ze || !qx || !qy) return h->fail(DGSWEM_E_ARG, "NULL state pointer");
-  CK(cudaSetDevice(h->prm.device));
-  const double* src[3] = {ze, qx, qy};
-  const size_t row = (size_t)h->ne * sizeof(double);
-  // stage in caller order (rows of length ne, leading dimension ld), then renumber into the tiled layout on the device
-  double* stage = h->stage_buf;
-  for (int c = 0; c < 3; ++c)
-    CK(cudaMemcpy2DAsync(stage + (size_t)c * h->ndof * h->ld, (size_t)h->ld * sizeof(double), src[c], row, row, h->ndof,
-                         cudaMemcpyHostToDevice, h->stream));
-  k_rows_to_tiled<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->W[0], stage, h->ld, h->perm_e, (int)h->ne, 3 * h->ndof);
-  CKL("k_rows_to_tiled");
-  k_fill_bytes<<<grid_for(h->ld, 256), 256, 0, h->stream>>>(h->wet, 1, (int)h->ld);
-  CKL("k_fill_bytes");
-  if (h->prm.wetdry) {
-    if (h->prm.p == 1) k_wetdry_only<1><<<grid_for(h->ne, 128), 128, 0, h->stream>>>(h->W[0], h->hv, h->wet, (int)h->ne, h->ld, h->prm.h0_dry);
-    else k_wetdry_only<2><<<grid_for(h->ne, 128), 128, 0, h->stream>>>(h->W[0], h->hv, h->wet, (int)h->ne, h->ld, h->prm.h0_dry);
-    CKL("k_wetdry_only");
-  }
-  CK(cudaStreamSynchronize(h->stream));   // the caller's buffers may be reused after return
-  h->t = t;
-  h->step_dt = 0.0;
-  h->last_out = h->W[0];
-  return DGSWEM_OK;
-}
+void dgswem_destroy(dgswem_t* h) { if (h) DISPATCH(h, api_destroy); }
 
-int dgswem_set_tide(dgswem_t* h, double amp, double omega, double phase) {
-  if (!h) return DGSWEM_E_ARG;
-  h->tide_amp = amp; h->tide_omega = omega; h->tide_phase = phase;
-  return DGSWEM_OK;
-}
-
-int dgswem_set_wind_holland(dgswem_t* h, const dgswem_holland* hol) {
-  if (!h) return DGSWEM_E_ARG;
-  drop_graphs(h);   // the vortex parameters are frozen arguments of a captured wind kernel
-  if (hol) {
-    if (!(hol->rmax > 0.0) || !(hol->rho_air > 0.0) || !(hol->rho_water > 0.0) || !(hol->B > 0.0))
-      return h->fail(DGSWEM_E_ARG, "Holland parameters must be positive");
-    h->hol = *hol; h->wind_on = true;
-  } else {
-    h->wind_on = false;
-  }
-  return DGSWEM_OK;
-}
-
-int dgswem_set_wind_forcing(dgswem_t* h, int stress_on, int pressure_on) {
-  if (!h) return DGSWEM_E_ARG;
-  drop_graphs(h);   // frozen kernel arguments
-  h->stress_on = stress_on != 0; h->press_on = pressure_on != 0;
-  return DGSWEM_OK;
-}
-
-int dgswem_set_rain(dgswem_t* h, double rate) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!std::isfinite(rate)) return h->fail(DGSWEM_E_ARG, "rain rate must be finite");
-  drop_graphs(h);
-  h->rain = rate;
-  return DGSWEM_OK;
-}
-
-int dgswem_step(dgswem_t* h, int64_t nsteps, double dt) {
-  if (!h) return DGSWEM_E_ARG;
-  if (nsteps < 0 || !(dt > 0.0)) return h->fail(DGSWEM_E_ARG, "need nsteps >= 0 and dt > 0");
-  if (h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a stage-granular step is in progress (dgswem_end_step)");
-  CK(cudaSetDevice(h->prm.device));
-  return h->prm.p == 1 ? run_steps<1>(h, nsteps, dt) : run_steps<2>(h, nsteps, dt);
-}
-
-// ---- stage-granular stepping + halo lists: the building blocks of a domain-decomposed run
-namespace {
-struct StageBufs { const double* win; const double* w0; double* wout; double a, b, c; int first; };
-inline StageBufs stage_bufs(dgswem* h, int s) {
-  const bool rk3 = h->prm.rk_order == 3;
-  const double* a = rk3 ? kA3 : kA2; const double* b = rk3 ? kB3 : kB2; const double* c = rk3 ? kC3 : kC2;
-  StageBufs B;
-  B.a = a[s]; B.b = b[s]; B.c = c[s]; B.first = s == 0; B.w0 = h->W[0];
-  if (s == 0) { B.win = h->W[0]; B.wout = h->W[1]; }
-  else if (!rk3 || s == 2) { B.win = h->W[s]; B.wout = h->W[0]; }
-  else { B.win = h->W[1]; B.wout = h->W[2]; }
-  return B;
-}
-}  // namespace
-
-int dgswem_begin_step(dgswem_t* h, double dt) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!(dt > 0.0)) return h->fail(DGSWEM_E_ARG, "need dt > 0");
-  if (h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a step is already in progress");
-  CK(cudaSetDevice(h->prm.device));
-  if (h->wind_on) { int rc = launch_wind(h, h->t); if (rc) return rc; }
-  h->step_dt = dt;
-  h->last_out = h->W[0];
-  return DGSWEM_OK;
-}
-
-int dgswem_stage_rhs(dgswem_t* h, int s) {
-  if (!h) return DGSWEM_E_ARG;
-  if (h->step_dt == 0.0) return h->fail(DGSWEM_E_ARG, "no step in progress (dgswem_begin_step)");
-  if (s < 0 || s >= h->nstage) return h->fail(DGSWEM_E_ARG, "stage index out of range");
-  CK(cudaSetDevice(h->prm.device));
-  const StageBufs B = stage_bufs(h, s);
-  const double ts = h->t + B.c * h->step_dt;
-  const int rc = h->prm.p == 1 ? run_stage_rhs<1>(h, B.win, B.w0, B.wout, h->step_dt, B.a, B.b, B.first, ts, s)
-                               : run_stage_rhs<2>(h, B.win, B.w0, B.wout, h->step_dt, B.a, B.b, B.first, ts, s);
-  if (rc == 0) h->last_out = B.wout;
-  return rc;
-}
-
-int dgswem_stage_limit(dgswem_t* h, int s) {
-  if (!h) return DGSWEM_E_ARG;
-  if (h->step_dt == 0.0) return h->fail(DGSWEM_E_ARG, "no step in progress (dgswem_begin_step)");
-  if (s < 0 || s >= h->nstage) return h->fail(DGSWEM_E_ARG, "stage index out of range");
-  if (h->prm.limiter == 0) return DGSWEM_OK;
-  CK(cudaSetDevice(h->prm.device));
-  const StageBufs B = stage_bufs(h, s);
-  return h->prm.p == 1 ? launch_limwd<1>(h, B.wout) : launch_limwd<2>(h, B.wout);
-}
-
-int dgswem_end_step(dgswem_t* h) {
-  if (!h) return DGSWEM_E_ARG;
-  if (h->step_dt == 0.0) return h->fail(DGSWEM_E_ARG, "no step in progress (dgswem_begin_step)");
-  h->t = h->t + h->step_dt;
-  h->step_dt = 0.0;
-  h->last_out = h->W[0];
-  return DGSWEM_OK;
-}
-
-int dgswem_set_halo(dgswem_t* h, int64_t n_send, const int32_t* send_ids, int64_t n_recv, const int32_t* recv_ids) {
-  if (!h) return DGSWEM_E_ARG;
-  if (h->prm.limiter == 2)
-    return h->fail(DGSWEM_E_ARG, "the vertex-neighbourhood limiter needs the elements around every vertex: one layer of edge-neighbour ghosts is not enough");
-  if (n_send < 0 || n_recv < 0 || (n_send > 0 && !send_ids) || (n_recv > 0 && !recv_ids)) return h->fail(DGSWEM_E_ARG, "bad halo lists");
-  CK(cudaSetDevice(h->prm.device));
-  // caller numbering -> internal numbering (host copy of inv_e)
-  std::vector<int> inv;
-  if (h->inv_e) {
-    inv.resize((size_t)h->ne);
-    CK(cudaMemcpyAsync(inv.data(), h->inv_e, (size_t)h->ne * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
-    CK(cudaStreamSynchronize(h->stream));
-  }
-  auto conv = [&](int64_t n, const int32_t* ids, std::vector<int>& out) -> bool {
-    out.resize((size_t)std::max<int64_t>(n, 1));
-    for (int64_t i = 0; i < n; ++i) {
-      if (ids[i] < 0 || ids[i] >= h->ne) return false;
-      out[(size_t)i] = inv.empty() ? ids[i] : inv[(size_t)ids[i]];
-    }
-    return true;
-  };
-  std::vector<int> snd, rcv;
-  if (!conv(n_send, send_ids, snd) || !conv(n_recv, recv_ids, rcv)) return h->fail(DGSWEM_E_ARG, "halo element id out of range");
-  int r;
-  if ((r = upload(h, h->halo_send, snd))) return r;
-  if ((r = upload(h, h->halo_recv, rcv))) return r;
-  h->n_send = n_send; h->n_recv = n_recv;
-  h->halo_buf = (double*)h->dalloc((size_t)3 * h->ndof * (size_t)std::max<int64_t>(std::max(n_send, n_recv), 1) * sizeof(double));
-  if (!h->halo_buf) return h->fail(DGSWEM_E_CUDA, "device allocation failed");
-  return DGSWEM_OK;
-}
-
-static int halo_rows(const dgswem* h, int what) { return what == 0 ? 3 * h->ndof : 3; }
-
-int dgswem_halo_pack(dgswem_t* h, int what, double* buf, int buf_on_device) {
-  if (!h) return DGSWEM_E_ARG;
-  if ((what != 0 && what != 1) || (!buf && h->n_send > 0)) return h->fail(DGSWEM_E_ARG, "bad halo_pack arguments");
-  if (h->n_send == 0) return DGSWEM_OK;
-  CK(cudaSetDevice(h->prm.device));
-  const int rows = halo_rows(h, what);
-  const double* src = what == 0 ? h->last_out : h->mean;
-  double* dbuf = buf_on_device ? buf : h->halo_buf;
-  k_halo_pack<<<grid_for(h->n_send, 256), 256, 0, h->stream>>>(dbuf, src, h->halo_send, (int)h->n_send, rows);
-  CKL("k_halo_pack");
-  if (!buf_on_device) {
-    CK(cudaMemcpyAsync(buf, dbuf, (size_t)rows * h->n_send * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-    CK(cudaStreamSynchronize(h->stream));
-  }
-  return DGSWEM_OK;
-}
-
-int dgswem_halo_unpack(dgswem_t* h, int what, const double* buf, int buf_on_device) {
-  if (!h) return DGSWEM_E_ARG;
-  if ((what != 0 && what != 1) || (!buf && h->n_recv > 0)) return h->fail(DGSWEM_E_ARG, "bad halo_unpack arguments");
-  if (h->n_recv == 0) return DGSWEM_OK;
-  CK(cudaSetDevice(h->prm.device));
-  const int rows = halo_rows(h, what);
-  double* dst = what == 0 ? h->last_out : h->mean;
-  const double* dbuf = buf;
-  if (!buf_on_device) {
-    CK(cudaMemcpyAsync(h->halo_buf, buf, (size_t)rows * h->n_recv * sizeof(double), cudaMemcpyHostToDevice, h->stream));
-    dbuf = h->halo_buf;
-  }
-  if (what == 0) k_halo_unpack<<<grid_for(h->n_recv, 256), 256, 0, h->stream>>>(dst, dbuf, h->halo_recv, (int)h->n_recv, rows);
-  else k_halo_unpack_means<<<grid_for(h->n_recv, 256), 256, 0, h->stream>>>(h->mean, h->last_out, dbuf, h->halo_recv, (int)h->n_recv, h->ndof);
-  CKL("k_halo_unpack");
-  if (!buf_on_device) CK(cudaStreamSynchronize(h->stream));
-  return DGSWEM_OK;
-}
-
-int dgswem_eval_rhs(dgswem_t* h, double* rze, double* rqx, double* rqy) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!rze || !rqx || !rqy) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
-  CK(cudaSetDevice(h->prm.device));
-  int rc;
-  if (h->wind_on && (rc = launch_wind(h, h->t))) return rc;
-  double* rbuf = h->W[1];   // scratch: W[1] holds no live data between steps
-  if (h->fused) {
-    rc = h->prm.p == 1 ? launch_stage<1, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, 0.0, 1.0, 1, false, false, scal(h, 0, tide_value(h, h->t)))
-                       : launch_stage<2, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, 0.0, 1.0, 1, false, false, scal(h, 0, tide_value(h, h->t)));
-    if (rc) return rc;
-  } else if (h->prm.p == 1) {
-    if ((rc = launch_edge<1>(h, h->W[0], scal(h, 0, tide_value(h, h->t))))) return rc;
-    if ((rc = launch_elem<1, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, 0.0, 1.0, 1, false, false))) return rc;
-  } else {
-    if ((rc = launch_edge<2>(h, h->W[0], scal(h, 0, tide_value(h, h->t))))) return rc;
-    if ((rc = launch_elem<2, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, 0.0, 1.0, 1, false, false))) return rc;
-  }
-  k_tiled_to_rows<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->stage_buf, h->ld, rbuf, h->inv_e, (int)h->ne, 3 * h->ndof);
-  CKL("k_tiled_to_rows");
-  const double* src = h->stage_buf;
-  double* dst[3] = {rze, rqx, rqy};
-  const size_t row = (size_t)h->ne * sizeof(double);
-  for (int c = 0; c < 3; ++c)
-    CK(cudaMemcpy2DAsync(dst[c], row, src + (size_t)c * h->ndof * h->ld, (size_t)h->ld * sizeof(double), row, h->ndof,
-                         cudaMemcpyDeviceToHost, h->stream));
-  CK(cudaStreamSynchronize(h->stream));
-  return DGSWEM_OK;
-}
-
-int dgswem_get_flux(dgswem_t* h, double* flux) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!flux) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
-  CK(cudaSetDevice(h->prm.device));
-  if (h->fused) {   // the element-centric stage kernel keeps no flux buffer: evaluate A1 on the current state
-    int rc = h->prm.p == 1 ? launch_edge<1>(h, h->W[0], scal(h, 0, tide_value(h, h->t))) : launch_edge<2>(h, h->W[0], scal(h, 0, tide_value(h, h->t)));
-    if (rc) return rc;
-  }
-  const double* src = h->flux;
-  if (h->inv_d) {
-    k_gather_rows<<<grid_for(h->nd, 256), 256, 0, h->stream>>>(h->stage_buf, h->ldd, h->flux, h->ldd, h->inv_d, (int)h->nd, 3 * h->nqe);
-    CKL("k_gather_rows");
-    src = h->stage_buf;
-  }
-  const size_t row = (size_t)h->nd * sizeof(double);
-  CK(cudaMemcpy2DAsync(flux, row, src, (size_t)h->ldd * sizeof(double), row, 3 * h->nqe, cudaMemcpyDeviceToHost, h->stream));
-  CK(cudaStreamSynchronize(h->stream));
-  return DGSWEM_OK;
-}
-
-int dgswem_get_state(dgswem_t* h, double* t, double* ze, double* qx, double* qy) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!ze || !qx || !qy) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
-  CK(cudaSetDevice(h->prm.device));
-  k_tiled_to_rows<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->stage_buf, h->ld, h->W[0], h->inv_e, (int)h->ne, 3 * h->ndof);
-  CKL("k_tiled_to_rows");
-  const double* src = h->stage_buf;
-  CK(cudaMemsetAsync(h->nf_flag, 0, sizeof(int), h->stream));
-  k_check_finite<<<148 * 8, 256, 0, h->stream>>>(h->W[0], (long long)3 * h->ndof * h->ld, h->nf_flag);
-  CKL("k_check_finite");
-  double* dst[3] = {ze, qx, qy};
-  const size_t row = (size_t)h->ne * sizeof(double);
-  for (int c = 0; c < 3; ++c)
-    CK(cudaMemcpy2DAsync(dst[c], row, src + (size_t)c * h->ndof * h->ld, (size_t)h->ld * sizeof(double), row, h->ndof,
-                         cudaMemcpyDeviceToHost, h->stream));
-  int flag = 0;
-  CK(cudaMemcpyAsync(&flag, h->nf_flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
-  CK(cudaStreamSynchronize(h->stream));
-  if (t) *t = h->t;
-  if (flag) return h->fail(DGSWEM_E_NONFINITE, "non-finite value in the state at t=%g", h->t);
-  return DGSWEM_OK;
-}
-
-int dgswem_get_wetdry(dgswem_t* h, uint8_t* wet) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!wet) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
-  CK(cudaSetDevice(h->prm.device));
-  const unsigned char* src = h->wet;
-  if (h->inv_e) {
-    k_gather_bytes<<<grid_for(h->ne, 256), 256, 0, h->stream>>>(h->wet_stage, h->wet, h->inv_e, (int)h->ne);
-    CKL("k_gather_bytes");
-    src = h->wet_stage;
-  }
-  CK(cudaMemcpyAsync(wet, src, (size_t)h->ne, cudaMemcpyDeviceToHost, h->stream));
-  CK(cudaStreamSynchronize(h->stream));
-  return DGSWEM_OK;
-}
-
-int dgswem_get_nodal(dgswem_t* h, double* zn, double* qxn, double* qyn) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!zn || !qxn || !qyn) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
-  CK(cudaSetDevice(h->prm.device));
-  double* out = h->stage_buf;   // [3][ldn] (3 * ldn <= the state-sized staging buffer: n_nodes < n_elem + 3 for any triangulation with a boundary)
-  if ((size_t)3 * h->ldn * sizeof(double) > h->stage_bytes) return h->fail(DGSWEM_E_ARG, "nodal output needs n_nodes <= ndof * n_elem");
-  if (h->prm.p == 1) k_nodal<1><<<grid_for(h->nn, 256), 256, 0, h->stream>>>(out, h->ldn, h->W[0], h->node_ptr, h->node_ev, (int)h->nn);
-  else k_nodal<2><<<grid_for(h->nn, 256), 256, 0, h->stream>>>(out, h->ldn, h->W[0], h->node_ptr, h->node_ev, (int)h->nn);
-  CKL("k_nodal");
-  double* dst[3] = {zn, qxn, qyn};
-  for (int c = 0; c < 3; ++c)
-    CK(cudaMemcpyAsync(dst[c], out + (size_t)c * h->ldn, (size_t)h->nn * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-  CK(cudaStreamSynchronize(h->stream));
-  return DGSWEM_OK;
-}
-
-int dgswem_get_wind(dgswem_t* h, double* tau) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!tau) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
-  CK(cudaSetDevice(h->prm.device));
-  const size_t row = (size_t)h->nn * sizeof(double);
-  CK(cudaMemcpy2DAsync(tau, row, h->tau, (size_t)h->ldn * sizeof(double), row, 2, cudaMemcpyDeviceToHost, h->stream));
-  CK(cudaStreamSynchronize(h->stream));
-  return DGSWEM_OK;
-}
-
-int dgswem_get_pressure(dgswem_t* h, double* etap) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!etap) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
-  CK(cudaSetDevice(h->prm.device));
-  CK(cudaMemcpyAsync(etap, h->etap, (size_t)h->nn * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-  CK(cudaStreamSynchronize(h->stream));
-  return DGSWEM_OK;
-}
-
-int dgswem_test_math(dgswem_t* h, int64_t n, const double* x, double* out) {
-  if (!h) return DGSWEM_E_ARG;
-  if (n < 1 || !x || !out) return h->fail(DGSWEM_E_ARG, "need n >= 1 and non-NULL pointers");
-  CK(cudaSetDevice(h->prm.device));
-  double* dx = (double*)h->dalloc((size_t)n * sizeof(double));
-  double* dout = (double*)h->dalloc((size_t)4 * n * sizeof(double));
-  if (!dx || !dout) return h->fail(DGSWEM_E_CUDA, "device allocation failed");
-  CK(cudaMemcpyAsync(dx, x, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
-  k_test_math<<<grid_for(n, 256), 256, 0, h->stream>>>(dx, (long long)n, dout);
-  CKL("k_test_math");
-  CK(cudaMemcpyAsync(out, dout, (size_t)4 * n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-  CK(cudaStreamSynchronize(h->stream));
-  return DGSWEM_OK;   // the two scratch buffers stay with the handle until dgswem_destroy
-}
-
-int dgswem_fp64_peak(dgswem_t* h, double* dfma_per_s) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!dfma_per_s) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
-  CK(cudaSetDevice(h->prm.device));
-  int sms = 0;
-  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->prm.device));
-  const int grid = sms * 8, threads = 256, rounds = 20000;
-  cudaEvent_t a, b;
-  CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
-  double best = 0.0;
-  for (int rep = 0; rep < 4; ++rep) {      // first repetition warms up
-    CK(cudaEventRecord(a, h->stream));
-    k_dfma_probe<<<grid, threads, 0, h->stream>>>(h->stage_buf, rounds, 0.999999, 1e-6);
-    CKL("k_dfma_probe");
-    CK(cudaEventRecord(b, h->stream));
-    CK(cudaEventSynchronize(b));
-    float ms = 0.f;
-    CK(cudaEventElapsedTime(&ms, a, b));
-    const double rate = (double)grid * threads * 8.0 * rounds / (ms * 1e-3);
-    if (rep > 0 && rate > best) best = rate;
-  }
-  cudaEventDestroy(a); cudaEventDestroy(b);
-  *dfma_per_s = best;
-  return DGSWEM_OK;
-}
-
-int dgswem_stage_form(const dgswem_t* h) { return (h && h->fused) ? 1 : 0; }
-
-int64_t dgswem_launch_count(const dgswem_t* h) { return h ? h->launches : 0; }
-
-int dgswem_profile(dgswem_t* h, int enable) {
-  if (!h) return DGSWEM_E_ARG;
-  h->profiling = enable != 0;
-  return DGSWEM_OK;
-}
-
-int dgswem_profile_read(dgswem_t* h, double* ms, int64_t* count) {
-  if (!h) return DGSWEM_E_ARG;
-  if (!ms || !count) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
-  CK(cudaSetDevice(h->prm.device));
-  CK(cudaStreamSynchronize(h->stream));
-  for (int k = 0; k < PK_COUNT; ++k) { ms[k] = 0.0; count[k] = 0; }
-  for (auto& r : h->prof) {
-    float t = 0.f;
-    if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) { ms[r.kind] += (double)t; count[r.kind]++; }
-    cudaEventDestroy(r.a); cudaEventDestroy(r.b);
-  }
-  h->prof.clear();
-  return DGSWEM_OK;
-}
-
-int dgswem_sync(dgswem_t* h) {
-  if (!h) return DGSWEM_E_ARG;
-  CK(cudaSetDevice(h->prm.device));
-  CK(cudaStreamSynchronize(h->stream));
-  return DGSWEM_OK;
-}
+int dgswem_end_step(dgswem_t* h) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_end_step); }
+int dgswem_sync(dgswem_t* h) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_sync); }
+int dgswem_set_state(dgswem_t* h, double t, const double* ze, const double* qx, const double* qy) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_set_state, t, ze, qx, qy); }
+int dgswem_set_tide(dgswem_t* h, double amp, double omega, double phase) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_set_tide, amp, omega, phase); }
+int dgswem_set_wind_holland(dgswem_t* h, const dgswem_holland* hol) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_set_wind_holland, hol); }
+int dgswem_set_wind_forcing(dgswem_t* h, int stress_on, int pressure_on) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_set_wind_forcing, stress_on, pressure_on); }
+int dgswem_set_rain(dgswem_t* h, double rate) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_set_rain, rate); }
+int dgswem_step(dgswem_t* h, int64_t nsteps, double dt) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_step, nsteps, dt); }
+int dgswem_begin_step(dgswem_t* h, double dt) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_begin_step, dt); }
+int dgswem_stage_rhs(dgswem_t* h, int s) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_stage_rhs, s); }
+int dgswem_stage_limit(dgswem_t* h, int s) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_stage_limit, s); }
+int dgswem_set_halo(dgswem_t* h, int64_t n_send, const int32_t* send_ids, int64_t n_recv, const int32_t* recv_ids) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_set_halo, n_send, send_ids, n_recv, recv_ids); }
+int dgswem_halo_pack(dgswem_t* h, int what, double* buf, int buf_on_device) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_halo_pack, what, buf, buf_on_device); }
+int dgswem_halo_unpack(dgswem_t* h, int what, const double* buf, int buf_on_device) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_halo_unpack, what, buf, buf_on_device); }
+int dgswem_eval_rhs(dgswem_t* h, double* rze, double* rqx, double* rqy) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_eval_rhs, rze, rqx, rqy); }
+int dgswem_get_flux(dgswem_t* h, double* flux) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_get_flux, flux); }
+int dgswem_get_state(dgswem_t* h, double* t, double* ze, double* qx, double* qy) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_get_state, t, ze, qx, qy); }
+int dgswem_get_wetdry(dgswem_t* h, uint8_t* wet) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_get_wetdry, wet); }
+int dgswem_get_nodal(dgswem_t* h, double* zn, double* qxn, double* qyn) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_get_nodal, zn, qxn, qyn); }
+int dgswem_get_wind(dgswem_t* h, double* tau) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_get_wind, tau); }
+int dgswem_get_pressure(dgswem_t* h, double* etap) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_get_pressure, etap); }
+int dgswem_test_math(dgswem_t* h, int64_t n, const double* x, double* out) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_test_math, n, x, out); }
+int dgswem_fp64_peak(dgswem_t* h, double* dfma_per_s) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_fp64_peak, dfma_per_s); }
+int dgswem_stage_form(const dgswem_t* h) { return h ? DISPATCH_C(h, api_stage_form) : 0; }
+int dgswem_precision(const dgswem_t* h) { return h ? h->precision : 0; }
+int64_t dgswem_launch_count(const dgswem_t* h) { return h ? DISPATCH_C(h, api_launch_count) : 0; }
+int dgswem_profile(dgswem_t* h, int enable) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_profile, enable); }
+int dgswem_profile_read(dgswem_t* h, double* ms, int64_t* count) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_profile_read, ms, count); }
 
 }  // extern "C"

@@ -1,0 +1,124 @@
+"""The fp32 variant of the CUDA path (dgswem_params.precision = 32, PAPER.md:158 "-r4", :529
+"computation is done with single-precision") against the binary32 build of the oracle -- element by element, EXACTLY:
+both sides perform the same sequence of IEEE binary32 operations -- and against the pinned
+binary64 oracle within the binary32 tolerance DESIGN.md section 11 states (relative L2 <= 2e-5 over these step counts).
+The ABI is binary64 in both precisions: what the fp32 handle returns are binary32 values widened exactly."""
+import math
+
+import numpy as np
+import pytest
+
+from workloads import c1, c2, c3, c4, c5, perturbed, with_forcing
+from workloads.configs import Workload
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def G():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2508_21208_b200 import build
+    build.build()
+    import paper_2508_21208_b200 as pk
+    return pk
+
+
+@pytest.fixture(scope="module")
+def O32():
+    from oracle import oracle32
+    oracle32.build()
+    return oracle32
+
+
+@pytest.fixture(autouse=True, params=["0", "1"], ids=["edge+elem", "stage"])
+def kernel_path(request, monkeypatch):
+    monkeypatch.setenv("DGSWEM_FUSED", request.param)
+    return request.param
+
+
+def _with_params(w, **kw):
+    prm = dict(w.params); prm.update(kw)
+    return Workload(w.name, w.mesh, w.bathy, prm, w.ze, w.qx, w.qy, w.dt, w.nsteps, tide=w.tide, holland=w.holland, notes=w.notes)
+
+
+RECIPES = {
+    "c1": lambda: c1(),
+    "c2p1": lambda: perturbed(c2(nq=40, p=1, state="hump", nsteps=30), amp_z=0.2),
+    "c2p2": lambda: perturbed(c2(nq=40, p=2, state="hump", nsteps=30), amp_z=0.2),
+    "c2rest": lambda: c2(nq=40, p=1, state="rest", nsteps=30),
+    "c3": lambda: perturbed(c3(nn=60, nsteps=40)),
+    "c4": lambda: c4(nqx=64, nqy=32, nsteps=80),
+    "c5": lambda: c5(nn=40, nsteps=40),
+    "c5-roe-vertexlim-pressure-rain": lambda: with_forcing(_with_params(c5(nn=40, nsteps=30), flux=1, limiter=2), pressure=True, rain=1e-5),
+    "c4-roe": lambda: _with_params(c4(nqx=64, nqy=32, nsteps=60), flux=1),
+}
+
+
+@pytest.mark.parametrize("recipe", sorted(RECIPES))
+def test_fp32_path_equals_the_fp32_oracle(O, O32, G, recipe):
+    w = RECIPES[recipe]()
+    o32 = O32.Oracle.from_workload(w)
+    g = G.Dgswem.from_workload(w, reorder=1, precision=32)
+    assert g.precision() == 32
+    wide = lambda a: np.asarray(a, dtype=np.float64)
+    assert np.array_equal(g.get_wetdry(), o32.get_wetdry())
+    r_cpu, r_gpu = o32.eval_rhs(), g.eval_rhs()
+    assert np.array_equal(g.get_flux(), wide(o32.get_flux()))
+    for c in range(3):
+        assert np.array_equal(r_gpu[c], wide(r_cpu[c]))
+    if w.holland is not None:
+        assert np.array_equal(g.get_wind(), wide(o32.get_wind()))
+        assert np.array_equal(g.get_pressure(), wide(o32.get_pressure()))
+    half = w.nsteps // 2
+    for n in (half, w.nsteps - half):
+        o32.step(n, w.dt); g.step(n, w.dt)
+    t_cpu, *s_cpu = o32.get_state()
+    t_gpu, *s_gpu = g.get_state()
+    assert t_cpu == t_gpu
+    for c in range(3):
+        assert np.isfinite(s_cpu[c]).all()
+        assert np.array_equal(s_gpu[c], wide(s_cpu[c]))
+        assert np.array_equal(s_gpu[c], s_gpu[c].astype(np.float32).astype(np.float64))      # binary32 values, widened
+    assert np.array_equal(g.get_wetdry(), o32.get_wetdry())
+    for a, b in zip(g.get_nodal(), o32.get_nodal()):
+        assert np.array_equal(a, wide(b))
+    g.close()
+    # ... and against the pinned binary64 oracle, within binary32 rounding
+    o = O.Oracle.from_workload(w)
+    o.step(w.nsteps, w.dt)
+    _, *s64 = o.get_state()
+    for c in range(3):
+        den = math.sqrt(float((s64[c] ** 2).sum()))
+        # relative part + the rounding floor of a state that cancels to zero in exact arithmetic (lake at rest: momentum
+        # noise ~ eps32 x pressure terms, about 1e-6 per entry; 1e-7 for the elevation)
+        floor = (1e-7 if c == 0 else 1e-5) * math.sqrt(s64[c].size)
+        assert math.sqrt(float(((s_gpu[c] - s64[c]) ** 2).sum())) <= 2e-5 * den + floor
+    assert (o.get_wetdry() != o32.get_wetdry()).mean() <= 0.01
+
+
+def test_fp32_graph_replay_and_stage_api(G):
+    """Graph replay, plain stream launches and the stage-granular API give the same bits in fp32 too."""
+    import os
+    w = c5(nn=30, nsteps=12)
+    outs = []
+    for mode in ("graph", "stream", "stages"):
+        if mode == "stream":
+            os.environ["DGSWEM_GRAPH"] = "0"
+        g = G.Dgswem.from_workload(w, precision=32)
+        os.environ.pop("DGSWEM_GRAPH", None)
+        if mode == "stages":
+            for _ in range(w.nsteps):
+                g.begin_step(w.dt)
+                for s in range(w.n_stage):
+                    g.stage_rhs(s); g.stage_limit(s)
+                g.end_step()
+        else:
+            g.step(w.nsteps, w.dt)
+        outs.append((g.get_state(), g.get_wetdry()))
+        g.close()
+    for k in (1, 2):
+        for a, b in zip(outs[0][0], outs[k][0]):
+            assert np.array_equal(a, b)
+        assert np.array_equal(outs[0][1], outs[k][1])
