@@ -205,6 +205,13 @@ def whole_job_value(world: int, dofs_stage: int, steps: int, seconds: float) -> 
     return world * dofs_stage * steps / seconds
 
 
+def workload_config(w) -> dict:
+    """What names the workload: the SAME dict on both arms (the driver compares them); how an arm ran it is in `run`."""
+    return {"workload": w.name, "n_elem": w.mesh.n_elem, "n_edge": w.mesh.n_edge, "n_nodes": w.mesh.n_nodes, "p": w.params["p"],
+            "rk_order": w.params["rk_order"], "dt": w.dt, "limiter": w.params["limiter"], "wetdry": w.params["wetdry"],
+            "flux": w.params.get("flux", 0), "wind": w.holland is not None, "tide": w.tide is not None}
+
+
 def run_reference(args, rank: int):
     """The CPU oracle, as it stands, on the host cores (bench contract: reference arm)."""
     if rank != 0:
@@ -226,11 +233,13 @@ def run_reference(args, rank: int):
     dt = time.perf_counter() - t0
     value = w.dofs * w.n_stage * args.steps / dt
     sample = f"{w.name}: {w.mesh.n_elem} elements, {args.steps} steps after {args.warmup} warm-up"
-    line = {"impl": "reference", "metric": METRIC.replace("fp64", "fp32") if args.dtype == "f32" else METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+    cfg = workload_config(w if scale == 1.0 else make_workload(args.workload))     # the arm's config names the full workload
+    line = {"impl": "reference", "metric": METRIC.replace("fp64", "fp32") if args.dtype == "f32" else METRIC, "value": value, "unit": UNIT,
+            "n_gpus": int(os.environ.get("WORLD_SIZE", args.gpus)), "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
-            "config": {"workload": w.name, "n_elem": w.mesh.n_elem, "p": w.params["p"], "rk_order": w.params["rk_order"],
-                       "dt": w.dt, "kind": "CPU oracle (oracle/dgswem_oracle.c, gcc -O2 -ffp-contract=off, OpenMP)"},
+            "config": cfg,
+            "run": {"kind": "CPU oracle (oracle/dgswem_oracle.c, gcc -O2 -ffp-contract=off, OpenMP)", "sample": sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -425,17 +434,25 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     line = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms / args.steps, "ms_per_step_with_per_launch_events": ms_prof / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
             "data": "synthetic",
-            "config": {"workload": w.name, "n_elem": w.mesh.n_elem, "n_edge": w.mesh.n_edge, "n_nodes": w.mesh.n_nodes,
-                       "p": w.params["p"], "rk_order": w.params["rk_order"], "dt": w.dt, "limiter": w.params["limiter"],
-                       "wetdry": w.params["wetdry"], "wind": w.holland is not None, "tide": w.tide is not None,
-                       "reorder": args.reorder, "stage_form": "element-centric stage kernel (no flux buffer)" if fused
-                       else "edge kernel + element kernel (flux buffer)", "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
-                       "l2": f"state {state_bytes / 1e6:.0f} MB per buffer + flux {w.mesh.n_edge * 3 * (w.params['p'] + 1) * 8 / 1e6:.0f} MB "
-                             "per stage exceed the 126 MB L2 (inputs larger than L2, no flush needed)"
-                             if state_bytes > 130e6 else "working set fits L2: a >L2 buffer is NOT flushed between steps; see DESIGN.md"},
+            "config": workload_config(w),
+            "run": {"reorder": args.reorder, "stage_form": "element-centric stage kernel (no flux buffer)" if fused
+                    else "edge kernel + element kernel (flux buffer)", "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                    "l2": f"state {state_bytes // 8 * rb / 1e6:.0f} MB per buffer exceeds the 126 MB L2 (inputs larger than L2, no flush needed)"
+                          if state_bytes // 8 * rb > 130e6 else "working set fits L2: a >L2 buffer is NOT flushed between steps; see DESIGN.md"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     g.close()
+
+
+def spawn_ranks(n: int) -> int:
+    """Re-run this command line under torch.distributed.run with n ranks on this node; returns its exit code."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), str(Path(__file__).resolve()), *sys.argv[1:]]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -452,6 +469,9 @@ def main():
     ap.add_argument("--decomp", type=int, default=0, help="domain decomposition instead of replicas: one partition per rank "
                     "(N > 1), or this many partitions on the one GPU (N = 1)")
     args = ap.parse_args()
+    if args.gpus > 1 and "RANK" not in os.environ:
+        # not under torchrun: spawn the N ranks ourselves (one process per GPU, rendezvous on 127.0.0.1) and hand over
+        raise SystemExit(spawn_ranks(args.gpus))
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -125,14 +125,17 @@ int dgswem_halo_unpack(dgswem_t*, int what, const double* buf, int buf_on_device
 /* TEST HOOK: L_h(current state) (eq. (5)) at the current time, each [ndof][n_elem]. */
 int dgswem_eval_rhs(dgswem_t*, double* rze, double* rqx, double* rqy);
 
-/* TEST HOOK: per-edge numerical flux buffer [3][nq_e][n_edge] of the last RHS evaluation
- * (caller's edge order; point j numbered along e+'s local edge). */
+/* TEST HOOK: per-edge numerical flux buffer [3][nq_e][n_edge] (caller's edge order; point j numbered along e+'s local
+ * edge; Alg. 2 l.25).  Edge + element form: the buffer of the last RHS evaluation.  Element-centric form (no
+ * buffer exists): EDGE is evaluated on the current state at the current time for this call.  Neither this call (in the
+ * element-centric form) nor dgswem_eval_rhs may be used between dgswem_begin_step and dgswem_end_step (E_ARG). */
 int dgswem_get_flux(dgswem_t*, double* flux);
 
-/* Copy the state (and time, if t != NULL) back; synchronises; E_NONFINITE if any value is not finite. */
+/* Copy the modal state of PAPER.md:193-195 (ZE, QX, QY[k, e]) back, and the time if t != NULL; synchronises;
+ * E_NONFINITE if any value is not finite (the arrays are still filled). */
 int dgswem_get_state(dgswem_t*, double* t, double* ze, double* qx, double* qy);
 
-/* Wet (1) / dry (0) flag per element, caller's order. */
+/* Wet (1) / dry (0) flag per element after the last WETDRY pass (R-8), caller's order; synchronises. */
 int dgswem_get_wetdry(dgswem_t*, uint8_t* wet);
 
 /* Nodal output ("we convert the modal representation to a nodal representation by averaging the
@@ -176,10 +179,11 @@ int64_t dgswem_launch_count(const dgswem_t*);
 int dgswem_profile(dgswem_t*, int enable);
 int dgswem_profile_read(dgswem_t*, double* ms, int64_t* count);
 
-/* Block until all enqueued work is done. */
+/* Block until all enqueued work is done (the paper's `!$acc wait`). */
 int dgswem_sync(dgswem_t*);
 
 const char* dgswem_last_error(const dgswem_t*);   /* valid until the next call on the handle; NULL handle: creation error */
+/* Release the handle and every device buffer it owns (the library owns all device memory); NULL is a no-op. */
 void dgswem_destroy(dgswem_t*);
 
 #ifdef __cplusplus

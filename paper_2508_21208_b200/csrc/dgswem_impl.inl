@@ -238,7 +238,11 @@ constexpr size_t kMaxProfRecords = 1 << 15;
 static inline void prof_begin(Handle* h, int kind) {
   if (!h->profiling || h->prof.size() >= kMaxProfRecords) return;
   Handle::ProfRec r; r.kind = kind; r.a = nullptr; r.b = nullptr;
-  if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) return;
+  if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) {
+    if (r.a) cudaEventDestroy(r.a);
+    (void)cudaGetLastError();   // a failed profiling event must not surface as the next launch's error
+    return;
+  }
   cudaEventRecord(r.a, h->stream);
   h->prof.push_back(r);
   h->prof_start = r.a;
@@ -303,8 +307,8 @@ int validate_mesh(Handle* h, long long nn, const double* xy, long long ne, const
 template <typename K>
 int resident_ctas(K kernel, int threads, size_t smem, int device) {
   int per_sm = 0, sms = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess) return 0;
-  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess) { (void)cudaGetLastError(); return 0; }
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) { (void)cudaGetLastError(); return 0; }
   return per_sm * sms;
 }
 
@@ -557,12 +561,20 @@ int run_steps(Handle* h, long long nsteps, double dt) {
   const bool need_tab = tide_on || h->wind_on;
   if (h->graph_one.exec && (h->graph_dt != dt || h->graph_wind != h->wind_on || h->graph_tide != tide_on)) drop_graphs(h);
   constexpr long long kScalRows = 4096;   // steps per table upload (256 KiB); longer calls go in chunks
-  if (need_tab && !h->scal_tab) {
-    h->scal_tab = (double*)h->dalloc((size_t)kScalRows * kScalStride * sizeof(double));
-    if (!h->scal_tab) return h->fail(DGSWEM_E_CUDA, "device allocation failed");
-    CK(cudaMallocHost((void**)&h->scal_host, (size_t)kScalRows * kScalStride * sizeof(double)));
-    CK(cudaEventCreateWithFlags(&h->scal_ev, cudaEventDisableTiming));
-    h->scal_cap = kScalRows;
+  if (need_tab && h->scal_cap == 0) {
+    // all three resources first, then published together: a failure leaves the handle as it was (scal_cap == 0)
+    double* tab = (double*)h->dalloc((size_t)kScalRows * kScalStride * sizeof(double));
+    if (!tab) return h->fail(DGSWEM_E_CUDA, "device allocation failed");
+    double* host = nullptr;
+    cudaEvent_t ev = nullptr;
+    cudaError_t e = cudaMallocHost((void**)&host, (size_t)kScalRows * kScalStride * sizeof(double));
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+      if (host) cudaFreeHost(host);
+      h->dfree(tab);
+      return h->cuda_fail(e, "scalar table setup");
+    }
+    h->scal_tab = tab; h->scal_host = host; h->scal_ev = ev; h->scal_cap = kScalRows;
   }
   const int many = h->ne < 65536 ? 8 : (h->ne < 1000000 ? 2 : 1);
   if (!h->graph_one.exec) {
@@ -609,7 +621,9 @@ int run_steps(Handle* h, long long nsteps, double dt) {
 
 void api_destroy(Handle* h) {
   if (!h) return;
-  cudaSetDevice(h->prm.device);
+  // (a handle whose creation failed before a device was chosen owns nothing on any device: its ordinal may be the
+  // rejected one and must not be made current)
+  if (h->stream || !h->allocs.empty()) cudaSetDevice(h->prm.device);
   if (h->stream) cudaStreamSynchronize(h->stream);
   for (auto& r : h->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   h->prof.clear();
@@ -620,6 +634,7 @@ void api_destroy(Handle* h) {
   h->release_all();
   if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
   delete h;
+  (void)cudaGetLastError();   // nothing ignored above may stay pending for the next launch check of another handle
 }
 
 int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* hooks, int64_t n_nodes,
@@ -1067,6 +1082,7 @@ int api_halo_unpack(Handle* h, int what, const double* buf, int buf_on_device) {
 int api_eval_rhs(Handle* h, double* rze, double* rqx, double* rqy) {
   if (!h) return DGSWEM_E_ARG;
   if (!rze || !rqx || !rqy) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
+  if (h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a stage-granular step is in progress: its stage buffer is the scratch of dgswem_eval_rhs");
   CK(cudaSetDevice(h->prm.device));
   int rc;
   if (h->wind_on && (rc = launch_wind(h, h->t))) return rc;
@@ -1097,6 +1113,7 @@ int api_eval_rhs(Handle* h, double* rze, double* rqx, double* rqy) {
 int api_get_flux(Handle* h, double* flux) {
   if (!h) return DGSWEM_E_ARG;
   if (!flux) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
+  if (h->fused && h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a stage-granular step is in progress");
   CK(cudaSetDevice(h->prm.device));
   if (h->fused) {   // the element-centric stage kernel keeps no flux buffer: evaluate A1 on the current state
     int rc = h->prm.p == 1 ? launch_edge<1>(h, h->W[0], scal(h, 0, tide_value(h, h->t))) : launch_edge<2>(h, h->W[0], scal(h, 0, tide_value(h, h->t)));

@@ -59,3 +59,28 @@ def test_reference_arm_rank0_only():
     assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
     assert line["config"]["workload"].startswith("C1")
+
+
+def test_bench_spawns_its_own_ranks_when_not_under_torchrun():
+    """`python bench.py --gpus 2` with no torchrun environment re-executes itself under torch.distributed.run with two
+    ranks (rendezvous on 127.0.0.1) and the line says n_gpus = 2 (it used to run one replica and say 1).
+    Checked here with the reference arm, which needs no GPU; the GPU arm takes the same path."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "2", "--warmup", "1",
+                        "--workload", "C1"], capture_output=True, text=True, env=env, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                                       # rank 0 alone prints
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["impl"] == "reference"
+
+
+def test_both_arms_name_the_workload_with_the_same_config_keys():
+    """The driver compares the two arms' `config` dicts: both come from bench.workload_config."""
+    sys.path.insert(0, str(ROOT))
+    import bench
+    w = bench.make_workload("C1")
+    cfg = bench.workload_config(w)
+    assert set(cfg) == {"workload", "n_elem", "n_edge", "n_nodes", "p", "rk_order", "dt", "limiter", "wetdry", "flux", "wind", "tide"}
+    src = (ROOT / "bench.py").read_text()
+    assert src.count('"config": workload_config(w)') + src.count('"config": cfg') >= 2
