@@ -164,6 +164,11 @@ struct Handle : ::dgswem {
   int *einfo = nullptr, *elem_edge = nullptr, *nbr = nullptr, *tri = nullptr, *nbinfo = nullptr;
   real* enl = nullptr;
   bool fused = false;         // element-centric stage kernel (k_stage) instead of k_edge + k_elem
+  bool tiled = false;         // ... in its shared-memory edge-tile form (k_stage_tile): each tile evaluates its unique edges once
+  int2* tile_info = nullptr;
+  unsigned char* it_blob = nullptr;
+  int *it_nb = nullptr, *eslot = nullptr;
+  int tile_cap = 0, tile_cap1 = 0, res_tile[2] = {0, 0};   // resident grid of k_stage_tile without / with the wind block
   int *node_ptr = nullptr, *node_ev = nullptr;   // node -> (internal element * 4 + vertex), ascending caller element id
   int *perm_e = nullptr, *inv_e = nullptr, *inv_d = nullptr;   // perm_e[new]=old, inv_e[old]=new, inv_d[old]=new
   unsigned char *wet = nullptr, *wet_stage = nullptr;
@@ -383,6 +388,35 @@ int launch_elem(Handle* h, const real* win, const real* w0, real* wout, double d
   return 0;
 }
 
+// the instantiation of k_stage_tile for (flux, stage variant): specialised like k_stage for p = 1 / LLF, generic otherwise
+using TileKernel = void (*)(const ElemArgs, const int);
+template <int P, int MODE>
+TileKernel tile_kernel(int flux, int variant) {
+  if (flux == 1) return k_stage_tile<P, MODE, -1, 1>;
+  if constexpr (P == 1 && MODE == MODE_UPDATE) {
+    switch (variant) {
+      case 0: return k_stage_tile<P, MODE, 0>;
+      case 1: return k_stage_tile<P, MODE, 1>;
+      case 2: return k_stage_tile<P, MODE, 2>;
+      case 3: return k_stage_tile<P, MODE, 3>;
+      case 6: return k_stage_tile<P, MODE, 6>;
+      case 7: return k_stage_tile<P, MODE, 7>;
+      default: break;
+    }
+  }
+  return k_stage_tile<P, MODE, -1>;
+}
+// (the attribute belongs to the function, not to the handle: always the largest tile possible, 3 x 128 items)
+template <int P>
+int tile_kernel_attrs(Handle* h, int smem) {
+  for (int flux = 0; flux < 2; ++flux)
+    for (int v = -1; v < 8; ++v) {
+      CK(cudaFuncSetAttribute(tile_kernel<P, MODE_UPDATE>(flux, v), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+      CK(cudaFuncSetAttribute(tile_kernel<P, MODE_RHS>(flux, v), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    }
+  return 0;
+}
+
 // A1-A5 (+A7) in one launch (element-centric form, no flux buffer)
 template <int P, int MODE>
 int launch_stage(Handle* h, const real* win, const real* w0, real* wout, double dt, real a, real b,
@@ -398,6 +432,19 @@ int launch_stage(Handle* h, const real* win, const real* w0, real* wout, double 
   A.dt = (real)dt; A.a = a; A.b = b; A.first_stage = first; A.wind = h->wind_on ? 1 : 0; A.fuse_wetdry = fuse_wd ? 1 : 0;
   // (persistent forms were measured slower on C3: next-tile neighbour-table prefetch 425 us, per-warp cp.async
   // staging of the next tile's rows in shared memory 445 us, against 374 us)
+  if (h->tiled) {           // shared-memory edge-tile form: one CTA per tile of 128 elements
+    A.tile_info = h->tile_info; A.it_blob = h->it_blob; A.it_nb = h->it_nb; A.eslot = h->eslot;
+    A.cap = h->tile_cap; A.cap1 = h->tile_cap1;
+    const int ntiles = grid_for(h->ne, kTile);
+    const int res = h->res_tile[h->wind_on ? 1 : 0];
+    const int grid = std::max(1, std::min(ntiles, res > 0 ? res : ntiles));
+    prof_begin(h, PK_ELEM);
+    tile_kernel<P, MODE>(h->prm.flux, MODE == MODE_UPDATE ? stage_variant(h, first) : -1)
+        <<<grid, kTile, StageTile<P>::smem(h->tile_cap, h->tile_cap1, h->wind_on), h->stream>>>(A, ntiles);
+    prof_end(h);
+    CKL("k_stage_tile");
+    return 0;
+  }
   prof_begin(h, PK_ELEM);
   const int grid = grid_for(h->ne, DGK_STAGE_THREADS);
   if (h->prm.flux == 1) {   // Roe: the generic-flag kernel only
@@ -709,7 +756,8 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
 
     // DGSWEM_FUSED=1/0: element-centric stage kernel (no flux buffer) on/off; default: on for p = 1
     h->fused = prm->p == 1;
-    if (const char* env = std::getenv("DGSWEM_FUSED")) h->fused = std::atoi(env) != 0;
+    h->tiled = false;
+    if (const char* env = std::getenv("DGSWEM_FUSED")) { h->fused = std::atoi(env) != 0; h->tiled = std::atoi(env) == 2; }
 
     const long long ne = h->ne, nd = h->nd, nn = h->nn, ld = h->ld, ldd = h->ldd, ldn = h->ldn;
     // ---- renumbering (internal only): perm_e[new] = old
@@ -788,6 +836,66 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
         enl[tix(6, 2 * l + 1, i)] = plus ? ny : -ny;
       }
     }
+    // ---- shared-memory edge-tile form: per tile of 128 elements the list of its unique edges ("items").  An edge whose
+    // two elements sit in the same tile is listed once, under the element with the lower index (side a; the other
+    // element reads the slot negated, in reversed point order); an edge to another tile or to the boundary is listed
+    // under its element of this tile.  Items are in (a, la) order; every tile's list starts at a multiple of 32.
+    const long long ntiles = ld / kTile;
+    std::vector<int2> tile_info(ntiles, make_int2(0, 0));
+    std::vector<unsigned char> it_blob;
+    std::vector<int> it_nb, eslot(ld, 0);
+    int tile_cap = 8, tile_cap1 = 8;
+    if (h->tiled) {
+      struct Item { int rec, nb; real nx, ny; };
+      std::vector<Item> items; items.reserve((size_t)(1.8 * ne) + 64);
+      std::vector<long long> first(ntiles + 1, 0);
+      for (long long t = 0; t < ntiles; ++t) {
+        int cnt = 0, n1 = 0;
+        // items to other tiles first (their neighbour rows are prefetched into slots 0 .. n1-1), then the rest
+        for (int pass = 0; pass < 2; ++pass) {
+          for (long long i = t * kTile; i < std::min<long long>((t + 1) * kTile, ne); ++i) {
+            for (int l = 0; l < 3; ++l) {
+              const int nbi = nbinfo[tix(3, l, i)];
+              const bool bnd = nbi < 0;
+              const long long nb = bnd ? -1 : (nbi & 0x1fffffff);
+              const int lo = bnd ? 0 : ((nbi >> 29) & 3);
+              const bool in_tile = !bnd && (nb / kTile) == t;
+              if (in_tile && nb < i) continue;   // listed under the lower element
+              const int kind = bnd ? ((nbi & 3) == 2 ? 3 : 2) : (in_tile ? 0 : 1);
+              if ((kind == 1) != (pass == 0)) continue;
+              const int a = (int)(i - t * kTile), b = in_tile ? (int)(nb - t * kTile) : 0;
+              items.push_back(Item{a | (l << 7) | (kind << 9) | (b << 11) | (lo << 18), kind == 1 ? (int)nb : 0,
+                                   enl[tix(6, 2 * l, i)], enl[tix(6, 2 * l + 1, i)]});
+              eslot[i] |= cnt << (10 * l);
+              if (in_tile) eslot[nb] |= (cnt | 512) << (10 * lo);
+              ++cnt;
+            }
+          }
+          if (pass == 0) n1 = cnt;
+        }
+        tile_info[t] = make_int2(cnt, n1);
+        first[t + 1] = first[t] + cnt;
+        tile_cap = std::max(tile_cap, (cnt + 7) / 8 * 8);
+        tile_cap1 = std::max(tile_cap1, (n1 + 7) / 8 * 8);
+      }
+      // fixed-size blocks per tile, so that one bulk copy of known size moves each
+      const size_t ib = (size_t)(4 + 2 * sizeof(real)) * tile_cap;
+      it_blob.assign(ib * ntiles, 0);
+      it_nb.assign((size_t)tile_cap1 * ntiles, 0);
+      for (long long t = 0; t < ntiles; ++t) {
+        int* rec = reinterpret_cast<int*>(it_blob.data() + ib * t);
+        real* nrm = reinterpret_cast<real*>(it_blob.data() + ib * t + 4 * (size_t)tile_cap);
+        for (long long k = first[t]; k < first[t + 1]; ++k) {
+          const long long i = k - first[t];
+          rec[i] = items[k].rec; nrm[i] = items[k].nx; nrm[tile_cap + i] = items[k].ny;
+          if (i < tile_info[t].y) it_nb[(size_t)tile_cap1 * t + i] = items[k].nb;
+        }
+      }
+      h->tile_cap = tile_cap; h->tile_cap1 = tile_cap1;
+      if (std::getenv("DGSWEM_TILE_STATS"))
+        std::fprintf(stderr, "dgswem tile stats: %lld tiles, items/tile mean %.1f max-cap %d, to other tiles mean %.1f max-cap %d\n", ntiles,
+                     (double)first[ntiles] / ntiles, tile_cap, [&] { double s1 = 0; for (auto& q : tile_info) s1 += q.y; return s1 / ntiles; }(), tile_cap1);
+    }
     // ---- edge geometry in internal order, from the e+ side
     std::vector<int2> ee(ldd, make_int2(0, -1));
     std::vector<int> einfo(ldd, 1 << 4);
@@ -826,6 +934,19 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
     if ((r = upload(h, h->nbr, nbr))) return r;
     if ((r = upload(h, h->nbinfo, nbinfo))) return r;
     if ((r = upload(h, h->enl, enl))) return r;
+    if (h->tiled) {
+      if ((r = prm->p == 1 ? tile_kernel_attrs<1>(h, (int)StageTile<1>::smem(3 * kTile, 3 * kTile, true)) : tile_kernel_attrs<2>(h, (int)StageTile<2>::smem(3 * kTile, 3 * kTile, true)))) return r;
+      for (int wnd = 0; wnd < 2; ++wnd) {   // resident grid of the persistent kernel at this handle's shared-memory size
+        const size_t sm = prm->p == 1 ? StageTile<1>::smem(tile_cap, tile_cap1, wnd != 0) : StageTile<2>::smem(tile_cap, tile_cap1, wnd != 0);
+        h->res_tile[wnd] = prm->p == 1 ? resident_ctas(tile_kernel<1, MODE_UPDATE>(prm->flux, wnd ? 2 : 0), kTile, sm, prm->device)
+                                       : resident_ctas(tile_kernel<2, MODE_UPDATE>(prm->flux, -1), kTile, sm, prm->device);
+        if (const char* env = std::getenv("DGSWEM_PERSISTENT_CTAS")) { const int c = std::atoi(env); if (c > 0) h->res_tile[wnd] = std::min(h->res_tile[wnd], c); }
+      }
+      if ((r = upload(h, h->tile_info, tile_info))) return r;
+      if ((r = upload(h, h->it_blob, it_blob))) return r;
+      if ((r = upload(h, h->it_nb, it_nb))) return r;
+      if ((r = upload(h, h->eslot, eslot))) return r;
+    }
     if ((r = upload(h, h->tri, trin))) return r;
     if ((r = upload(h, h->edge_elem, ee))) return r;
     if ((r = upload(h, h->einfo, einfo))) return r;
@@ -1250,7 +1371,7 @@ int api_fp64_peak(Handle* h, double* dfma_per_s) {
   return DGSWEM_OK;
 }
 
-int api_stage_form(const Handle* h) { return (h && h->fused) ? 1 : 0; }
+int api_stage_form(const Handle* h) { return (h && h->fused) ? (h->tiled ? 2 : 1) : 0; }
 
 int64_t api_launch_count(const Handle* h) { return h ? h->launches : 0; }
 
