@@ -435,7 +435,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             "ms_per_step": ms / args.steps, "ms_per_step_with_per_launch_events": ms_prof / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
             "data": "synthetic",
             "config": workload_config(w),
-            "run": {"reorder": args.reorder, "stage_form": ("element-centric stage kernel, shared-memory edge tile (no flux buffer)" if g.stage_form() == 2 else "element-centric stage kernel (no flux buffer)") if fused
+            "run": {"reorder": args.reorder, "stage_form": ("element-centric stage kernel, TMA-staged operands (no flux buffer)" if g.stage_form() == 3 else "element-centric stage kernel, shared-memory edge tile (no flux buffer)" if g.stage_form() == 2 else "element-centric stage kernel (no flux buffer)") if fused
                     else "edge kernel + element kernel (flux buffer)", "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                     "l2": f"state {state_bytes // 8 * rb / 1e6:.0f} MB per buffer exceeds the 126 MB L2 (inputs larger than L2, no flush needed)"
                           if state_bytes // 8 * rb > 130e6 else "working set fits L2: a >L2 buffer is NOT flushed between steps; see DESIGN.md"},

@@ -16,7 +16,7 @@ SRC = PKG / "csrc" / "dgswem.cu"
 DEPS = [SRC, PKG / "csrc" / "dgswem_kernels.cuh", PKG / "csrc" / "dgswem_impl.inl", ROOT / "include" / "dgswem.h"]
 LIB = PKG / "libdgswem.so"
 
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false",
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false", "-split-compile", "0",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-O2", "-shared"]
 
 

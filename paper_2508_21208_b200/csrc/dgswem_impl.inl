@@ -165,6 +165,10 @@ struct Handle : ::dgswem {
   real* enl = nullptr;
   bool fused = false;         // element-centric stage kernel (k_stage) instead of k_edge + k_elem
   bool tiled = false;         // ... in its shared-memory edge-tile form (k_stage_tile): each tile evaluates its unique edges once
+  bool staged = false;        // ... with TMA-staged operands (k_stage_stg)
+  int *nbs = nullptr, *stg_nb = nullptr;
+  int2* stg_info = nullptr;
+  int stg_cap1 = 0, res_stg[2] = {0, 0};
   int2* tile_info = nullptr;
   unsigned char* it_blob = nullptr;
   int *it_nb = nullptr, *eslot = nullptr;
@@ -417,6 +421,33 @@ int tile_kernel_attrs(Handle* h, int smem) {
   return 0;
 }
 
+// the same for k_stage_stg
+template <int P, int MODE>
+TileKernel stg_kernel(int flux, int variant) {
+  if (flux == 1) return k_stage_stg<P, MODE, -1, 1>;
+  if constexpr (P == 1 && MODE == MODE_UPDATE) {
+    switch (variant) {
+      case 0: return k_stage_stg<P, MODE, 0>;
+      case 1: return k_stage_stg<P, MODE, 1>;
+      case 2: return k_stage_stg<P, MODE, 2>;
+      case 3: return k_stage_stg<P, MODE, 3>;
+      case 6: return k_stage_stg<P, MODE, 6>;
+      case 7: return k_stage_stg<P, MODE, 7>;
+      default: break;
+    }
+  }
+  return k_stage_stg<P, MODE, -1>;
+}
+template <int P>
+int stg_kernel_attrs(Handle* h, int smem) {
+  for (int flux = 0; flux < 2; ++flux)
+    for (int v = -1; v < 8; ++v) {
+      CK(cudaFuncSetAttribute(stg_kernel<P, MODE_UPDATE>(flux, v), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+      CK(cudaFuncSetAttribute(stg_kernel<P, MODE_RHS>(flux, v), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    }
+  return 0;
+}
+
 // A1-A5 (+A7) in one launch (element-centric form, no flux buffer)
 template <int P, int MODE>
 int launch_stage(Handle* h, const real* win, const real* w0, real* wout, double dt, real a, real b,
@@ -432,6 +463,18 @@ int launch_stage(Handle* h, const real* win, const real* w0, real* wout, double 
   A.dt = (real)dt; A.a = a; A.b = b; A.first_stage = first; A.wind = h->wind_on ? 1 : 0; A.fuse_wetdry = fuse_wd ? 1 : 0;
   // (persistent forms were measured slower on C3: next-tile neighbour-table prefetch 425 us, per-warp cp.async
   // staging of the next tile's rows in shared memory 445 us, against 374 us)
+  if (h->staged) {          // TMA-staged operands, persistent CTAs
+    A.tile_info = h->stg_info; A.it_nb = h->stg_nb; A.nbs = h->nbs; A.cap1 = h->stg_cap1; A.cap = 0;
+    const int ntiles = grid_for(h->ne, kTile);
+    const int res = h->res_stg[h->wind_on ? 1 : 0];
+    const int grid = std::max(1, std::min(ntiles, res > 0 ? res : ntiles));
+    prof_begin(h, PK_ELEM);
+    stg_kernel<P, MODE>(h->prm.flux, MODE == MODE_UPDATE ? stage_variant(h, first) : -1)
+        <<<grid, kTile, StageStg<P>::smem(h->stg_cap1, h->wind_on), h->stream>>>(A, ntiles);
+    prof_end(h);
+    CKL("k_stage_stg");
+    return 0;
+  }
   if (h->tiled) {           // shared-memory edge-tile form: one CTA per tile of 128 elements
     A.tile_info = h->tile_info; A.it_blob = h->it_blob; A.it_nb = h->it_nb; A.eslot = h->eslot;
     A.cap = h->tile_cap; A.cap1 = h->tile_cap1;
@@ -757,7 +800,7 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
     // DGSWEM_FUSED=1/0: element-centric stage kernel (no flux buffer) on/off; default: on for p = 1
     h->fused = prm->p == 1;
     h->tiled = false;
-    if (const char* env = std::getenv("DGSWEM_FUSED")) { h->fused = std::atoi(env) != 0; h->tiled = std::atoi(env) == 2; }
+    if (const char* env = std::getenv("DGSWEM_FUSED")) { h->fused = std::atoi(env) != 0; h->tiled = std::atoi(env) == 2; h->staged = std::atoi(env) == 3; }
 
     const long long ne = h->ne, nd = h->nd, nn = h->nn, ld = h->ld, ldd = h->ldd, ldn = h->ldn;
     // ---- renumbering (internal only): perm_e[new] = old
@@ -896,6 +939,43 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
         std::fprintf(stderr, "dgswem tile stats: %lld tiles, items/tile mean %.1f max-cap %d, to other tiles mean %.1f max-cap %d\n", ntiles,
                      (double)first[ntiles] / ntiles, tile_cap, [&] { double s1 = 0; for (auto& q : tile_info) s1 += q.y; return s1 / ntiles; }(), tile_cap1);
     }
+    // ---- TMA-staged element-centric form: per tile the (deduplicated) list of neighbours in other tiles, and per
+    // (element, local edge) the column of the neighbour's modes in the staged rows: its index in the tile, or 128 + its
+    // position in that list; | neighbour's local edge << 9; boundary: bit 31 | code
+    std::vector<int> nbs(3 * ld, (int)0x80000001), stg_nb;
+    std::vector<int2> stg_info(ntiles, make_int2(0, 0));
+    int stg_cap1 = 8;
+    if (h->staged) {
+      std::vector<std::vector<int>> lists(ntiles);
+      for (long long t = 0; t < ntiles; ++t) {
+        std::vector<int>& L = lists[t];
+        for (long long i = t * kTile; i < std::min<long long>((t + 1) * kTile, ne); ++i) {
+          for (int l = 0; l < 3; ++l) {
+            const int nbi = nbinfo[tix(3, l, i)];
+            if (nbi < 0) { nbs[tix(3, l, i)] = nbi; continue; }
+            const long long nb = nbi & 0x1fffffff;
+            const int lo = (nbi >> 29) & 3;
+            int col;
+            if (nb / kTile == t) {
+              col = (int)(nb - t * kTile);
+            } else {
+              auto itf = std::find(L.begin(), L.end(), (int)nb);
+              if (itf == L.end()) { L.push_back((int)nb); col = kTile + (int)L.size() - 1; } else col = kTile + (int)(itf - L.begin());
+            }
+            nbs[tix(3, l, i)] = col | (lo << 9);
+          }
+        }
+        stg_info[t] = make_int2(0, (int)L.size());
+        stg_cap1 = std::max(stg_cap1, ((int)L.size() + 7) / 8 * 8);
+      }
+      stg_nb.assign((size_t)stg_cap1 * ntiles, 0);
+      for (long long t = 0; t < ntiles; ++t) std::copy(lists[t].begin(), lists[t].end(), stg_nb.begin() + (size_t)stg_cap1 * t);
+      h->stg_cap1 = stg_cap1;
+      if (std::getenv("DGSWEM_TILE_STATS")) {
+        double s1 = 0; for (auto& q : stg_info) s1 += q.y;
+        std::fprintf(stderr, "dgswem staged form: %lld tiles, neighbours in other tiles mean %.1f cap %d\n", ntiles, s1 / ntiles, stg_cap1);
+      }
+    }
     // ---- edge geometry in internal order, from the e+ side
     std::vector<int2> ee(ldd, make_int2(0, -1));
     std::vector<int> einfo(ldd, 1 << 4);
@@ -934,6 +1014,18 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
     if ((r = upload(h, h->nbr, nbr))) return r;
     if ((r = upload(h, h->nbinfo, nbinfo))) return r;
     if ((r = upload(h, h->enl, enl))) return r;
+    if (h->staged) {
+      if ((r = prm->p == 1 ? stg_kernel_attrs<1>(h, (int)StageStg<1>::smem(3 * kTile, true)) : stg_kernel_attrs<2>(h, (int)StageStg<2>::smem(3 * kTile, true)))) return r;
+      for (int wnd = 0; wnd < 2; ++wnd) {
+        const size_t sm = prm->p == 1 ? StageStg<1>::smem(stg_cap1, wnd != 0) : StageStg<2>::smem(stg_cap1, wnd != 0);
+        h->res_stg[wnd] = prm->p == 1 ? resident_ctas(stg_kernel<1, MODE_UPDATE>(prm->flux, wnd ? 2 : 0), kTile, sm, prm->device)
+                                      : resident_ctas(stg_kernel<2, MODE_UPDATE>(prm->flux, -1), kTile, sm, prm->device);
+        if (const char* env = std::getenv("DGSWEM_PERSISTENT_CTAS")) { const int c = std::atoi(env); if (c > 0) h->res_stg[wnd] = std::min(h->res_stg[wnd], c); }
+      }
+      if ((r = upload(h, h->nbs, nbs))) return r;
+      if ((r = upload(h, h->stg_nb, stg_nb))) return r;
+      if ((r = upload(h, h->stg_info, stg_info))) return r;
+    }
     if (h->tiled) {
       if ((r = prm->p == 1 ? tile_kernel_attrs<1>(h, (int)StageTile<1>::smem(3 * kTile, 3 * kTile, true)) : tile_kernel_attrs<2>(h, (int)StageTile<2>::smem(3 * kTile, 3 * kTile, true)))) return r;
       for (int wnd = 0; wnd < 2; ++wnd) {   // resident grid of the persistent kernel at this handle's shared-memory size
@@ -1371,7 +1463,7 @@ int api_fp64_peak(Handle* h, double* dfma_per_s) {
   return DGSWEM_OK;
 }
 
-int api_stage_form(const Handle* h) { return (h && h->fused) ? (h->tiled ? 2 : 1) : 0; }
+int api_stage_form(const Handle* h) { return (h && h->fused) ? (h->staged ? 3 : h->tiled ? 2 : 1) : 0; }
 
 int64_t api_launch_count(const Handle* h) { return h ? h->launches : 0; }
 

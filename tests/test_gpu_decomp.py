@@ -31,7 +31,7 @@ CASES = {
 }
 
 
-@pytest.mark.parametrize("fused", ["0", "1", "2"], ids=["edge+elem", "stage", "stage-tile"])
+@pytest.mark.parametrize("fused", ["0", "1", "2", "3"], ids=["edge+elem", "stage", "stage-tile", "stage-staged"])
 @pytest.mark.parametrize("n_parts", [2, 5])
 @pytest.mark.parametrize("case", sorted(CASES))
 def test_partitioned_run_equals_undivided_run(O, G, monkeypatch, case, n_parts, fused):

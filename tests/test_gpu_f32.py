@@ -32,7 +32,7 @@ def O32():
     return oracle32
 
 
-@pytest.fixture(autouse=True, params=["0", "1", "2"], ids=["edge+elem", "stage", "stage-tile"])
+@pytest.fixture(autouse=True, params=["0", "1", "2", "3"], ids=["edge+elem", "stage", "stage-tile", "stage-staged"])
 def kernel_path(request, monkeypatch):
     monkeypatch.setenv("DGSWEM_FUSED", request.param)
     return request.param
