@@ -493,35 +493,66 @@ int orc_wetdry_elem(const orc_tables* T, real h0, const real* hv, real* ze, real
 }
 
 /* ----------------------------------------------------------------- SSP-RK */
-/* Shu-Osher SSP(2,2) / SSP(3,3) [R-2] ("optimized SSPRK" whose coefficients the
- * paper does not print; BASELINE configs name SSP-RK2 / RK3).
- *   stage s: u = w^(s-1) + dt L(w^(s-1), t + c_s dt);  w^(s) = u (s=1) or a_s w^0 + b_s u. */
-static const real RK2_A[2] = {RL(0.0), RL(0.5)}, RK2_B[2] = {RL(1.0), RL(0.5)}, RK2_C[2] = {RL(0.0), RL(1.0)};
-static const real RK3_A[3] = {RL(0.0), RL(0.75), RL(1.0) / RL(3.0)}, RK3_B[3] = {RL(1.0), RL(0.25), RL(2.0) / RL(3.0)}, RK3_C[3] = {RL(0.0), RL(1.0), RL(0.5)};
+/* Two-register Shu-Osher SSP Runge-Kutta schemes [R-2, R-19] ("an optimized version of the ... SSPRK"
+ * whose coefficients the paper does not print; BASELINE configs name SSP-RK2 / RK3).  Every stage has the form
+ *   u = w^(s-1) + (beta_s dt) L(w^(s-1), t + c_s dt);   w^(s) = u  (a_s = 0, b_s = 1)  or  a_s w^0 + b_s u.
+ * (order, stages):
+ *   (2,2)  SSP(2,2):  beta = 1;    w2 = 1/2 w0 + 1/2 u;                  c = (0, 1)
+ *   (3,3)  SSP(3,3):  beta = 1;    w2 = 3/4 w0 + 1/4 u; w3 = 1/3 w0 + 2/3 u;  c = (0, 1, 1/2)
+ *   (2,s)  optimal s-stage second-order scheme, s = 3, 4:  beta = 1/(s-1);  w_s = 1/s w0 + (s-1)/s u;  c_i = (i-1)/(s-1)
+ *   (3,4)  optimal 4-stage third-order scheme:  beta = 1/2;  w3 = 2/3 w0 + 1/3 u;  c = (0, 1/2, 1, 1/2)
+ * The many-stage schemes trade one more L evaluation for a time step (s-1) x (second order) or 2 x (third order) as large. */
+typedef struct { int ns; real a[4], b[4]; double beta[4], c[4]; } rk_scheme;
+static int rk_get(int order, int stages, rk_scheme* k) {
+  if (stages == 0) stages = order;
+  memset(k, 0, sizeof(*k));
+  k->ns = stages;
+  for (int s = 0; s < 4; ++s) { k->a[s] = RL(0.0); k->b[s] = RL(1.0); k->beta[s] = 1.0; k->c[s] = 0.0; }
+  if (order == 2 && stages == 2) {
+    k->a[1] = RL(0.5); k->b[1] = RL(0.5); k->c[1] = 1.0;
+  } else if (order == 3 && stages == 3) {
+    k->a[1] = RL(0.75); k->b[1] = RL(0.25); k->c[1] = 1.0;
+    k->a[2] = RL(1.0) / RL(3.0); k->b[2] = RL(2.0) / RL(3.0); k->c[2] = 0.5;
+  } else if (order == 2 && (stages == 3 || stages == 4)) {
+    for (int s = 0; s < stages; ++s) { k->beta[s] = 1.0 / (double)(stages - 1); k->c[s] = (double)s / (double)(stages - 1); }
+    k->a[stages - 1] = RL(1.0) / (real)stages; k->b[stages - 1] = (real)(stages - 1) / (real)stages;
+  } else if (order == 3 && stages == 4) {
+    for (int s = 0; s < 4; ++s) k->beta[s] = 0.5;
+    k->c[1] = 0.5; k->c[2] = 1.0; k->c[3] = 0.5;
+    k->a[2] = RL(2.0) / RL(3.0); k->b[2] = RL(1.0) / RL(3.0);
+  } else {
+    return -1;
+  }
+  return 0;
+}
 
-int orc_ssprk_step(int order, int64_t n, real* w, real* w0, real* rhs, double t, double dt,
-                   orc_rhs_fn rhs_fn, orc_post_fn post_fn, void* ctx) {
-  const real *A, *B, *C;
-  if (order == 2) { A = RK2_A; B = RK2_B; C = RK2_C; }
-  else if (order == 3) { A = RK3_A; B = RK3_B; C = RK3_C; }
-  else return -1;
+int orc_ssprk_step_s(int order, int stages, int64_t n, real* w, real* w0, real* rhs, double t, double dt,
+                     orc_rhs_fn rhs_fn, orc_post_fn post_fn, void* ctx) {
+  rk_scheme K;
+  if (rk_get(order, stages, &K) != 0) return -1;
   memcpy(w0, w, (size_t)n * sizeof(real));
-  for (int s = 0; s < order; ++s) {
-    rhs_fn(ctx, s, t + C[s] * dt, w, rhs);
-    if (s == 0) {
+  for (int s = 0; s < K.ns; ++s) {
+    rhs_fn(ctx, s, t + K.c[s] * dt, w, rhs);
+    const double dts = K.beta[s] * dt;          /* binary64 like t and dt; rounded once where it meets the state */
+    const real a = K.a[s], b = K.b[s];
+    if (a == RL(0.0) && b == RL(1.0)) {         /* plain stage: no combine (bitwise: not u + 0 w0) */
 #pragma omp parallel for schedule(static)
-      for (int64_t i = 0; i < n; ++i) w[i] = fma(dt, rhs[i], w[i]);
+      for (int64_t i = 0; i < n; ++i) w[i] = fma(dts, rhs[i], w[i]);
     } else {
-      const real a = A[s], b = B[s];
 #pragma omp parallel for schedule(static)
       for (int64_t i = 0; i < n; ++i) {
-        real u = fma(dt, rhs[i], w[i]);
+        real u = fma(dts, rhs[i], w[i]);
         w[i] = fma(b, u, a * w0[i]);
       }
     }
     if (post_fn) post_fn(ctx, s, w);
   }
   return 0;
+}
+
+int orc_ssprk_step(int order, int64_t n, real* w, real* w0, real* rhs, double t, double dt,
+                   orc_rhs_fn rhs_fn, orc_post_fn post_fn, void* ctx) {
+  return orc_ssprk_step_s(order, 0, n, w, w0, rhs, t, dt, rhs_fn, post_fn, ctx);
 }
 
 /* ------------------------------------------------------------------ model */
@@ -560,6 +591,7 @@ orc_model* orc_create(const orc_params* prm, int64_t n_nodes, const real* xy, co
   orc_model* m = (orc_model*)calloc(1, sizeof(orc_model));
   m->prm = *prm;
   if (orc_make_tables(prm->p, &m->T) != 0) { free(m); return NULL; }
+  { rk_scheme K; if (rk_get(prm->rk_order, prm->rk_stages, &K) != 0) { free(m); return NULL; } }
   m->n_nodes = n_nodes; m->n_elem = n_elem; m->n_edge = n_edge;
   m->xy = NEW(real, 2 * n_nodes); memcpy(m->xy, xy, sizeof(real) * 2 * n_nodes);
   m->bathy = NEW(real, n_nodes); memcpy(m->bathy, bathy, sizeof(real) * n_nodes);
@@ -945,7 +977,7 @@ void orc_step(orc_model* m, int64_t nsteps, double dt) {
   const int64_t n = 3 * (int64_t)m->T.ndof * m->n_elem;
   for (int64_t s = 0; s < nsteps; ++s) {
     if (m->wind_on) wind_all(m, m->t);
-    orc_ssprk_step(m->prm.rk_order, n, m->w, m->w0, m->rhs, m->t, dt, dg_rhs, dg_post, m);
+    orc_ssprk_step_s(m->prm.rk_order, m->prm.rk_stages, n, m->w, m->w0, m->rhs, m->t, dt, dg_rhs, dg_post, m);
     m->t = m->t + dt;
   }
 }

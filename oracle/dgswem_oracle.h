@@ -43,6 +43,7 @@ typedef struct {
   int32_t limiter;    /* 0 off, 1 edge-neighbour Barth-Jespersen [R-7], 2 vertex-neighbourhood Barth-Jespersen [R-18] */
   int32_t wetdry;
   int32_t flux;       /* 0 local Lax-Friedrichs [R-3], 1 Roe [R-17] */
+  int32_t rk_stages;  /* 0: = rk_order (SSP(2,2) / SSP(3,3)); many-stage schemes [R-19]: (order 2: 3 or 4 stages), (order 3: 4 stages) */
 } orc_params;
 
 typedef struct { double x0, y0, vx, vy, rmax, dp, B, rho_air, rho_water, f; } orc_holland;   /* binary64 in every build */
@@ -90,6 +91,8 @@ int    orc_wetdry_elem(const orc_tables* T, real h0, const real* hv, real* ze, r
 /* generic SSP-RK step: w <- one step of size dt, with user RHS and post-stage hooks */
 typedef void (*orc_rhs_fn)(void* ctx, int stage, double t_stage, const real* w, real* rhs);
 typedef void (*orc_post_fn)(void* ctx, int stage, real* w);
+int    orc_ssprk_step_s(int order, int stages, int64_t n, real* w, real* w0, real* rhs, double t, double dt,
+                        orc_rhs_fn rhs_fn, orc_post_fn post_fn, void* ctx);
 int    orc_ssprk_step(int order, int64_t n, real* w, real* w0, real* rhs, double t, double dt,
                       orc_rhs_fn rhs_fn, orc_post_fn post_fn, void* ctx);
 

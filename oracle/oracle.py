@@ -47,7 +47,7 @@ def build(force: bool = False) -> Path:
 class Params(C.Structure):
     _fields_ = [("p", C.c_int32), ("rk_order", C.c_int32), ("g", REAL), ("cf", REAL),
                 ("coriolis_f", REAL), ("h0_dry", REAL), ("limiter", C.c_int32), ("wetdry", C.c_int32),
-                ("flux", C.c_int32)]
+                ("flux", C.c_int32), ("rk_stages", C.c_int32)]
 
 
 class Holland(C.Structure):
@@ -104,6 +104,7 @@ def lib():
     L.orc_limit_var_vertex.argtypes = [C.c_int, PR, PR, PR]; L.orc_limit_var_vertex.restype = R
     L.orc_wetdry_elem.argtypes = [C.POINTER(Tables), R, PR, PR, PR, PR]; L.orc_wetdry_elem.restype = C.c_int
     L.orc_ssprk_step.argtypes = [C.c_int, I64, PR, PR, PR, D, D, RHS_FN, POST_FN, VP]; L.orc_ssprk_step.restype = C.c_int
+    L.orc_ssprk_step_s.argtypes = [C.c_int, C.c_int, I64, PR, PR, PR, D, D, RHS_FN, POST_FN, VP]; L.orc_ssprk_step_s.restype = C.c_int
     L.orc_create.argtypes = [C.POINTER(Params), I64, PR, PR, I64, C.POINTER(I32), I64, C.POINTER(I32),
                              C.POINTER(C.c_int8), C.POINTER(I32), C.POINTER(I32)]
     L.orc_create.restype = VP
@@ -203,8 +204,8 @@ def wetdry_elem(p, h0, hv, ze, qx, qy):
     return wet, ze, qx, qy
 
 
-def ssprk_step(order, w, t, dt, rhs_py, post_py=None):
-    """One SSP-RK step with a Python RHS rhs_py(stage, t_stage, w)->array."""
+def ssprk_step(order, w, t, dt, rhs_py, post_py=None, stages=0):
+    """One SSP-RK step with a Python RHS rhs_py(stage, t_stage, w)->array; stages = 0: as many as the order."""
     w = np.array(w, dtype=NP)
     n = w.size
     w0, rhs = np.zeros(n, dtype=NP), np.zeros(n, dtype=NP)
@@ -219,7 +220,7 @@ def ssprk_step(order, w, t, dt, rhs_py, post_py=None):
             wa = np.ctypeslib.as_array(wp, shape=(n,))
             post_py(stage, wa)
 
-    rc = lib().orc_ssprk_step(order, n, _dp(w), _dp(w0), _dp(rhs), t, dt, RHS_FN(_rhs), POST_FN(_post), None)
+    rc = lib().orc_ssprk_step_s(order, stages, n, _dp(w), _dp(w0), _dp(rhs), t, dt, RHS_FN(_rhs), POST_FN(_post), None)
     assert rc == 0
     return w
 
@@ -232,7 +233,7 @@ class Oracle:
         L = lib()
         self.L = L
         self.prm = Params(**{k: params[k] for k in ("p", "rk_order", "g", "cf", "coriolis_f", "h0_dry", "limiter", "wetdry")},
-                          flux=int(params.get("flux", 0)))
+                          flux=int(params.get("flux", 0)), rk_stages=int(params.get("rk_stages", 0)))
         self.p = params["p"]
         self.ndof = (self.p + 1) * (self.p + 2) // 2
         self.nqe = self.p + 1

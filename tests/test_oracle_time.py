@@ -8,6 +8,7 @@ import pytest
 from helpers import G, l2_project, small_mesh
 from workloads import c1, c2, c4, default_params
 from workloads.mesh import rect_mesh
+from workloads.mesh import vertex_to_modal_p1
 
 
 # ------------------------------------------------------------------ SSP-RK
@@ -36,6 +37,85 @@ def test_ssprk_stage_times_and_exact_stage_polynomials(O):
         w = O.ssprk_step(order, np.array([1.0]), 0.0, 1.0, lambda s, ts, ww: z * ww)
         taylor = sum(z ** k / math.factorial(k) for k in range(order + 1))
         assert abs(w[0] - taylor) < 1e-15
+
+
+# many-stage schemes (reading R-19): (order, stages) and the textbook stability polynomial of each, i.e. the factor one
+# step applies to dw/dt = lambda w: SSP(s,2): 1/s + (s-1)/s (1 + z/(s-1))^s; SSP(4,3): 2/3 (1 + z/2) + 1/3 (1 + z/2)^4,
+# written out in powers of z
+MANY_STAGE = {(2, 3): ([0.0, 0.5, 1.0], [1.0, 1.0, 0.5, 1.0 / 12.0]),
+              (2, 4): ([0.0, 1.0 / 3.0, 2.0 / 3.0, 1.0], [1.0, 1.0, 0.5, 1.0 / 9.0, 1.0 / 108.0]),
+              (3, 4): ([0.0, 0.5, 1.0, 0.5], [1.0, 1.0, 0.5, 1.0 / 6.0, 1.0 / 48.0])}
+
+
+@pytest.mark.parametrize("scheme", sorted(MANY_STAGE))
+def test_many_stage_ssprk_stability_polynomial_and_stage_times(O, scheme):
+    order, stages = scheme
+    cs, poly = MANY_STAGE[scheme]
+    seen = []
+    O.ssprk_step(order, np.array([1.0]), 10.0, 0.5, lambda s, ts, ww: (seen.append(ts), 0.0 * ww)[1], stages=stages)
+    assert len(seen) == stages and np.allclose(seen, [10.0 + c * 0.5 for c in cs], rtol=0, atol=1e-15)
+    for z in (-0.3, 0.7, -1.9):
+        w = O.ssprk_step(order, np.array([1.0, -2.0]), 0.0, 1.0, lambda s, ts, ww: z * ww, stages=stages)
+        exact = sum(ck * z ** k for k, ck in enumerate(poly))
+        assert abs(w[0] - exact) < 4e-16 * max(1.0, abs(exact)) * 8 and abs(w[1] + 2.0 * exact) < 1e-14
+    # the polynomial matches exp(z) through z^order and not beyond
+    for k in range(order + 1):
+        assert abs(poly[k] - 1.0 / math.factorial(k)) < 1e-15
+    assert abs(poly[order + 1] - 1.0 / math.factorial(order + 1)) > 1e-3
+
+
+@pytest.mark.parametrize("scheme", sorted(MANY_STAGE))
+def test_many_stage_ssprk_order_with_time_dependent_forcing(O, scheme):
+    """dw/dt = -w + cos t, w(0) = 0, exact w = (cos t + sin t - exp(-t)) / 2: the observed order is the scheme's,
+    which needs both the stage weights and the stage times to be right."""
+    order, stages = scheme
+    errs = []
+    for n in (16, 32, 64):
+        w = np.array([0.0]); dt = 2.0 / n
+        for i in range(n):
+            w = O.ssprk_step(order, w, i * dt, dt, lambda s, ts, ww: -ww + math.cos(ts), stages=stages)
+        errs.append(abs(w[0] - 0.5 * (math.cos(2.0) + math.sin(2.0) - math.exp(-2.0))))
+    r1, r2 = errs[0] / errs[1], errs[1] / errs[2]
+    assert abs(math.log2(r1) - order) < 0.25 and abs(math.log2(r2) - order) < 0.15, (errs, r1, r2)
+
+
+def test_many_stage_ssprk_is_ssp_with_larger_step(O):
+    """Strong stability: with L the first-order upwind operator on a periodic grid (forward Euler is TVD for
+    nu = a dt / dx <= 1), SSP(s,2) stays TVD up to nu = s - 1 and SSP(4,3) up to nu = 2 (the schemes' SSP coefficients,
+    which is what "optimized" buys), and each loses it a little beyond: a square wave's total variation is the witness."""
+    n = 64
+    u0 = np.where((np.arange(n) >= 16) & (np.arange(n) < 40), 1.0, 0.0)
+    tv = lambda u: np.abs(u - np.roll(u, 1)).sum()
+    up = lambda s, ts, u: -(u - np.roll(u, 1))          # a / dx = 1: dt is the Courant number
+    for (order, stages), c_ssp in (((2, 2), 1.0), ((3, 3), 1.0), ((2, 3), 2.0), ((2, 4), 3.0), ((3, 4), 2.0)):
+        for nu, must_hold in ((c_ssp, True), (1.6 * c_ssp, False)):
+            u = u0.copy(); worst = 0.0
+            for i in range(40):
+                u = O.ssprk_step(order, u, 0.0, nu, up, stages=stages)
+                worst = max(worst, tv(u) - tv(u0))
+            assert (worst <= 1e-12) == must_hold, (order, stages, nu, worst)
+
+
+def test_many_stage_scheme_in_the_model(O):
+    """The model takes rk_stages: seiche amplitude after a fixed time agrees between SSP(3,3) at dt and SSP(4,3) at
+    2 dt to the schemes' third-order accuracy, and an unknown (order, stages) pair is refused."""
+    mesh = rect_mesh(8, 8, 1000.0, 1000.0)
+    H = 10.0
+    ze0 = vertex_to_modal_p1(0.01 * np.cos(np.pi * mesh.xy[:, 0] / 1000.0), mesh.tri, 3)
+    z = np.zeros_like(ze0)
+    res = {}
+    for stages, dt, n in ((0, 1.0, 40), (4, 2.0, 20)):
+        prm = default_params(p=1, rk_order=3); prm["rk_stages"] = stages
+        o = O.Oracle(prm, mesh.xy, np.full(mesh.n_nodes, H), mesh.tri, mesh.edge_elem, mesh.edge_local, mesh.edge_bc, mesh.elem_edge)
+        o.set_state(0.0, ze0, z, z)
+        o.step(n, dt)
+        t, ze, _, _ = o.get_state()
+        assert t == 40.0
+        res[stages] = ze
+    assert 1e-9 < np.abs(res[0] - res[4]).max() < 2e-6       # different schemes, same solution to O(dt^3)
+    prm = default_params(p=1, rk_order=3); prm["rk_stages"] = 5
+    with pytest.raises(Exception):
+        O.Oracle(prm, mesh.xy, np.full(mesh.n_nodes, H), mesh.tri, mesh.edge_elem, mesh.edge_local, mesh.edge_bc, mesh.elem_edge)
 
 
 def test_rk_time_dependent_forcing_uses_stage_time(O):

@@ -48,7 +48,7 @@ class Workload:
 
     @property
     def n_stage(self) -> int:
-        return self.params["rk_order"]
+        return self.params.get("rk_stages", 0) or self.params["rk_order"]
 
     @property
     def dofs(self) -> int:
