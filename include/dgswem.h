@@ -39,7 +39,7 @@ typedef struct dgswem dgswem_t;   /* opaque */
 
 typedef struct {
   int32_t p;            /* polynomial degree, 1 or 2 (paper runs p=1)              */
-  int32_t rk_order;     /* 2: SSP(2,2), 3: SSP(3,3) (R-2)                */
+  int32_t rk_order;     /* order of the SSP Runge-Kutta scheme, 2 or 3 (R-2); see rk_stages */
   double  g;            /* gravity, e.g. 9.81                                                    */
   double  cf;           /* quadratic bottom friction coefficient, 0 = off (R-6)        */
   double  coriolis_f;   /* Coriolis parameter, 0 = off                             */
@@ -54,6 +54,9 @@ typedef struct {
                            metric) or 32 (the paper's own runs, PAPER.md:158 "-r4", :529).
                            Every pointer of this ABI stays binary64: values are rounded on the way in and are
                            exact on the way out; time, time step, tide and storm track stay binary64 inside */
+  int32_t rk_stages;    /* 0: as many stages as rk_order (SSP(2,2), SSP(3,3)).  Many-stage SSP schemes (PAPER.md:109
+                           "optimized ... SSPRK"; R-19), two-register Shu-Osher form: rk_order 2 with 3 or 4
+                           stages (optimal SSP(s,2), SSP coefficient s-1), rk_order 3 with 4 stages (SSP(4,3), coefficient 2) */
 } dgswem_params;
 
 /* Holland (1980) vortex, R-9: centre (x0+vx t, y0+vy t), radius of max wind rmax [m],
@@ -106,7 +109,7 @@ int dgswem_step(dgswem_t*, int64_t nsteps, double dt);
 /* ---- Stage-granular stepping and halo lists: building blocks of a domain-decomposed run (
  * PAPER.md:476-519 "Multiple GPUs").  A driver splits the mesh into partitions with one layer of edge-neighbour
  * ghost elements (whose outer edges it closes as land edges), creates one handle per partition and, for every step,
- * calls  begin_step;  for s in 0..rk_order-1: { stage_rhs(s); [limiter on: exchange what=1; stage_limit(s);]
+ * calls  begin_step;  for s in 0..n_stage-1: { stage_rhs(s); [limiter on: exchange what=1; stage_limit(s);]
  * exchange what=0 };  end_step  -- where "exchange" = halo_pack on the owner, transport, halo_unpack on the ghost side.
  * The ghost elements' own results are meaningless and are overwritten by every exchange; owned elements then get the
  * same bits as in an undivided run.  dgswem_step must not be called between begin_step and end_step.

@@ -20,7 +20,8 @@ E_NONFINITE = -4
 class Params(C.Structure):
     _fields_ = [("p", C.c_int32), ("rk_order", C.c_int32), ("g", C.c_double), ("cf", C.c_double),
                 ("coriolis_f", C.c_double), ("h0_dry", C.c_double), ("limiter", C.c_int32), ("wetdry", C.c_int32),
-                ("reorder", C.c_int32), ("device", C.c_int32), ("flux", C.c_int32), ("precision", C.c_int32)]
+                ("reorder", C.c_int32), ("device", C.c_int32), ("flux", C.c_int32), ("precision", C.c_int32),
+                ("rk_stages", C.c_int32)]
 
 
 class Holland(C.Structure):
@@ -120,7 +121,7 @@ class Dgswem:
         self.p = int(params["p"])
         self.ndof = (self.p + 1) * (self.p + 2) // 2
         self.nqe = self.p + 1
-        self.n_stage = int(params["rk_order"])
+        self.n_stage = int(params.get("rk_stages", 0)) or int(params["rk_order"])
         xy = np.ascontiguousarray(xy, dtype=np.float64)
         bathy = np.ascontiguousarray(bathy, dtype=np.float64)
         tri = np.ascontiguousarray(tri, dtype=np.int32)
@@ -132,7 +133,7 @@ class Dgswem:
         assert xy.shape == (self.n_nodes, 2) and bathy.shape == (self.n_nodes,) and tri.shape == (self.n_elem, 3)
         assert edge_elem.shape == (self.n_edge, 2) and edge_local.shape == (self.n_edge, 2)
         assert edge_bc.shape == (self.n_edge,) and elem_edge.shape == (self.n_elem, 3)
-        prm = Params(p=self.p, rk_order=self.n_stage, g=params["g"], cf=params["cf"], coriolis_f=params["coriolis_f"],
+        prm = Params(p=self.p, rk_order=int(params["rk_order"]), rk_stages=int(params.get("rk_stages", 0)), g=params["g"], cf=params["cf"], coriolis_f=params["coriolis_f"],
                      h0_dry=params["h0_dry"], limiter=int(params["limiter"]), wetdry=int(params["wetdry"]),
                      reorder=int(reorder), device=int(device), flux=int(params.get("flux", 0)),
                      precision=int(precision))

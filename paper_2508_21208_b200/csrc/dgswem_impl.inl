@@ -135,8 +135,11 @@ std::vector<int> hilbert_order(const std::vector<double>& px, const std::vector<
 }  // namespace
 
 // ------------------------------------------------------------------------------------ handle
+struct RkScheme { int ns; real a[4], b[4]; double beta[4], c[4]; };   // see rk_get
+
 struct Handle : ::dgswem {
   dgswem_params prm{};
+  RkScheme rk{};
   int ndof = 0, nqe = 0, nqa = 0, nstage = 0;
   long long nn = 0, ne = 0, nd = 0, ld = 0, ldd = 0, ldn = 0;
   cudaStream_t stream = nullptr;
@@ -577,28 +580,55 @@ int run_stage(Handle* h, const real* win, const real* w0, real* wout, double dt,
   return rc;
 }
 
-// Shu-Osher SSP(2,2) / SSP(3,3) (R-2)
-static const real kA2[2] = {RL(0.0), RL(0.5)}, kB2[2] = {RL(1.0), RL(0.5)};
-static const real kA3[3] = {RL(0.0), RL(0.75), RL(1.0) / RL(3.0)}, kB3[3] = {RL(1.0), RL(0.25), RL(2.0) / RL(3.0)};
-static const double kC2[2] = {0.0, 1.0}, kC3[3] = {0.0, 1.0, 0.5};   // stage times: binary64 like t and dt
+// Two-register Shu-Osher SSP Runge-Kutta schemes (R-2, R-19): stage s is
+//   u = w^(s-1) + (beta_s dt) L(w^(s-1), t + c_s dt);  w^(s) = u  (plain stage)  or  a_s w^n + b_s u.
+// (order, stages): (2,2), (3,3), the optimal many-stage schemes (2,3), (2,4) and (3,4).
+inline bool rk_get(int order, int stages, RkScheme& k) {
+  if (stages == 0) stages = order;
+  k.ns = stages;
+  for (int s = 0; s < 4; ++s) { k.a[s] = RL(0.0); k.b[s] = RL(1.0); k.beta[s] = 1.0; k.c[s] = 0.0; }
+  if (order == 2 && stages == 2) {
+    k.a[1] = RL(0.5); k.b[1] = RL(0.5); k.c[1] = 1.0;
+  } else if (order == 3 && stages == 3) {
+    k.a[1] = RL(0.75); k.b[1] = RL(0.25); k.c[1] = 1.0;
+    k.a[2] = RL(1.0) / RL(3.0); k.b[2] = RL(2.0) / RL(3.0); k.c[2] = 0.5;
+  } else if (order == 2 && (stages == 3 || stages == 4)) {
+    for (int s = 0; s < stages; ++s) { k.beta[s] = 1.0 / (double)(stages - 1); k.c[s] = (double)s / (double)(stages - 1); }
+    k.a[stages - 1] = RL(1.0) / (real)stages; k.b[stages - 1] = (real)(stages - 1) / (real)stages;
+  } else if (order == 3 && stages == 4) {
+    for (int s = 0; s < 4; ++s) k.beta[s] = 0.5;
+    k.c[1] = 0.5; k.c[2] = 1.0; k.c[3] = 0.5;
+    k.a[2] = RL(2.0) / RL(3.0); k.b[2] = RL(1.0) / RL(3.0);
+  } else {
+    return false;
+  }
+  return true;
+}
+
+// buffers and coefficients of stage s: w^n stays in W[0] until the last stage overwrites it; the stages in between
+// alternate W[1], W[2]
+struct StageBufs { const real* win; const real* w0; real* wout; real a, b; double c, beta; int first; };
+inline StageBufs stage_bufs(Handle* h, int s) {
+  const RkScheme& K = h->rk;
+  StageBufs B;
+  B.a = K.a[s]; B.b = K.b[s]; B.c = K.c[s]; B.beta = K.beta[s];
+  B.first = (K.a[s] == RL(0.0) && K.b[s] == RL(1.0)) ? 1 : 0;   // plain stage: no combine with w^n (and no read of it)
+  B.w0 = h->W[0];
+  B.win = s == 0 ? h->W[0] : h->W[1 + ((s - 1) & 1)];
+  B.wout = s == K.ns - 1 ? h->W[0] : h->W[1 + (s & 1)];
+  return B;
+}
 
 // enqueue the kernels of one time step starting at time t (values) or at table row *step_ctr (capturing)
 template <int P>
 int enqueue_step(Handle* h, double dt, double t) {
-  const bool rk3 = h->prm.rk_order == 3;
-  const real* a = rk3 ? kA3 : kA2; const real* b = rk3 ? kB3 : kB2; const double* c = rk3 ? kC3 : kC2;
   if (h->wind_on) { int rc = launch_wind(h, t); if (rc) return rc; }
-  // current state lives in W[0]; RK2: W0 -> W1 -> W0 ; RK3: W0 -> W1 -> W2 -> W0
-  int rc = run_stage<P>(h, h->W[0], h->W[0], h->W[1], dt, a[0], b[0], 1, t + c[0] * dt, 0);
-  if (rc) return rc;
-  if (!rk3) {
-    rc = run_stage<P>(h, h->W[1], h->W[0], h->W[0], dt, a[1], b[1], 0, t + c[1] * dt, 1);
-  } else {
-    rc = run_stage<P>(h, h->W[1], h->W[0], h->W[2], dt, a[1], b[1], 0, t + c[1] * dt, 1);
+  for (int s = 0; s < h->rk.ns; ++s) {
+    const StageBufs B = stage_bufs(h, s);
+    const int rc = run_stage<P>(h, B.win, B.w0, B.wout, B.beta * dt, B.a, B.b, B.first, t + B.c * dt, s);
     if (rc) return rc;
-    rc = run_stage<P>(h, h->W[2], h->W[0], h->W[0], dt, a[2], b[2], 0, t + c[2] * dt, 2);
   }
-  return rc;
+  return 0;
 }
 
 void drop_graphs(Handle* h) {
@@ -634,8 +664,7 @@ int capture_steps(Handle* h, int steps, double dt, bool need_tab, Handle::StepGr
 
 template <int P>
 int run_steps(Handle* h, long long nsteps, double dt) {
-  const bool rk3 = h->prm.rk_order == 3;
-  const double* c = rk3 ? kC3 : kC2;
+  const double* c = h->rk.c;
   if (!h->graphs_on || h->profiling || nsteps == 0) {
     for (long long n = 0; n < nsteps; ++n) {
       int rc = enqueue_step<P>(h, dt, h->t);
@@ -739,8 +768,9 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
     return bail(h->fail(DGSWEM_E_ARG, "NULL argument"));
   if (n_nodes < 3 || n_elem < 1 || n_edge < 3 || n_elem > 0x1fffffff || n_edge > 0x7ffffff0 || n_nodes > 0x7ffffff0)
     return bail(h->fail(DGSWEM_E_ARG, "bad sizes"));
-  if ((prm->p != 1 && prm->p != 2) || (prm->rk_order != 2 && prm->rk_order != 3))
-    return bail(h->fail(DGSWEM_E_ARG, "p must be 1 or 2, rk_order 2 or 3"));
+  if (prm->p != 1 && prm->p != 2) return bail(h->fail(DGSWEM_E_ARG, "p must be 1 or 2"));
+  if (!rk_get(prm->rk_order, prm->rk_stages, h->rk))
+    return bail(h->fail(DGSWEM_E_ARG, "(rk_order, rk_stages) must be (2, 0|2), (3, 0|3), (2, 3), (2, 4) or (3, 4)"));
   if (prm->flux < 0 || prm->flux > 1 || prm->limiter < 0 || prm->limiter > 2)
     return bail(h->fail(DGSWEM_E_ARG, "flux must be 0 (LLF) or 1 (Roe), limiter 0, 1 (edge neighbours) or 2 (vertex neighbourhood)"));
   if (!(prm->h0_dry > 0.0) || !(prm->g > 0.0) || prm->cf < 0.0)
@@ -749,7 +779,7 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
   if (!(prm->h0_dry >= 1e-100) || !(prm->g * prm->h0_dry >= 1e-100) || !(prm->g <= 1e100) || !(prm->h0_dry <= 1e100))
     return bail(h->fail(DGSWEM_E_ARG, "need 1e-100 <= h0_dry <= 1e100, g <= 1e100 and g*h0_dry >= 1e-100"));
   h->prm = *prm;
-  h->ndof = (prm->p + 1) * (prm->p + 2) / 2; h->nqe = prm->p + 1; h->nqa = prm->p == 1 ? 3 : 6; h->nstage = prm->rk_order;
+  h->ndof = (prm->p + 1) * (prm->p + 2) / 2; h->nqe = prm->p + 1; h->nqa = prm->p == 1 ? 3 : 6; h->nstage = h->rk.ns;
   h->nn = n_nodes; h->ne = n_elem; h->nd = n_edge;
   h->ld = round_up(n_elem, 256); h->ldd = round_up(n_edge, 256); h->ldn = round_up(n_nodes, 64);
   int rc = validate_mesh(h, n_nodes, xy, n_elem, tri, n_edge, edge_elem, edge_local, edge_bc, elem_edge);
@@ -1053,7 +1083,7 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
       if ((r = upload(h, h->inv_d, inv_d))) return r;
     }
     const size_t wbytes = (size_t)3 * h->ndof * ld * sizeof(real);
-    for (int i = 0; i < h->nstage; ++i) {
+    for (int i = 0; i < std::min(h->nstage, 3); ++i) {
       h->W[i] = (real*)h->dalloc(wbytes);
       if (!h->W[i]) return h->fail(DGSWEM_E_CUDA, "device allocation of %zu bytes failed", wbytes);
       CK(cudaMemsetAsync(h->W[i], 0, wbytes, h->stream));
@@ -1162,20 +1192,6 @@ int api_step(Handle* h, int64_t nsteps, double dt) {
 }
 
 // ---- stage-granular stepping + halo lists: the building blocks of a domain-decomposed run
-namespace {
-struct StageBufs { const real* win; const real* w0; real* wout; real a, b; double c; int first; };
-inline StageBufs stage_bufs(Handle* h, int s) {
-  const bool rk3 = h->prm.rk_order == 3;
-  const real* a = rk3 ? kA3 : kA2; const real* b = rk3 ? kB3 : kB2; const double* c = rk3 ? kC3 : kC2;
-  StageBufs B;
-  B.a = a[s]; B.b = b[s]; B.c = c[s]; B.first = s == 0; B.w0 = h->W[0];
-  if (s == 0) { B.win = h->W[0]; B.wout = h->W[1]; }
-  else if (!rk3 || s == 2) { B.win = h->W[s]; B.wout = h->W[0]; }
-  else { B.win = h->W[1]; B.wout = h->W[2]; }
-  return B;
-}
-}  // namespace
-
 int api_begin_step(Handle* h, double dt) {
   if (!h) return DGSWEM_E_ARG;
   if (!(dt > 0.0)) return h->fail(DGSWEM_E_ARG, "need dt > 0");
@@ -1194,8 +1210,8 @@ int api_stage_rhs(Handle* h, int s) {
   CK(cudaSetDevice(h->prm.device));
   const StageBufs B = stage_bufs(h, s);
   const double ts = h->t + B.c * h->step_dt;
-  const int rc = h->prm.p == 1 ? run_stage_rhs<1>(h, B.win, B.w0, B.wout, h->step_dt, B.a, B.b, B.first, ts, s)
-                               : run_stage_rhs<2>(h, B.win, B.w0, B.wout, h->step_dt, B.a, B.b, B.first, ts, s);
+  const int rc = h->prm.p == 1 ? run_stage_rhs<1>(h, B.win, B.w0, B.wout, B.beta * h->step_dt, B.a, B.b, B.first, ts, s)
+                               : run_stage_rhs<2>(h, B.win, B.w0, B.wout, B.beta * h->step_dt, B.a, B.b, B.first, ts, s);
   if (rc == 0) h->last_out = B.wout;
   return rc;
 }

@@ -94,7 +94,7 @@ class PartitionedDgswem:
         self.transport = transport if transport is not None else LocalTransport()
         self.n_elem = int(np.asarray(tri).shape[0])
         self.limiter = bool(params["limiter"])
-        self.n_stage = int(params["rk_order"])
+        self.n_stage = int(params.get("rk_stages", 0)) or int(params["rk_order"])
         bathy = np.asarray(bathy, dtype=np.float64)
         self.handles, self.plans, self.sbuf, self.rbuf = [], [], [], []
         for p in self.mine:
