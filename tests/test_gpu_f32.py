@@ -1,7 +1,7 @@
 """The fp32 variant of the CUDA path (dgswem_params.precision = 32, PAPER.md:158 "-r4", :529
 "computation is done with single-precision") against the binary32 build of the oracle -- element by element, EXACTLY:
 both sides perform the same sequence of IEEE binary32 operations -- and against the pinned
-binary64 oracle within the binary32 tolerance DESIGN.md section 11 states (relative L2 <= 2e-5 over these step counts).
+binary64 oracle within the binary32 tolerance DESIGN.md section 4 states (relative L2 <= 2e-5 over these step counts).
 The ABI is binary64 in both precisions: what the fp32 handle returns are binary32 values widened exactly."""
 import math
 
