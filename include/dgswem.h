@@ -119,6 +119,13 @@ int dgswem_step(dgswem_t*, int64_t nsteps, double dt);
  *   host memory (buf_on_device = 0, synchronous) or device memory (1, asynchronous on the handle's stream). */
 int dgswem_begin_step(dgswem_t*, double dt);
 int dgswem_stage_rhs(dgswem_t*, int s);
+/* The same in two halves, so that the halo exchange can overlap the interior elements ("overlapping
+ * computation and communication"): part = 1 evaluates the stage on the send-list elements only (after which
+ * dgswem_halo_pack may be enqueued and the packed buffer sent), part = 2 on all the others; part = 0 is
+ * dgswem_stage_rhs.  Same bits as the undivided call (every element's arithmetic is independent of the launch it runs
+ * in).  Stage forms that cannot run on a subset (DGSWEM_FUSED = 0, 2, 3) do the whole stage in part 1 and nothing in
+ * part 2. */
+int dgswem_stage_rhs_part(dgswem_t*, int s, int part);
 int dgswem_stage_limit(dgswem_t*, int s);
 int dgswem_end_step(dgswem_t*);
 int dgswem_set_halo(dgswem_t*, int64_t n_send, const int32_t* send_ids, int64_t n_recv, const int32_t* recv_ids);

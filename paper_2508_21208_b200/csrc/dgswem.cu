@@ -87,7 +87,8 @@ int dgswem_set_wind_forcing(dgswem_t* h, int stress_on, int pressure_on) { if (!
 int dgswem_set_rain(dgswem_t* h, double rate) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_set_rain, rate); }
 int dgswem_step(dgswem_t* h, int64_t nsteps, double dt) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_step, nsteps, dt); }
 int dgswem_begin_step(dgswem_t* h, double dt) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_begin_step, dt); }
-int dgswem_stage_rhs(dgswem_t* h, int s) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_stage_rhs, s); }
+int dgswem_stage_rhs(dgswem_t* h, int s) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_stage_rhs, s, 0); }
+int dgswem_stage_rhs_part(dgswem_t* h, int s, int part) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_stage_rhs, s, part); }
 int dgswem_stage_limit(dgswem_t* h, int s) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_stage_limit, s); }
 int dgswem_set_halo(dgswem_t* h, int64_t n_send, const int32_t* send_ids, int64_t n_recv, const int32_t* recv_ids) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_set_halo, n_send, send_ids, n_recv, recv_ids); }
 int dgswem_halo_pack(dgswem_t* h, int what, double* buf, int buf_on_device) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_halo_pack, what, buf, buf_on_device); }

@@ -198,6 +198,9 @@ struct Handle : ::dgswem {
   double step_dt = 0.0;        // dt of the step in progress (0: none)
   real* last_out = nullptr;  // stage buffer written by the last dgswem_stage_rhs (W[0] between steps)
   int *halo_send = nullptr, *halo_recv = nullptr;   // internal element ids
+  int* send_uniq = nullptr;            // the send list without repeats (an element may go to several neighbours)
+  unsigned char* send_mask = nullptr;  // [ld] 1 where the element is in the send list
+  long long n_send_uniq = 0;
   long long n_send = 0, n_recv = 0;
   double* halo_buf = nullptr;  // device staging for host-side pack/unpack, [rows][max(n_send, n_recv)]
 
@@ -454,8 +457,12 @@ int stg_kernel_attrs(Handle* h, int smem) {
 // A1-A5 (+A7) in one launch (element-centric form, no flux buffer)
 template <int P, int MODE>
 int launch_stage(Handle* h, const real* win, const real* w0, real* wout, double dt, real a, real b,
-                 int first, bool fuse_wd, bool write_mean, ScalRef zeta_b) {
+                 int first, bool fuse_wd, bool write_mean, ScalRef zeta_b, int part = 0) {
+  // part: 0 the whole mesh; 1 the send-list elements only, 2 all the others (form 1; the other forms do everything in part 1)
+  const bool split = part != 0 && !h->tiled && !h->staged && h->n_send_uniq > 0;
+  if (part == 2 && !split) return 0;
   ElemArgs A;
+  A.subset = h->send_uniq; A.skip = h->send_mask; A.nsub = (int)h->n_send_uniq;
   A.win = win; A.w0 = w0; A.wout = wout; A.flux = h->flux; A.elem_edge = h->elem_edge; A.jinv = h->jinv;
   A.lfac = h->lfac; A.hv = h->hv; A.tri = h->tri; A.tau = h->tau; A.wet = h->wet;
   A.etap = h->etap; A.stress = h->stress_on ? 1 : 0; A.press = h->press_on ? 1 : 0; A.rain = (real)h->rain;
@@ -489,6 +496,32 @@ int launch_stage(Handle* h, const real* win, const real* w0, real* wout, double 
         <<<grid, kTile, StageTile<P>::smem(h->tile_cap, h->tile_cap1, h->wind_on), h->stream>>>(A, ntiles);
     prof_end(h);
     CKL("k_stage_tile");
+    return 0;
+  }
+  if (split) {   // the listed elements (small: generic-flag kernel) / all but the flagged ones (specialised like the full launch)
+    if (part == 1 && h->n_send_uniq == 0) return 0;
+    prof_begin(h, PK_ELEM);
+    const int grid = grid_for(part == 1 ? h->n_send_uniq : h->ne, DGK_STAGE_THREADS);
+    if (h->prm.flux == 1) {
+      if (part == 1) k_stage<P, MODE, -1, 1, 1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A);
+      else k_stage<P, MODE, -1, 1, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A);
+    } else if (part == 1) {
+      k_stage<P, MODE, -1, 0, 1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A);
+    } else if constexpr (MODE == MODE_UPDATE && P == 1) {
+      switch (stage_variant(h, first)) {
+        case 0: k_stage<P, MODE, 0, 0, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+        case 1: k_stage<P, MODE, 1, 0, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+        case 2: k_stage<P, MODE, 2, 0, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+        case 3: k_stage<P, MODE, 3, 0, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+        case 6: k_stage<P, MODE, 6, 0, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+        case 7: k_stage<P, MODE, 7, 0, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+        default: k_stage<P, MODE, -1, 0, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      }
+    } else {
+      k_stage<P, MODE, -1, 0, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A);
+    }
+    prof_end(h);
+    CKL("k_stage (part)");
     return 0;
   }
   prof_begin(h, PK_ELEM);
@@ -556,13 +589,14 @@ double tide_value(const Handle* h, double t) {
 // one RK stage, first part: EDGE -> GATHER+AREA+RK (+wet/dry when no limiter follows)
 template <int P>
 int run_stage_rhs(Handle* h, const real* win, const real* w0, real* wout, double dt, real a, real b, int first,
-                  double t_stage, int stage) {
+                  double t_stage, int stage, int part = 0) {
   const bool lim = h->prm.limiter != 0;
   const bool wd = h->prm.wetdry != 0;
   int rc;
   if (h->fused) {
-    rc = launch_stage<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim, scal(h, stage, tide_value(h, t_stage)));
+    rc = launch_stage<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim, scal(h, stage, tide_value(h, t_stage)), part);
   } else {
+    if (part == 2) return 0;   // the edge + element pair does the whole stage in part 1
     rc = launch_edge<P>(h, win, scal(h, stage, tide_value(h, t_stage)));
     if (rc) return rc;
     rc = launch_elem<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim);
@@ -1203,15 +1237,16 @@ int api_begin_step(Handle* h, double dt) {
   return DGSWEM_OK;
 }
 
-int api_stage_rhs(Handle* h, int s) {
+int api_stage_rhs(Handle* h, int s, int part) {
   if (!h) return DGSWEM_E_ARG;
   if (h->step_dt == 0.0) return h->fail(DGSWEM_E_ARG, "no step in progress (dgswem_begin_step)");
   if (s < 0 || s >= h->nstage) return h->fail(DGSWEM_E_ARG, "stage index out of range");
+  if (part < 0 || part > 2) return h->fail(DGSWEM_E_ARG, "part must be 0 (all), 1 (send-list elements) or 2 (the others)");
   CK(cudaSetDevice(h->prm.device));
   const StageBufs B = stage_bufs(h, s);
   const double ts = h->t + B.c * h->step_dt;
-  const int rc = h->prm.p == 1 ? run_stage_rhs<1>(h, B.win, B.w0, B.wout, B.beta * h->step_dt, B.a, B.b, B.first, ts, s)
-                               : run_stage_rhs<2>(h, B.win, B.w0, B.wout, B.beta * h->step_dt, B.a, B.b, B.first, ts, s);
+  const int rc = h->prm.p == 1 ? run_stage_rhs<1>(h, B.win, B.w0, B.wout, B.beta * h->step_dt, B.a, B.b, B.first, ts, s, part)
+                               : run_stage_rhs<2>(h, B.win, B.w0, B.wout, B.beta * h->step_dt, B.a, B.b, B.first, ts, s, part);
   if (rc == 0) h->last_out = B.wout;
   return rc;
 }
@@ -1260,8 +1295,20 @@ int api_set_halo(Handle* h, int64_t n_send, const int32_t* send_ids, int64_t n_r
   if (!conv(n_send, send_ids, snd) || !conv(n_recv, recv_ids, rcv)) return h->fail(DGSWEM_E_ARG, "halo element id out of range");
   int r;
   CK(cudaStreamSynchronize(h->stream));        // nothing in flight may still read the lists being replaced
-  h->dfree(h->halo_send); h->dfree(h->halo_recv); h->dfree(h->halo_buf);
+  h->dfree(h->halo_send); h->dfree(h->halo_recv); h->dfree(h->halo_buf); h->dfree(h->send_uniq); h->dfree(h->send_mask);
   h->halo_send = nullptr; h->halo_recv = nullptr; h->halo_buf = nullptr; h->n_send = 0; h->n_recv = 0;
+  h->send_uniq = nullptr; h->send_mask = nullptr; h->n_send_uniq = 0;
+  {
+    std::vector<unsigned char> mask((size_t)h->ld, 0);
+    std::vector<int> uniq;
+    for (int64_t i = 0; i < n_send; ++i)
+      if (!mask[(size_t)snd[(size_t)i]]) { mask[(size_t)snd[(size_t)i]] = 1; uniq.push_back(snd[(size_t)i]); }
+    std::sort(uniq.begin(), uniq.end());
+    h->n_send_uniq = (long long)uniq.size();
+    if (uniq.empty()) uniq.push_back(0);
+    if ((r = upload(h, h->send_uniq, uniq))) return r;
+    if ((r = upload(h, h->send_mask, mask))) return r;
+  }
   if ((r = upload(h, h->halo_send, snd))) return r;
   if ((r = upload(h, h->halo_recv, rcv))) return r;
   h->n_send = n_send; h->n_recv = n_recv;

@@ -31,11 +31,16 @@ CASES = {
 }
 
 
-@pytest.mark.parametrize("fused", ["0", "1", "2", "3"], ids=["edge+elem", "stage", "stage-tile", "stage-staged"])
+@pytest.mark.parametrize("fused", ["0", "1", "1-no-overlap", "2", "3"],
+                         ids=["edge+elem", "stage", "stage-no-overlap", "stage-tile", "stage-staged"])   # overlap is forced on otherwise
 @pytest.mark.parametrize("n_parts", [2, 5])
 @pytest.mark.parametrize("case", sorted(CASES))
 def test_partitioned_run_equals_undivided_run(O, G, monkeypatch, case, n_parts, fused):
-    """... and the ORACLE's run, directly (not only transitively through the undivided GPU run)."""
+    """... and the ORACLE's run, directly (not only transitively through the undivided GPU run).  By default every stage
+    is split into the send-list elements (dgswem_stage_rhs_part 1), whose packed values travel on the communication
+    stream while the interior elements are computed (part 2); "no-overlap" is the unsplit order of calls."""
+    overlap = not fused.endswith("no-overlap")
+    fused = fused[0]
     from paper_2508_21208_b200.decomp import PartitionedDgswem
     monkeypatch.setenv("DGSWEM_FUSED", fused)
     w = CASES[case]()
@@ -50,7 +55,7 @@ def test_partitioned_run_equals_undivided_run(O, G, monkeypatch, case, n_parts, 
     wet_ref = ref.get_wetdry()
     ref.close()
     pd = PartitionedDgswem(w.params, m.xy, w.bathy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, n_parts,
-                           tide=w.tide, holland=w.holland)
+                           tide=w.tide, holland=w.holland, overlap=overlap)
     assert sum(s.n_owned for s in pd.subs) == m.n_elem
     assert all(s.n_local > s.n_owned for s in pd.subs)            # every partition has ghosts
     pd.set_state(0.0, w.ze, w.qx, w.qy)
@@ -86,5 +91,7 @@ def test_stage_api_equals_dgswem_step_and_rejects_misuse(G):
         b.step(1, w.dt)                     # dgswem_step inside a stage-granular step
     with pytest.raises(G.DgswemError):
         b.stage_rhs(7)
+    with pytest.raises(G.DgswemError):
+        b.stage_rhs(0, part=3)
     b.end_step()
     a.close(); b.close()

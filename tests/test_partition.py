@@ -117,3 +117,89 @@ def test_dist_transport_delivers_every_ghost_gloo(tmp_path, world):
     for r in range(world):
         ok, ns, nr = (tmp_path / f"rank{r}.txt").read_text().split()
         assert ok == "1" and int(ns) > 0 and int(nr) > 0
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# End to end on CPU: two ranks (gloo), one partition each, HOST tensors through DistTransport every RK stage, with the
+# oracle standing in for the kernels of each partition (its RHS on the local mesh: owned elements + one ghost layer,
+# ghost outer edges closed).  What this pins without a GPU: the ghost layer is all a stage needs, the send / receive
+# lists and the transport put every value where the next stage reads it, and the order of calls of
+# PartitionedDgswem.step (stage -> exchange state) reproduces the undivided run.  The RK combine is numpy here (no fma),
+# so the comparison with the undivided oracle is to round-off, not bitwise (bitwise is the GPU tests' job).
+def _e2e_workload():
+    from workloads import c3
+    return c3(nn=14, nsteps=6)            # jittered, permuted, shelf bathymetry, M2 tide on the east side
+
+
+def _e2e_worker(rank, world, port, out_dir):
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, str(ROOT))
+    from oracle import oracle as orc
+    from paper_2508_21208_b200.partition import partition
+    from paper_2508_21208_b200.decomp import HaloPlan, DistTransport
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    try:
+        w = _e2e_workload(); m = w.mesh
+        prm = dict(w.params); prm["wetdry"] = 0; prm["limiter"] = 0
+        sub = partition(m.xy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, world)[rank]
+        plan = HaloPlan(sub)
+        o = orc.Oracle(prm, sub.xy, np.asarray(w.bathy)[sub.node_gid], sub.tri, sub.edge_elem, sub.edge_local, sub.edge_bc, sub.elem_edge)
+        o.set_tide(*w.tide)
+        gid = sub.elem_gid
+        # a non-trivial smooth state so that every mode and every exchange matters
+        rng = np.random.default_rng(7)
+        full = [0.05 * rng.standard_normal((3, m.n_elem)) for _ in range(3)]
+        st = [np.ascontiguousarray(f[:, gid]) for f in full]
+        wet = np.ones(sub.n_local, dtype=np.uint8)
+        tr = DistTransport()
+
+        def exchange(state):
+            snd = torch.from_numpy(np.concatenate([a[:, plan.send_ids] for a in state], axis=0).copy())
+            rcv = torch.zeros((9, plan.n_recv), dtype=torch.float64)
+            tr.exchange([plan], [snd], [rcv])
+            r = rcv.numpy()
+            for c in range(3):
+                state[c][:, plan.recv_ids] = r[3 * c:3 * c + 3]
+
+        t, dt = 0.0, w.dt
+        for _ in range(w.nsteps):
+            w0 = [a.copy() for a in st]
+            for s, (a, b, cs) in enumerate(((0.0, 1.0, 0.0), (0.5, 0.5, 1.0))):      # SSP(2,2)
+                o.set_state_raw(t + cs * dt, *st, wet)
+                rhs = o.eval_rhs()
+                st = [a * w0[c] + b * (st[c] + dt * rhs[c]) if s else st[c] + dt * rhs[c] for c in range(3)]
+                exchange(st)
+            t += dt
+        np.save(Path(out_dir, f"state{rank}.npy"), np.stack([a[:, :sub.n_owned] for a in st]))
+        np.save(Path(out_dir, f"gid{rank}.npy"), gid[:sub.n_owned])
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_decomposed_run_equals_undivided_oracle_gloo(tmp_path):
+    import torch.multiprocessing as mp
+    from oracle import oracle as orc
+    orc.build()
+    w = _e2e_workload(); m = w.mesh
+    prm = dict(w.params); prm["wetdry"] = 0; prm["limiter"] = 0
+    o = orc.Oracle(prm, m.xy, w.bathy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge)
+    o.set_tide(*w.tide)
+    rng = np.random.default_rng(7)
+    full = [0.05 * rng.standard_normal((3, m.n_elem)) for _ in range(3)]
+    o.set_state_raw(0.0, *full, np.ones(m.n_elem, dtype=np.uint8))
+    o.step(w.nsteps, w.dt)
+    _, *ref = o.get_state()
+    world = 2
+    mp.spawn(_e2e_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    seen = np.zeros(m.n_elem, dtype=bool)
+    for r in range(world):
+        st = np.load(tmp_path / f"state{r}.npy"); gid = np.load(tmp_path / f"gid{r}.npy")
+        assert not seen[gid].any()
+        seen[gid] = True
+        for c in range(3):
+            scale = np.abs(ref[c]).max()
+            assert np.abs(st[c] - ref[c][:, gid]).max() <= 1e-12 * scale, (r, c)
+    assert seen.all()
+    # and the exchange is what makes it so: without it the ghosts go stale and the owned elements next to them drift
+    assert np.abs(ref[0]).max() > 1e-3
