@@ -51,8 +51,8 @@ def test_product_does_not_touch_the_oracle():
 
 
 def test_sass_has_fp64_and_no_float_atomics():
-    """The kernels are fp64 (DADD/DMUL present) and contain no floating-point atomics or FMA
-    contractions."""
+    """The kernels are fp64 (DADD/DMUL present) and contain no floating-point atomics (the DFMAs are
+    the explicit fma() calls of the canonical arithmetic, the compiler contracts nothing by itself: -fmad=false)."""
     import shutil, subprocess
     if shutil.which("cuobjdump") is None:
         pytest.skip("cuobjdump not available")
