@@ -169,6 +169,7 @@ struct Handle : ::dgswem {
   bool fused = false;         // element-centric stage kernel (k_stage) instead of k_edge + k_elem
   bool tiled = false;         // ... in its shared-memory edge-tile form (k_stage_tile): each tile evaluates its unique edges once
   bool staged = false;        // ... with TMA-staged operands (k_stage_stg)
+  int pf_dist = 0;            // k_stage: L2 prefetch distance in tiles (DGSWEM_PF_DIST; 0 = off)
   int *nbs = nullptr, *stg_nb = nullptr;
   int2* stg_info = nullptr;
   int stg_cap1 = 0, res_stg[2] = {0, 0};
@@ -462,7 +463,7 @@ int launch_stage(Handle* h, const real* win, const real* w0, real* wout, double 
   const bool split = part != 0 && !h->tiled && !h->staged && h->n_send_uniq > 0;
   if (part == 2 && !split) return 0;
   ElemArgs A;
-  A.subset = h->send_uniq; A.skip = h->send_mask; A.nsub = (int)h->n_send_uniq;
+  A.subset = h->send_uniq; A.skip = h->send_mask; A.nsub = (int)h->n_send_uniq; A.pf_dist = h->pf_dist;
   A.win = win; A.w0 = w0; A.wout = wout; A.flux = h->flux; A.elem_edge = h->elem_edge; A.jinv = h->jinv;
   A.lfac = h->lfac; A.hv = h->hv; A.tri = h->tri; A.tau = h->tau; A.wet = h->wet;
   A.etap = h->etap; A.stress = h->stress_on ? 1 : 0; A.press = h->press_on ? 1 : 0; A.rain = (real)h->rain;
@@ -864,6 +865,10 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
     // DGSWEM_FUSED=1/0: element-centric stage kernel (no flux buffer) on/off; default: on for p = 1
     h->fused = prm->p == 1;
     h->tiled = false;
+    // k_stage's L2 prefetch: on where a stage buffer does not stay in the 126 MB L2 anyway (C3: 336 -> 305 us per launch at any
+    // distance from 50 to 600 tiles; C4, whose state fits, gains nothing)
+    h->pf_dist = ((size_t)3 * h->ndof * h->ld * sizeof(real) > ((size_t)100 << 20)) ? 200 : 0;
+    if (const char* env = std::getenv("DGSWEM_PF_DIST")) h->pf_dist = std::max(0, std::atoi(env));
     if (const char* env = std::getenv("DGSWEM_FUSED")) { h->fused = std::atoi(env) != 0; h->tiled = std::atoi(env) == 2; h->staged = std::atoi(env) == 3; }
 
     const long long ne = h->ne, nd = h->nd, nn = h->nn, ld = h->ld, ldd = h->ldd, ldn = h->ldn;
