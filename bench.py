@@ -465,7 +465,7 @@ def main():
     ap.add_argument("--workload", default="C3")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"], help="working precision of the path (f32: SURVEY 8(f) NEXT-2, "
                     "the paper's own precision; the driver's default line stays C3 / f64)")
-    ap.add_argument("--reorder", type=int, default=1)
+    ap.add_argument("--reorder", type=int, default=1, help="internal renumbering: 0 none, 1 Hilbert curve (default), 2 reverse Cuthill-McKee")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--decomp", type=int, default=0, help="domain decomposition instead of replicas: one partition per rank "
                     "(N > 1), or this many partitions on the one GPU (N = 1)")

@@ -47,7 +47,8 @@ typedef struct {
   int32_t limiter;      /* slope limiter after every stage: 0 off, 1 edge-neighbour
                            Barth-Jespersen (R-7), 2 vertex-neighbourhood Barth-Jespersen (R-18)   */
   int32_t wetdry;       /* 0/1: wet/dry pass after every stage (R-8)               */
-  int32_t reorder;      /* 0: keep caller's numbering internally; 1: Hilbert-curve renumbering   */
+  int32_t reorder;      /* internal renumbering (invisible at this ABI; north_star (b)): 0 keep the caller's numbering,
+                           1 Hilbert curve through the element centroids, 2 reverse Cuthill-McKee on the element graph */
   int32_t device;       /* CUDA device ordinal                                                   */
   int32_t flux;         /* numerical flux: 0 local Lax-Friedrichs (R-3), 1 Roe (R-17)      */
   int32_t precision;    /* working precision of state, tables and kernels: 64 (or 0; default, the BASELINE

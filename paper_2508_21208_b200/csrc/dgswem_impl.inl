@@ -132,6 +132,39 @@ std::vector<int> hilbert_order(const std::vector<double>& px, const std::vector<
   return order;   // order[new] = old
 }
 
+// Reverse Cuthill-McKee on the element adjacency graph (two elements are adjacent when they share an edge): breadth-first
+// levels from a low-degree start element, neighbours by ascending degree (ties by index), every component in turn,
+// the whole order reversed.  The other renumbering north_star names; narrows the distance between edge neighbours.
+std::vector<int> rcm_order(long long ne, long long nd, const int32_t* edge_elem) {
+  std::vector<int> adj(3 * ne, -1), deg(ne, 0);
+  for (long long d = 0; d < nd; ++d) {
+    const int a = edge_elem[2 * d], b = edge_elem[2 * d + 1];
+    if (b < 0) continue;
+    adj[3 * (long long)a + deg[a]++] = b;
+    adj[3 * (long long)b + deg[b]++] = a;
+  }
+  std::vector<int> order; order.reserve(ne);
+  std::vector<char> seen(ne, 0);
+  std::vector<int> starts(ne);
+  std::iota(starts.begin(), starts.end(), 0);
+  std::stable_sort(starts.begin(), starts.end(), [&](int x, int y) { return deg[x] < deg[y]; });
+  for (int s0 : starts) {
+    if (seen[s0]) continue;
+    seen[s0] = 1;
+    size_t head = order.size();
+    order.push_back(s0);
+    while (head < order.size()) {
+      const int e = order[head++];
+      int nb[3]; int k = 0;
+      for (int l = 0; l < deg[e]; ++l) { const int q = adj[3 * (long long)e + l]; if (!seen[q]) { seen[q] = 1; nb[k++] = q; } }
+      std::sort(nb, nb + k, [&](int x, int y) { return deg[x] != deg[y] ? deg[x] < deg[y] : x < y; });
+      for (int i = 0; i < k; ++i) order.push_back(nb[i]);
+    }
+  }
+  std::reverse(order.begin(), order.end());
+  return order;   // order[new] = old
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------ handle
@@ -806,6 +839,7 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
   if (prm->p != 1 && prm->p != 2) return bail(h->fail(DGSWEM_E_ARG, "p must be 1 or 2"));
   if (!rk_get(prm->rk_order, prm->rk_stages, h->rk))
     return bail(h->fail(DGSWEM_E_ARG, "(rk_order, rk_stages) must be (2, 0|2), (3, 0|3), (2, 3), (2, 4) or (3, 4)"));
+  if (prm->reorder < 0 || prm->reorder > 2) return bail(h->fail(DGSWEM_E_ARG, "reorder must be 0 (none), 1 (Hilbert curve) or 2 (reverse Cuthill-McKee)"));
   if (prm->flux < 0 || prm->flux > 1 || prm->limiter < 0 || prm->limiter > 2)
     return bail(h->fail(DGSWEM_E_ARG, "flux must be 0 (LLF) or 1 (Roe), limiter 0, 1 (edge neighbours) or 2 (vertex neighbourhood)"));
   if (!(prm->h0_dry > 0.0) || !(prm->g > 0.0) || prm->cf < 0.0)
@@ -882,12 +916,14 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
         cy[e] = (xy[2 * (long long)t[0] + 1] + xy[2 * (long long)t[1] + 1] + xy[2 * (long long)t[2] + 1]) / 3.0;
       }
       perm_e = hilbert_order(cx, cy);
+    } else if (prm->reorder == 2) {
+      perm_e = rcm_order(ne, nd, edge_elem);
     } else {
       std::iota(perm_e.begin(), perm_e.end(), 0);
       std::iota(perm_d.begin(), perm_d.end(), 0);
     }
     for (long long i = 0; i < ne; ++i) inv_e[perm_e[i]] = (int)i;
-    if (prm->reorder == 1) {
+    if (prm->reorder != 0) {
       // edges follow the elements: sorted by (first, second) of their two elements in the new element
       // numbering, so an edge sits next to the first element that needs it and the
       // state gather of consecutive edges walks consecutive elements
@@ -1116,7 +1152,7 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
     if ((r = upload(h, h->nxy, nxy))) return r;
     if ((r = upload(h, h->node_ptr, node_ptr))) return r;
     if ((r = upload(h, h->node_ev, node_ev))) return r;
-    if (prm->reorder == 1) {
+    if (prm->reorder != 0) {
       if ((r = upload(h, h->perm_e, perm_e))) return r;
       if ((r = upload(h, h->inv_e, inv_e))) return r;
       if ((r = upload(h, h->inv_d, inv_d))) return r;

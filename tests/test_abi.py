@@ -72,7 +72,7 @@ def _raw_create(lib, w, *, params=None, tri=None, edge_elem=None, edge_bc=None, 
     m = w.mesh
     prm = dict(w.params) if params is None else params
     P = Params(p=int(prm["p"]), rk_order=int(prm["rk_order"]), g=prm["g"], cf=prm["cf"], coriolis_f=prm["coriolis_f"],
-               h0_dry=prm["h0_dry"], limiter=int(prm["limiter"]), wetdry=int(prm["wetdry"]), reorder=1, device=0,
+               h0_dry=prm["h0_dry"], limiter=int(prm["limiter"]), wetdry=int(prm["wetdry"]), reorder=int(prm.get("reorder", 1)), device=0,
                rk_stages=int(prm.get("rk_stages", 0)))
     xy = np.ascontiguousarray(m.xy, dtype=np.float64)
     bathy = np.ascontiguousarray(w.bathy, dtype=np.float64)
@@ -100,7 +100,7 @@ def test_create_validates_arguments_and_mesh_on_the_host(lib):
     from workloads import c1
     w = c1(nq=4)
     m = w.mesh
-    for key, val in (("p", 3), ("rk_order", 4), ("rk_stages", 5), ("rk_stages", 1), ("h0_dry", 0.0), ("h0_dry", 1e-200), ("g", -9.81), ("cf", -1.0)):
+    for key, val in (("p", 3), ("rk_order", 4), ("rk_stages", 5), ("rk_stages", 1), ("reorder", 3), ("h0_dry", 0.0), ("h0_dry", 1e-200), ("g", -9.81), ("cf", -1.0)):
         bad = dict(w.params); bad[key] = val
         rc, msg = _raw_create(lib, w, params=bad)
         assert rc == -1, (key, val, rc, msg)
