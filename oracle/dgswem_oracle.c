@@ -43,8 +43,12 @@
 
 /* ------------------------------------------------------------------ basis */
 /* Dubiner orthogonal modal basis on the reference triangle (-1,-1),(1,-1),(-1,1),
- * PAPER.md:97-103 eq. (4); mode order 00, 01, 10, then 02, 11, 20.
- * Input barycentrics; xi_1 = 2 lam_1 - 1, xi_2 = 2 lam_2 - 1.  d1, d2 = d/dxi_1, d/dxi_2. */
+ * PAPER.md:97-103 eq. (4); mode order 00, 01, 10, then 02, 11, 20, then 03, 12, 21, 30 (p = 3).
+ * Input barycentrics; xi_1 = 2 lam_1 - 1, xi_2 = 2 lam_2 - 1.  d1, d2 = d/dxi_1, d/dxi_2.
+ * phi_ij = A_i(xi_1, xi_2) B_j^(2i+1)(xi_2) with A_i = P_i(eta_1) s^i (Legendre in the collapsed coordinate, s = (1 - xi_2)/2:
+ * A_1 = a = xi_1 + (1 + xi_2)/2, A_2 = (3 a^2 - s^2)/2, A_3 = (5 a^3 - 3 a s^2)/2) and B_j^(alpha) the Jacobi polynomial
+ * P_j^(alpha,0): B_1^(3) = (5 y + 3)/2, B_1^(5) = (7 y + 5)/2, B_2^(1) = (5 y^2 + 2 y - 1)/2, B_2^(3) = (21 y^2 + 18 y + 1)/4,
+ * B_3^(1) = (35 y^3 + 15 y^2 - 15 y - 3)/8.  All ten modes are always written (callers use the first ndof). */
 void orc_basis(real lam0, real lam1, real lam2, real* phi, real* d1, real* d2) {
   (void)lam0;
   real xi1 = RL(2.0) * lam1 - RL(1.0);
@@ -63,14 +67,33 @@ void orc_basis(real lam0, real lam1, real lam2, real* phi, real* d1, real* d2) {
   d1[3] = RL(0.0);            d2[3] = RL(5.0) * xi2 + RL(1.0);
   d1[4] = r;              d2[4] = RL(0.5) * r + RL(2.5) * phi[2];
   d1[5] = RL(3.0) * phi[2];   d2[5] = RL(0.5) * (RL(3.0) * phi[2] + s);
+  /* p = 3 */
+  {
+    const real y = xi2, a = phi[2];
+    const real b3 = RL(0.125) * ((((RL(35.0) * y) * y) * y + (RL(15.0) * y) * y) - RL(15.0) * y - RL(3.0));
+    const real db3 = RL(0.125) * (((RL(105.0) * y) * y + RL(30.0) * y) - RL(15.0));
+    const real b2 = RL(0.25) * (((RL(21.0) * y) * y + RL(18.0) * y) + RL(1.0));
+    const real db2 = RL(0.25) * (RL(42.0) * y + RL(18.0));
+    const real b1 = RL(0.5) * (RL(7.0) * y + RL(5.0));
+    const real a2 = phi[5];                                   /* A_2 */
+    const real da2x = d1[5], da2y = d2[5];
+    const real a3 = RL(0.5) * (((RL(5.0) * a) * a) * a - ((RL(3.0) * a) * s) * s);
+    const real da3x = RL(0.5) * ((RL(15.0) * a) * a - (RL(3.0) * s) * s);
+    const real da3y = RL(0.5) * (((RL(7.5) * a) * a - (RL(1.5) * s) * s) + (RL(3.0) * a) * s);
+    phi[6] = b3;          d1[6] = RL(0.0);      d2[6] = db3;
+    phi[7] = a * b2;      d1[7] = b2;           d2[7] = RL(0.5) * b2 + a * db2;
+    phi[8] = a2 * b1;     d1[8] = da2x * b1;    d2[8] = da2y * b1 + RL(3.5) * a2;
+    phi[9] = a3;          d1[9] = da3x;         d2[9] = da3y;
+  }
 }
 
 /* Quadrature [R-5] (paper: "Gauss-Lobatto", no orders): edges Gauss-Legendre
- * with p+1 points; area: p=1 three interior points (2/3,1/6,1/6), p=2 six-point degree-4 rule.
+ * with p+1 points; area: p=1 three interior points (2/3,1/6,1/6), p=2 six-point degree-4 rule, p=3 the classical
+ * twelve-point degree-6 rule (two 3-point orbits, one 6-point orbit).
  * Reference mass M_ij = 2/((2i+1)(i+j+1)) (diagonal). */
 int orc_make_tables(int p, orc_tables* T) {
   memset(T, 0, sizeof(*T));
-  if (p != 1 && p != 2) return -1;
+  if (p != 1 && p != 2 && p != 3) return -1;
   T->p = p;
   T->ndof = (p + 1) * (p + 2) / 2;
   T->nqe = p + 1;
@@ -81,6 +104,28 @@ int orc_make_tables(int p, orc_tables* T) {
     for (int i = 0; i < 3; ++i) {
       for (int v = 0; v < 3; ++v) T->la[i][v] = (v == i) ? RL(2.0) / RL(3.0) : RL(1.0) / RL(6.0);
       T->wa[i] = RL(2.0) / RL(3.0);
+    }
+  } else if (p == 3) {
+    T->ge[0] = -RL(0.86113631159405258); T->ge[1] = -RL(0.33998104358485626); T->ge[2] = RL(0.33998104358485626); T->ge[3] = RL(0.86113631159405258);
+    T->we[0] = RL(0.34785484513745386); T->we[1] = RL(0.65214515486254614); T->we[2] = RL(0.65214515486254614); T->we[3] = RL(0.34785484513745386);
+    T->nqa = 12;
+    const real a1 = RL(0.249286745170910), w1 = RL(0.116786275726379);
+    const real a2 = RL(0.063089014491502), w2 = RL(0.050844906370207);
+    const real b3 = RL(0.053145049844817), c3 = RL(0.310352451033784), w3 = RL(0.082851075618374);
+    for (int i = 0; i < 3; ++i) {
+      for (int v = 0; v < 3; ++v) {
+        T->la[i][v]     = (v == i) ? RL(1.0) - RL(2.0) * a1 : a1;
+        T->la[3 + i][v] = (v == i) ? RL(1.0) - RL(2.0) * a2 : a2;
+      }
+      T->wa[i] = RL(2.0) * w1;
+      T->wa[3 + i] = RL(2.0) * w2;
+    }
+    /* the six permutations of (b3, c3, 1 - b3 - c3) */
+    static const int perm[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
+    const real tri3[3] = {b3, c3, (RL(1.0) - b3) - c3};
+    for (int q = 0; q < 6; ++q) {
+      for (int v = 0; v < 3; ++v) T->la[6 + q][v] = tri3[perm[q][v]];
+      T->wa[6 + q] = RL(2.0) * w3;
     }
   } else {
     T->ge[0] = -RL(0.77459666924148338); T->ge[1] = RL(0.0); T->ge[2] = RL(0.77459666924148338);
@@ -97,9 +142,10 @@ int orc_make_tables(int p, orc_tables* T) {
       T->wa[3 + i] = RL(2.0) * w2;
     }
   }
-  const real M[6] = {RL(2.0), RL(1.0), RL(1.0) / RL(3.0), RL(2.0) / RL(3.0), RL(2.0) / RL(9.0), RL(2.0) / RL(15.0)};
+  const real M[10] = {RL(2.0), RL(1.0), RL(1.0) / RL(3.0), RL(2.0) / RL(3.0), RL(2.0) / RL(9.0), RL(2.0) / RL(15.0),
+                      RL(0.5), RL(1.0) / RL(6.0), RL(0.1), RL(1.0) / RL(14.0)};
   for (int k = 0; k < T->ndof; ++k) T->invM[k] = RL(1.0) / M[k];
-  real phi[6], d1[6], d2[6];
+  real phi[ORC_MAXDOF], d1[ORC_MAXDOF], d2[ORC_MAXDOF];
   for (int i = 0; i < T->nqa; ++i) {
     orc_basis(T->la[i][0], T->la[i][1], T->la[i][2], phi, d1, d2);
     for (int k = 0; k < T->ndof; ++k) {
@@ -347,7 +393,7 @@ real orc_limit_var(int p, real* w, const real* mean_nb, const int* has_nb) {
   }
   w[1] = alpha * b;
   w[2] = alpha * c;
-  if (p == 2 && alpha < RL(1.0)) { w[3] = RL(0.0); w[4] = RL(0.0); w[5] = RL(0.0); }
+  if (p >= 2 && alpha < RL(1.0)) { for (int k = 3; k < (p + 1) * (p + 2) / 2; ++k) w[k] = RL(0.0); }
   return alpha;
 }
 
@@ -372,7 +418,7 @@ real orc_limit_var_vertex(int p, real* w, const real* vmin, const real* vmax) {
   }
   w[1] = alpha * b;
   w[2] = alpha * c;
-  if (p == 2 && alpha < RL(1.0)) { w[3] = RL(0.0); w[4] = RL(0.0); w[5] = RL(0.0); }
+  if (p >= 2 && alpha < RL(1.0)) { for (int k = 3; k < (p + 1) * (p + 2) / 2; ++k) w[k] = RL(0.0); }
   return alpha;
 }
 
@@ -431,7 +477,7 @@ static void thin_layer_momentum(real h0, const real* Hh, real* qx, real* qy) {
  * barely deeper than H0 and the C4 workload goes non-finite). */
 int orc_wetdry_elem(const orc_tables* T, real h0, const real* hv, real* ze, real* qx, real* qy) {
   const int ndof = T->ndof;
-  if (T->p == 2) {
+  if (T->p >= 2) {
     /* pre-step: full polynomial depth at the vertices, all edge points, all area points;
      * threshold H1 = 10 H0 so that the linear part below governs every thin element */
     const real h1 = RL(10.0) * h0;
@@ -456,7 +502,7 @@ int orc_wetdry_elem(const orc_tables* T, real h0, const real* hv, real* ze, real
       real hq = fma(hv[2], T->la[i][2], fma(hv[1], T->la[i][1], hv[0] * T->la[i][0]));
       if (z + hq <= h1) low = 1;
     }
-    if (low) for (int k = 3; k < 6; ++k) { ze[k] = RL(0.0); qx[k] = RL(0.0); qy[k] = RL(0.0); }
+    if (low) for (int k = 3; k < ndof; ++k) { ze[k] = RL(0.0); qx[k] = RL(0.0); qy[k] = RL(0.0); }
   }
   real zv[3], H[3];
   vertex_values(ze, zv);

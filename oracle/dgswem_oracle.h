@@ -32,12 +32,12 @@ typedef double real;
 #endif
 #define RL(x) ((real)(x))
 
-#define ORC_MAXDOF 6
-#define ORC_MAXQA 6
-#define ORC_MAXQE 3
+#define ORC_MAXDOF 10
+#define ORC_MAXQA 12
+#define ORC_MAXQE 4
 
 typedef struct {
-  int32_t p;          /* 1 or 2 */
+  int32_t p;          /* 1, 2 or 3 */
   int32_t rk_order;   /* 2: SSP(2,2), 3: SSP(3,3) */
   real g, cf, coriolis_f, h0_dry;
   int32_t limiter;    /* 0 off, 1 edge-neighbour Barth-Jespersen [R-7], 2 vertex-neighbourhood Barth-Jespersen [R-18] */

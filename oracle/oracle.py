@@ -23,7 +23,7 @@ REAL = C.c_float if F32 else C.c_double
 NP = np.float32 if F32 else np.float64
 LIB = HERE / ("liborc32.so" if F32 else "liborc.so")
 
-MAXDOF, MAXQA, MAXQE = 6, 6, 3
+MAXDOF, MAXQA, MAXQE = 10, 12, 4
 
 
 def build(force: bool = False) -> Path:
@@ -134,7 +134,7 @@ def lib():
 
 # ------------------------------------------------------------------ piece-level helpers
 def basis(lam0, lam1, lam2):
-    phi, d1, d2 = (np.zeros(6, dtype=NP) for _ in range(3))
+    phi, d1, d2 = (np.zeros(MAXDOF, dtype=NP) for _ in range(3))
     lib().orc_basis(lam0, lam1, lam2, _dp(phi), _dp(d1), _dp(d2))
     return phi, d1, d2
 

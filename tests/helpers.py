@@ -53,9 +53,9 @@ def small_mesh(nq=2, L=1000.0, jitter=0.25, seed=7, permute=True, ocean=False):
 
 
 # ----------------------------------------------------------------------- oracle-basis utilities
-def eval_basis(O, lam):
-    """phi[nq, 6] via the oracle's (separately pinned) basis."""
-    return np.array([O.basis(*l)[0] for l in lam])
+def eval_basis(O, lam, ndof=6):
+    """phi[nq, ndof] via the oracle's (separately pinned) basis (it evaluates all ten modes up to p = 3)."""
+    return np.array([O.basis(*l)[0] for l in lam])[:, :ndof]
 
 
 def l2_project(O, mesh, fn, p):
@@ -63,8 +63,8 @@ def l2_project(O, mesh, fn, p):
     onto the Dubiner basis, by high-order quadrature; M_k from the closed form."""
     ndof = (p + 1) * (p + 2) // 2
     lam, wt = tri_rule_bary(10)
-    phi = eval_basis(O, lam)[:, :ndof]
-    Mref = np.array([2.0, 1.0, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 9.0, 2.0 / 15.0])[:ndof]
+    phi = eval_basis(O, lam, 10)[:, :ndof]
+    Mref = np.array([2.0, 1.0, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 9.0, 2.0 / 15.0, 0.5, 1.0 / 6.0, 0.1, 1.0 / 14.0])[:ndof]
     xy, tri = mesh.xy, mesh.tri
     out = np.zeros((ndof, tri.shape[0]))
     for e, t in enumerate(tri):
@@ -138,7 +138,7 @@ def brute_force_rhs(O, mesh, bathy, p, ze, qx, qy, *, h0=1e-3, cf=0.0, fcor=0.0,
             n = np.array([ev[1], -ev[0]]) / Ln
             pts = X[a][None, :] + s_e[:, None] * ev[None, :]
             lam_own = np.zeros((len(s_e), 3)); lam_own[:, a] = 1 - s_e; lam_own[:, b] = s_e
-            ph_own = eval_basis(O, lam_own)[:, :ndof]
+            ph_own = eval_basis(O, lam_own, 10)[:, :ndof]
             wp = [ph_own @ W[c, :, e] for c in range(3)]
             hq_e = lam_own @ hv
             bc = mesh.edge_bc[d]
@@ -148,7 +148,7 @@ def brute_force_rhs(O, mesh, bathy, p, ze, qx, qy, *, h0=1e-3, cf=0.0, fcor=0.0,
                 T = np.array([[Xo[1][0] - Xo[0][0], Xo[2][0] - Xo[0][0]], [Xo[1][1] - Xo[0][1], Xo[2][1] - Xo[0][1]]])
                 l12 = np.linalg.solve(T, (pts - Xo[0]).T).T
                 lam_o = np.stack([1 - l12.sum(1), l12[:, 0], l12[:, 1]], 1)
-                ph_o = eval_basis(O, lam_o)[:, :ndof]
+                ph_o = eval_basis(O, lam_o, 10)[:, :ndof]
                 wm = [ph_o @ W[c, :, other] for c in range(3)]
             elif bc == 1:
                 qn = wp[1] * n[0] + wp[2] * n[1]

@@ -19,7 +19,7 @@ def make_oracle(O, mesh, bathy, **kw):
 
 
 # ------------------------------------------------------------------ (a) bottom friction
-@pytest.mark.parametrize("p", [1, 2])
+@pytest.mark.parametrize("p", [1, 2, 3])
 def test_friction_uniform_flow_closed_form(O, p):
     """Uniform flow (zeta, Qx, Qy) = const over a flat bottom: in an element without a wall edge the flux terms cancel
     (divergence theorem, exact quadrature of a constant), so d(mean Q)/dt is the source alone:
@@ -41,7 +41,7 @@ def test_friction_uniform_flow_closed_form(O, p):
     scale = max(abs(ex_x), abs(ex_y))
     # the edge and volume flux terms cancel to round-off of THEIR size, (g H^2/2) L/A ~ 30: absolute floor of the comparison
     lfmax = np.abs(o.get_geometry()[2]).max()
-    cancel = 2e-15 * (G * H * H) * lfmax
+    cancel = 2e-15 * (G * H * H) * lfmax * (1 if p < 3 else 3)     # (inverse masses up to 14 and 12 + 12 points at p = 3)
     assert cancel < 1e-9 * scale
     assert np.abs(r[1, 0, interior] - ex_x).max() <= 1e-13 * scale + cancel
     assert np.abs(r[2, 0, interior] - ex_y).max() <= 1e-13 * scale + cancel
@@ -77,7 +77,7 @@ def test_friction_off_in_dry_flagged_elements_and_cf_zero(O):
     assert np.abs(r0[2, 0, interior] + 2e-3 * 3.0).max() <= 1e-12
 
 
-@pytest.mark.parametrize("p", [1, 2])
+@pytest.mark.parametrize("p", [1, 2, 3])
 def test_bruteforce_with_strong_friction(O, p):
     """Brute-force weak form (dense mass solve, 12x12 rule) with C_f = 0.25, where friction is the same size as the
     pressure terms: the oracle agrees within its quadrature error, and the same comparison against a friction-free
@@ -148,7 +148,7 @@ def _post_case(O, p=1, seed=21):
     return mesh, bathy, st
 
 
-@pytest.mark.parametrize("p", [1, 2])
+@pytest.mark.parametrize("p", [1, 2, 3])
 def test_limiter_all_neighbour_wiring_wet_gate_and_means(O, p):
     """limiter_all on a hand-built 8-element state: alpha of every (element, variable) recomputed here from the mesh's
     own edge tables and the pre-limit means; an element flagged dry must be skipped (its slopes survive); means are
@@ -388,3 +388,40 @@ def test_p2_prestep_exact_threshold_is_inclusive(O):
             pytest.skip("vertex value not exactly representable through the modal solve")
         wet, z2, _, _ = O.wetdry_elem(2, h0, hv, ze, np.zeros(6), np.zeros(6))
         assert (not z2[3:].any()) == zeroed
+
+
+def test_p3_wetdry_prestep_uses_the_p3_point_sets_and_clears_all_higher_modes(O):
+    """The same pre-step at p = 3: 3 vertices + 3 x 4 edge points + 12 area points of the p = 3 tables; modes 3-9 of all
+    variables are cleared iff the full cubic depth is <= H1 = 10 H0 at one of them.  The state has a mean and one cubic
+    mode (phi_30) only, scaled so that exactly one point is low."""
+    h0 = 1e-3
+    hv = np.array([1.0, 1.0, 1.0])
+    T = O.tables(3)
+    la, el = T.np("la")[:T.nqa], T.np("elam")[:T.nqe]
+    assert T.nqa == 12 and T.nqe == 4 and T.ndof == 10
+    pts = [(1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, 0.0, 1.0)] + [tuple(x) for x in la]
+    for l in range(3):
+        a, b = (l + 1) % 3, (l + 2) % 3
+        for j in range(4):
+            lam = [0.0, 0.0, 0.0]; lam[a] = el[j][0]; lam[b] = el[j][1]
+            pts.append(tuple(lam))
+    pts = np.array(pts)
+    phi = eval_basis(O, pts, 10)
+    f9 = np.sort(phi[:, 9])
+    gap = f9[1] - f9[0]
+    assert gap > 1e-3
+    c = 0.2 / gap
+    q10 = np.full(10, 0.2); q10[0] = 1.0
+    for hmin, zeroed in ((5 * h0, True), (11 * h0, False)):
+        ze = np.zeros(10); ze[9] = c; ze[0] = hmin - 1.0 - c * f9[0]
+        depth = phi @ ze + 1.0
+        assert abs(depth.min() - hmin) < 1e-12 and np.sort(depth)[1] > 100 * h0
+        wet, z2, x2, y2 = O.wetdry_elem(3, h0, hv, ze, q10, q10)
+        if zeroed:
+            assert not z2[3:].any() and not x2[3:].any() and not y2[3:].any()
+        else:
+            assert np.array_equal(z2, ze) and np.array_equal(x2, q10) and np.array_equal(y2, q10)
+    # the p = 3 limiter clears modes 3-9 of a limited variable and leaves the mean
+    w = np.array([1.0, 0.5, 0.2, 0.1, 0.1, 0.1, 0.05, 0.05, 0.05, 0.05])
+    alpha, w2 = O.limit_var(3, w, [1.1, 0.9, 1.0], [1, 1, 1])
+    assert 0.0 <= alpha < 1.0 and w2[0] == 1.0 and not w2[3:].any() and np.allclose(w2[1:3], alpha * w[1:3], rtol=1e-15)

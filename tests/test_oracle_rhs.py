@@ -79,7 +79,7 @@ def test_depth_floor_in_flux(O):
 
 
 # ------------------------------------------------------------------ RHS invariants
-@pytest.mark.parametrize("p", [1, 2])
+@pytest.mark.parametrize("p", [1, 2, 3])
 def test_constant_state_flat_bottom_rhs_zero_in_interior(O, p):
     """A constant state (zeta, Qx, Qy) on a flat bottom is preserved by every element that has
     no wall edge (walls reflect the momentum)."""
@@ -96,7 +96,7 @@ def test_constant_state_flat_bottom_rhs_zero_in_interior(O, p):
     assert max(np.abs(r[c][:, has_wall]).max() for c in (1, 2)) > 1e-3     # walls do act
 
 
-@pytest.mark.parametrize("p", [1, 2])
+@pytest.mark.parametrize("p", [1, 2, 3])
 def test_lake_at_rest_variable_bathymetry(O, p):
     """Well-balancedness: zeta = const, Q = 0 over variable continuous piecewise-linear h_b
     gives RHS = 0 (to round-off relative to the size of the cancelling terms) and the state
@@ -125,7 +125,7 @@ def test_lake_at_rest_with_ocean_boundary_at_same_level(O):
         assert np.abs(r[c]).max() <= 1e-13 * max(s[c].max(), 1.0)
 
 
-@pytest.mark.parametrize("p", [1, 2])
+@pytest.mark.parametrize("p", [1, 2, 3])
 def test_rotation_equivariance(O, p):
     """Rotating mesh and momentum by 90 degrees rotates the RHS: (x,y)->(-y,x), (Qx,Qy)->(-Qy,Qx)."""
     mesh = small_mesh(nq=3, permute=False)
@@ -167,9 +167,12 @@ def _smooth_state(O, mesh, p, kind, seed=3):
         if p == 1:
             fx = lambda x, y: 1.0 + 2e-3 * x - 1e-3 * y
             fy = lambda x, y: -0.5 + 1e-3 * x + 3e-3 * y
-        else:
+        elif p == 2:
             fx = lambda x, y: 1.0 + 2e-3 * x - 1e-3 * y + 1e-6 * x * y - 2e-6 * x * x
             fy = lambda x, y: -0.5 + 1e-3 * x + 3e-3 * y + 2e-6 * y * y - 1e-6 * x * y
+        else:
+            fx = lambda x, y: 1.0 + 2e-3 * x - 1e-3 * y + 1e-6 * x * y - 2e-6 * x * x + 3e-9 * x * x * x - 2e-9 * x * y * y
+            fy = lambda x, y: -0.5 + 1e-3 * x + 3e-3 * y + 2e-6 * y * y - 1e-6 * x * y - 1e-9 * y * y * y + 4e-9 * x * x * y
         return [l2_project(O, mesh, f, p) for f in (fz, fx, fy)]
     # generic: discontinuous, all three variables, mild amplitude
     ndof = (p + 1) * (p + 2) // 2
@@ -181,7 +184,7 @@ def _smooth_state(O, mesh, p, kind, seed=3):
     return W
 
 
-@pytest.mark.parametrize("p", [1, 2])
+@pytest.mark.parametrize("p", [1, 2, 3])
 @pytest.mark.parametrize("which", ["two", "eight"])
 def test_bruteforce_polynomial_exact_case(O, p, which):
     """Where the oracle's quadrature is exact, its RHS equals the weak form (3) integrated
@@ -198,7 +201,7 @@ def test_bruteforce_polynomial_exact_case(O, p, which):
     assert np.abs(r - bf).max() < 1e-11 * max(1.0, np.abs(bf).max())
 
 
-@pytest.mark.parametrize("p", [1, 2])
+@pytest.mark.parametrize("p", [1, 2, 3])
 def test_bruteforce_generic_state_within_quadrature_error(O, p):
     """Discontinuous state with momentum, friction, Coriolis, an ocean boundary: the oracle
     differs from the exactly integrated weak form only by its quadrature error (non-polynomial
@@ -219,12 +222,13 @@ def test_bruteforce_generic_state_within_quadrature_error(O, p):
         assert np.abs(r[c] - bf[c]).max() < (2e-3 if p == 1 else 2e-4) * sc
 
 
-@pytest.mark.parametrize("p", [1, 2])
+@pytest.mark.parametrize("p", [1, 2, 3])
 def test_bruteforce_continuity_row_exact_with_full_degree_momentum(O, p):
     mesh = small_mesh(nq=2, L=1000.0)
     bathy = np.full(mesh.n_nodes, 10.0)
     W = _smooth_state(O, mesh, p, "continuity_exact")
-    assert p == 1 or np.abs(W[1][3:]).max() > 1e-3          # quadratic state modes are exercised
+    assert p == 1 or np.abs(W[1][3:6]).max() > 1e-3         # quadratic state modes are exercised
+    assert p < 3 or np.abs(W[1][6:]).min(axis=1).max() > 0 and np.abs(W[1][6:]).max() > 1e-3   # ... and the cubic ones
     o = make_oracle(O, mesh, bathy, p=p)
     o.set_state(0.0, *W)
     r = np.stack(o.eval_rhs())

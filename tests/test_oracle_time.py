@@ -146,25 +146,26 @@ def _seiche(O, nq, p, amp=1e-4, t_end=300.0):
     t, ze, qx, qy = o.get_state()
     zex = l2_project(O, mesh, lambda x, y: amp * np.cos(k * x) * math.cos(om * t), p)
     qex = l2_project(O, mesh, lambda x, y: amp * math.sqrt(G * H) * np.sin(k * x) * math.sin(om * t), p)
-    Mref = np.array([2.0, 1.0, 1 / 3, 2 / 3, 2 / 9, 2 / 15])[:ze.shape[0], None]
+    Mref = np.array([2.0, 1.0, 1 / 3, 2 / 3, 2 / 9, 2 / 15, 1 / 2, 1 / 6, 1 / 10, 1 / 14])[:ze.shape[0], None]
     l2 = lambda a: math.sqrt(float((a * a * Mref).sum()))
     return l2(ze - zex) / l2(zex), l2(qx - qex) / l2(qex), om
 
 
-@pytest.mark.parametrize("p", [1, 2])
+@pytest.mark.parametrize("p", [1, 2, 3])
 def test_seiche_convergence_order(O, p):
     """Small-amplitude standing wave in the closed flat 10 km basin (linear theory: period
     2L/sqrt(gH) = 2019 s): the L2 error of zeta and Qx converges with order ~ p+1."""
-    nqs = (8, 16, 32) if p == 1 else (4, 8, 16)
+    nqs = (8, 16, 32) if p == 1 else (4, 8, 16) if p == 2 else (3, 6, 12)
     ez, eq = [], []
     for nq in nqs:
-        a, b, om = _seiche(O, nq, p)
+        # (p = 3 reaches the linear theory's own error, O(amp / H) relative, on these meshes: a smaller wave)
+        a, b, om = _seiche(O, nq, p, amp=1e-4 if p < 3 else 1e-7)
         ez.append(a); eq.append(b)
     assert abs(2 * math.pi / om - 2019.0) < 1.0
     for e in (ez, eq):
         o1, o2 = math.log2(e[0] / e[1]), math.log2(e[1] / e[2])
         assert o2 > p + 0.6 and o1 > p + 0.3, (p, e)
-    assert ez[-1] < (2e-3 if p == 1 else 2e-4)
+    assert ez[-1] < (2e-3 if p == 1 else 2e-4 if p == 2 else 1e-5)
 
 
 def test_seiche_period(O):
