@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- fp64 DOF-updates/s per RK stage of the DG-SWEM hot path on B200 (BASELINE.json metric).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C1|C2p1|C2p2|C4|C5|H] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C1|C2p1|C2p2|C2p3|C4|C5|C5p3|H] [--impl ours|reference]
 
 A "step" is one full explicit time step of the workload: WIND (if on) and, per RK stage, EDGE ->
 GATHER+AREA+RK(+wet/dry) -> (limiter+wet/dry), i.e. every row of SURVEY.md section 8(a).  Default
@@ -47,6 +47,10 @@ def make_workload(name: str, scale: float = 1.0):
         return c2(nq=max(8, int(512 * scale)), p=1)
     if name == "C2p2":
         return c2(nq=max(8, int(512 * scale)), p=2)
+    if name == "C2p3":
+        return c2(nq=max(8, int(512 * scale)), p=3)
+    if name == "C5p3":      # the C5 mesh and recipe at p = 3
+        return c5(nn=max(20, int(round(1323 * scale))), p=3)
     if name == "C4":
         return c4(nqx=max(16, int(1024 * scale)), nqy=max(8, int(512 * scale)))
     if name == "C5":
@@ -96,7 +100,7 @@ def alg_bytes(w, kind: str, stage_first: bool, fused: bool = False, rb: int = 8)
         # what a write-if-changed pass must READ: the state rows the two steps look at (p = 2: not the quadratic momentum
         # modes), neighbour table, the neighbours' means (once per element), vertex bathymetry, wet flag.  What it writes
         # depends on the data (only values a step changed) and is NOT credited: the fraction is a lower bound.
-        rows = 9 if w.params["p"] == 1 else 12
+        rows = 9 if w.params["p"] == 1 else w.ndof + 6
         return ne * (rows * rb + 12 + 3 * rb + 3 * rb + 1)
     if kind == "wind":
         return nn * 4 * rb

@@ -11,7 +11,7 @@
  *     the call and never retained (only exception: the halo buffers of dgswem_halo_pack / _unpack when
  *     flagged buf_on_device).  All other device memory is owned by the handle.
  *   - element arrays are [ndof][n_elem] doubles, mode index slow, in the CALLER's element order
- *     (any internal reordering is invisible); ndof = (p+1)(p+2)/2; mode order 00,01,10,(02,11,20).
+ *     (any internal reordering is invisible); ndof = (p+1)(p+2)/2; mode order 00,01,10,(02,11,20),(03,12,21,30).
  *   - triangles are counter-clockwise, 0-based; local edge l joins local vertices (l+1)%3 -> (l+2)%3.
  *   - return value 0 = success; <0 = error (DGSWEM_E_*), text via dgswem_last_error().
  *   - calls on one handle must not be concurrent.  Work is enqueued on the handle's stream;
@@ -38,7 +38,8 @@ extern "C" {
 typedef struct dgswem dgswem_t;   /* opaque */
 
 typedef struct {
-  int32_t p;            /* polynomial degree, 1 or 2 (paper runs p=1)              */
+  int32_t p;            /* polynomial degree 1, 2 or 3 (paper runs p=1; p = 3 runs the edge + element
+                           kernel pair only)                                                      */
   int32_t rk_order;     /* order of the SSP Runge-Kutta scheme, 2 or 3 (R-2); see rk_stages */
   double  g;            /* gravity, e.g. 9.81                                                    */
   double  cf;           /* quadratic bottom friction coefficient, 0 = off (R-6)        */

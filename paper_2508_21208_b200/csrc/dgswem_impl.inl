@@ -16,7 +16,9 @@ constexpr real kG_edge2 = RL(0.77459666924148338);   // sqrt(3/5)
 inline long long round_up(long long n, long long m) { return (n + m - 1) / m * m; }
 
 // ------------------------------------------------------------------------------------ tables
-// Dubiner basis (eq. (4)), mode order 00,01,10,02,11,20, from barycentrics.
+// Dubiner basis (eq. (4)), mode order 00,01,10, 02,11,20, 03,12,21,30, from barycentrics:
+// phi_ij = A_i B_j^(2i+1)(xi_2), A_i = P_i(eta_1) s^i in the collapsed coordinate (A_1 = a = xi_1 + (1 + xi_2)/2,
+// A_2 = (3 a^2 - s^2)/2, A_3 = (5 a^3 - 3 a s^2)/2, s = (1 - xi_2)/2), B_j^(alpha) = Jacobi P_j^(alpha,0).
 void dubiner(real l1, real l2, real* phi, real* g1, real* g2) {
   const real xi1 = RL(2.0) * l1 - RL(1.0);
   const real xi2 = RL(2.0) * l2 - RL(1.0);
@@ -34,17 +36,54 @@ void dubiner(real l1, real l2, real* phi, real* g1, real* g2) {
   g1[3] = RL(0.0);           g2[3] = RL(5.0) * xi2 + RL(1.0);
   g1[4] = r;             g2[4] = RL(0.5) * r + RL(2.5) * phi[2];
   g1[5] = RL(3.0) * phi[2];  g2[5] = RL(0.5) * (RL(3.0) * phi[2] + s);
+  {   // p = 3
+    const real y = xi2, a = phi[2];
+    const real b3 = RL(0.125) * ((((RL(35.0) * y) * y) * y + (RL(15.0) * y) * y) - RL(15.0) * y - RL(3.0));
+    const real db3 = RL(0.125) * (((RL(105.0) * y) * y + RL(30.0) * y) - RL(15.0));
+    const real b2 = RL(0.25) * (((RL(21.0) * y) * y + RL(18.0) * y) + RL(1.0));
+    const real db2 = RL(0.25) * (RL(42.0) * y + RL(18.0));
+    const real b1 = RL(0.5) * (RL(7.0) * y + RL(5.0));
+    const real a2 = phi[5];
+    const real da2x = g1[5], da2y = g2[5];
+    const real a3 = RL(0.5) * (((RL(5.0) * a) * a) * a - ((RL(3.0) * a) * s) * s);
+    const real da3x = RL(0.5) * ((RL(15.0) * a) * a - (RL(3.0) * s) * s);
+    const real da3y = RL(0.5) * (((RL(7.5) * a) * a - (RL(1.5) * s) * s) + (RL(3.0) * a) * s);
+    phi[6] = b3;       g1[6] = RL(0.0);    g2[6] = db3;
+    phi[7] = a * b2;   g1[7] = b2;         g2[7] = RL(0.5) * b2 + a * db2;
+    phi[8] = a2 * b1;  g1[8] = da2x * b1;  g2[8] = da2y * b1 + RL(3.5) * a2;
+    phi[9] = a3;       g1[9] = da3x;       g2[9] = da3y;
+  }
 }
 
 void make_tables(int p, Tables& T) {
   std::memset(&T, 0, sizeof(T));
-  const int ndof = (p + 1) * (p + 2) / 2, nqe = p + 1, nqa = (p == 1) ? 3 : 6;
-  real ge[3] = {0, 0, 0}, we[3] = {0, 0, 0}, wa[6] = {0, 0, 0, 0, 0, 0};
+  const int ndof = (p + 1) * (p + 2) / 2, nqe = p + 1, nqa = (p == 1) ? 3 : (p == 2) ? 6 : 12;
+  real ge[4] = {0, 0, 0, 0}, we[4] = {0, 0, 0, 0}, wa[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
   if (p == 1) {
     ge[0] = -kG_edge1; ge[1] = kG_edge1; we[0] = RL(1.0); we[1] = RL(1.0);
     for (int i = 0; i < 3; ++i) {
       for (int v = 0; v < 3; ++v) T.la[i][v] = (v == i) ? RL(2.0) / RL(3.0) : RL(1.0) / RL(6.0);
       wa[i] = RL(2.0) / RL(3.0);
+    }
+  } else if (p == 3) {   // 4-point Gauss-Legendre; the classical 12-point degree-6 rule (two 3-point orbits, one 6-point orbit)
+    ge[0] = -RL(0.86113631159405258); ge[1] = -RL(0.33998104358485626); ge[2] = RL(0.33998104358485626); ge[3] = RL(0.86113631159405258);
+    we[0] = RL(0.34785484513745386); we[1] = RL(0.65214515486254614); we[2] = RL(0.65214515486254614); we[3] = RL(0.34785484513745386);
+    const real a1 = RL(0.249286745170910), w1 = RL(0.116786275726379);
+    const real a2 = RL(0.063089014491502), w2 = RL(0.050844906370207);
+    const real b3 = RL(0.053145049844817), c3 = RL(0.310352451033784), w3 = RL(0.082851075618374);
+    for (int i = 0; i < 3; ++i) {
+      for (int v = 0; v < 3; ++v) {
+        T.la[i][v] = (v == i) ? RL(1.0) - RL(2.0) * a1 : a1;
+        T.la[3 + i][v] = (v == i) ? RL(1.0) - RL(2.0) * a2 : a2;
+      }
+      wa[i] = RL(2.0) * w1;
+      wa[3 + i] = RL(2.0) * w2;
+    }
+    static const int perm[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
+    const real tri3[3] = {b3, c3, (RL(1.0) - b3) - c3};
+    for (int q = 0; q < 6; ++q) {
+      for (int v = 0; v < 3; ++v) T.la[6 + q][v] = tri3[perm[q][v]];
+      wa[6 + q] = RL(2.0) * w3;
     }
   } else {
     ge[0] = -kG_edge2; ge[1] = RL(0.0); ge[2] = kG_edge2;
@@ -60,10 +99,11 @@ void make_tables(int p, Tables& T) {
       wa[3 + i] = RL(2.0) * w2;
     }
   }
-  const real mass[6] = {RL(2.0), RL(1.0), RL(1.0) / RL(3.0), RL(2.0) / RL(3.0), RL(2.0) / RL(9.0), RL(2.0) / RL(15.0)};
-  real invM[6];
-  for (int k = 0; k < 6; ++k) invM[k] = RL(1.0) / mass[k];
-  real phi[6], g1[6], g2[6];
+  const real mass[10] = {RL(2.0), RL(1.0), RL(1.0) / RL(3.0), RL(2.0) / RL(3.0), RL(2.0) / RL(9.0), RL(2.0) / RL(15.0),
+                         RL(0.5), RL(1.0) / RL(6.0), RL(0.1), RL(1.0) / RL(14.0)};
+  real invM[10];
+  for (int k = 0; k < 10; ++k) invM[k] = RL(1.0) / mass[k];
+  real phi[10], g1[10], g2[10];
   for (int i = 0; i < nqa; ++i) {
     dubiner(T.la[i][1], T.la[i][2], phi, g1, g2);
     for (int k = 0; k < ndof; ++k) {
@@ -181,7 +221,7 @@ struct Handle : ::dgswem {
   bool have_hooks = false;
   std::vector<void*> allocs;
   long long launches = 0;
-  int res_edge[2] = {0, 0};   // resident grid of the persistent edge kernel [p-1]
+  int res_edge[3] = {0, 0, 0};   // resident grid of the persistent edge kernel [p-1]
   int res_limwd = 0;          // same for the limiter kernel of this handle's p
 
   // optional per-kernel timing (dgswem_profile): CUDA events recorded on the stream around every launch
@@ -626,10 +666,15 @@ int run_stage_rhs(Handle* h, const real* win, const real* w0, real* wout, double
                   double t_stage, int stage, int part = 0) {
   const bool lim = h->prm.limiter != 0;
   const bool wd = h->prm.wetdry != 0;
-  int rc;
-  if (h->fused) {
-    rc = launch_stage<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim, scal(h, stage, tide_value(h, t_stage)), part);
-  } else {
+  int rc = 0;
+  bool done = false;
+  if constexpr (P <= 2) {
+    if (h->fused) {
+      rc = launch_stage<P, MODE_UPDATE>(h, win, w0, wout, dt, a, b, first, wd && !lim, lim, scal(h, stage, tide_value(h, t_stage)), part);
+      done = true;
+    }
+  }
+  if (!done) {
     if (part == 2) return 0;   // the edge + element pair does the whole stage in part 1
     rc = launch_edge<P>(h, win, scal(h, stage, tide_value(h, t_stage)));
     if (rc) return rc;
@@ -836,7 +881,7 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
     return bail(h->fail(DGSWEM_E_ARG, "NULL argument"));
   if (n_nodes < 3 || n_elem < 1 || n_edge < 3 || n_elem > 0x1fffffff || n_edge > 0x7ffffff0 || n_nodes > 0x7ffffff0)
     return bail(h->fail(DGSWEM_E_ARG, "bad sizes"));
-  if (prm->p != 1 && prm->p != 2) return bail(h->fail(DGSWEM_E_ARG, "p must be 1 or 2"));
+  if (prm->p < 1 || prm->p > 3) return bail(h->fail(DGSWEM_E_ARG, "p must be 1, 2 or 3"));
   if (!rk_get(prm->rk_order, prm->rk_stages, h->rk))
     return bail(h->fail(DGSWEM_E_ARG, "(rk_order, rk_stages) must be (2, 0|2), (3, 0|3), (2, 3), (2, 4) or (3, 4)"));
   if (prm->reorder < 0 || prm->reorder > 2) return bail(h->fail(DGSWEM_E_ARG, "reorder must be 0 (none), 1 (Hilbert curve) or 2 (reverse Cuthill-McKee)"));
@@ -848,7 +893,7 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
   if (!(prm->h0_dry >= 1e-100) || !(prm->g * prm->h0_dry >= 1e-100) || !(prm->g <= 1e100) || !(prm->h0_dry <= 1e100))
     return bail(h->fail(DGSWEM_E_ARG, "need 1e-100 <= h0_dry <= 1e100, g <= 1e100 and g*h0_dry >= 1e-100"));
   h->prm = *prm;
-  h->ndof = (prm->p + 1) * (prm->p + 2) / 2; h->nqe = prm->p + 1; h->nqa = prm->p == 1 ? 3 : 6; h->nstage = h->rk.ns;
+  h->ndof = (prm->p + 1) * (prm->p + 2) / 2; h->nqe = prm->p + 1; h->nqa = prm->p == 1 ? 3 : prm->p == 2 ? 6 : 12; h->nstage = h->rk.ns;
   h->nn = n_nodes; h->ne = n_elem; h->nd = n_edge;
   h->ld = round_up(n_elem, 256); h->ldd = round_up(n_edge, 256); h->ldn = round_up(n_nodes, 64);
   int rc = validate_mesh(h, n_nodes, xy, n_elem, tri, n_edge, edge_elem, edge_local, edge_bc, elem_edge);
@@ -870,25 +915,32 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
   auto body = [&]() -> int {
     // ---- tables to constant memory (both degrees; identical for every handle)
     Tables T1, T2;
-    make_tables(1, T1); make_tables(2, T2);
+    Tables T3;
+    make_tables(1, T1); make_tables(2, T2); make_tables(3, T3);
+    CK(cudaMemcpyToSymbolAsync(c_tab3, &T3, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
     CK(cudaMemcpyToSymbolAsync(c_tab1, &T1, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
     CK(cudaMemcpyToSymbolAsync(c_tab2, &T2, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
     CK(cudaStreamSynchronize(h->stream));
 
     h->res_edge[0] = resident_ctas(k_edge_pipe<1>, DGK_EDGE_THREADS, 0, prm->device);
     h->res_edge[1] = resident_ctas(k_edge_pipe<2>, DGK_EDGE_THREADS, 0, prm->device);
+    h->res_edge[2] = resident_ctas(k_edge_pipe<3>, DGK_EDGE_THREADS, 0, prm->device);
     // tuning / test knob: DGSWEM_PERSISTENT_CTAS=n caps the persistent grid at n CTAs (so that small
     // meshes walk several tiles per CTA); 0 switches the persistent kernel off
     CK(cudaFuncSetAttribute(k_limwd_tma<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<1>::kSmem));
     CK(cudaFuncSetAttribute(k_limwd_tma<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<2>::kSmem));
     CK(cudaFuncSetAttribute(k_limwd_tma<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<1>::kSmem));
     CK(cudaFuncSetAttribute(k_limwd_tma<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<2>::kSmem));
+    CK(cudaFuncSetAttribute(k_limwd_tma<3, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<3>::kSmem));
+    CK(cudaFuncSetAttribute(k_limwd_tma<3, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LimTile<3>::kSmem));
     if (prm->limiter == 2)
       h->res_limwd = prm->p == 1 ? resident_ctas(k_limwd_tma<1, 2>, 128, LimTile<1>::kSmem, prm->device)
-                                 : resident_ctas(k_limwd_tma<2, 2>, 128, LimTile<2>::kSmem, prm->device);
+                   : prm->p == 2 ? resident_ctas(k_limwd_tma<2, 2>, 128, LimTile<2>::kSmem, prm->device)
+                                 : resident_ctas(k_limwd_tma<3, 2>, 128, LimTile<3>::kSmem, prm->device);
     else
       h->res_limwd = prm->p == 1 ? resident_ctas(k_limwd_tma<1, 1>, 128, LimTile<1>::kSmem, prm->device)
-                                 : resident_ctas(k_limwd_tma<2, 1>, 128, LimTile<2>::kSmem, prm->device);
+                   : prm->p == 2 ? resident_ctas(k_limwd_tma<2, 1>, 128, LimTile<2>::kSmem, prm->device)
+                                 : resident_ctas(k_limwd_tma<3, 1>, 128, LimTile<3>::kSmem, prm->device);
     if (const char* env = std::getenv("DGSWEM_PERSISTENT_CTAS")) {
       const int cap = std::atoi(env);
 
@@ -904,6 +956,7 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
     h->pf_dist = ((size_t)3 * h->ndof * h->ld * sizeof(real) > ((size_t)100 << 20)) ? 200 : 0;
     if (const char* env = std::getenv("DGSWEM_PF_DIST")) h->pf_dist = std::max(0, std::atoi(env));
     if (const char* env = std::getenv("DGSWEM_FUSED")) { h->fused = std::atoi(env) != 0; h->tiled = std::atoi(env) == 2; h->staged = std::atoi(env) == 3; }
+    if (prm->p == 3) { h->fused = false; h->tiled = false; h->staged = false; }   // p = 3: the edge + element pair only (the element-centric forms would need > 255 registers)
 
     const long long ne = h->ne, nd = h->nd, nn = h->nn, ld = h->ld, ldd = h->ldd, ldn = h->ldn;
     // ---- renumbering (internal only): perm_e[new] = old
@@ -1214,6 +1267,7 @@ int api_set_state(Handle* h, double t, const double* ze, const double* qx, const
   CKL("k_fill_bytes");
   if (h->prm.wetdry) {
     if (h->prm.p == 1) k_wetdry_only<1><<<grid_for(h->ne, 128), 128, 0, h->stream>>>(h->W[0], h->hv, h->wet, (int)h->ne, h->ld, h->prm.h0_dry);
+    else if (h->prm.p == 3) k_wetdry_only<3><<<grid_for(h->ne, 128), 128, 0, h->stream>>>(h->W[0], h->hv, h->wet, (int)h->ne, h->ld, h->prm.h0_dry);
     else k_wetdry_only<2><<<grid_for(h->ne, 128), 128, 0, h->stream>>>(h->W[0], h->hv, h->wet, (int)h->ne, h->ld, h->prm.h0_dry);
     CKL("k_wetdry_only");
   }
@@ -1263,7 +1317,7 @@ int api_step(Handle* h, int64_t nsteps, double dt) {
   if (nsteps < 0 || !(dt > 0.0)) return h->fail(DGSWEM_E_ARG, "need nsteps >= 0 and dt > 0");
   if (h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a stage-granular step is in progress (dgswem_end_step)");
   CK(cudaSetDevice(h->prm.device));
-  return h->prm.p == 1 ? run_steps<1>(h, nsteps, dt) : run_steps<2>(h, nsteps, dt);
+  return h->prm.p == 1 ? run_steps<1>(h, nsteps, dt) : h->prm.p == 2 ? run_steps<2>(h, nsteps, dt) : run_steps<3>(h, nsteps, dt);
 }
 
 // ---- stage-granular stepping + halo lists: the building blocks of a domain-decomposed run
@@ -1287,7 +1341,8 @@ int api_stage_rhs(Handle* h, int s, int part) {
   const StageBufs B = stage_bufs(h, s);
   const double ts = h->t + B.c * h->step_dt;
   const int rc = h->prm.p == 1 ? run_stage_rhs<1>(h, B.win, B.w0, B.wout, B.beta * h->step_dt, B.a, B.b, B.first, ts, s, part)
-                               : run_stage_rhs<2>(h, B.win, B.w0, B.wout, B.beta * h->step_dt, B.a, B.b, B.first, ts, s, part);
+               : h->prm.p == 2 ? run_stage_rhs<2>(h, B.win, B.w0, B.wout, B.beta * h->step_dt, B.a, B.b, B.first, ts, s, part)
+                               : run_stage_rhs<3>(h, B.win, B.w0, B.wout, B.beta * h->step_dt, B.a, B.b, B.first, ts, s, part);
   if (rc == 0) h->last_out = B.wout;
   return rc;
 }
@@ -1299,7 +1354,7 @@ int api_stage_limit(Handle* h, int s) {
   if (h->prm.limiter == 0) return DGSWEM_OK;
   CK(cudaSetDevice(h->prm.device));
   const StageBufs B = stage_bufs(h, s);
-  return h->prm.p == 1 ? launch_limwd<1>(h, B.wout) : launch_limwd<2>(h, B.wout);
+  return h->prm.p == 1 ? launch_limwd<1>(h, B.wout) : h->prm.p == 2 ? launch_limwd<2>(h, B.wout) : launch_limwd<3>(h, B.wout);
 }
 
 int api_end_step(Handle* h) {
@@ -1411,9 +1466,12 @@ int api_eval_rhs(Handle* h, double* rze, double* rqx, double* rqy) {
   } else if (h->prm.p == 1) {
     if ((rc = launch_edge<1>(h, h->W[0], scal(h, 0, tide_value(h, h->t))))) return rc;
     if ((rc = launch_elem<1, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, RL(0.0), RL(1.0), 1, false, false))) return rc;
-  } else {
+  } else if (h->prm.p == 2) {
     if ((rc = launch_edge<2>(h, h->W[0], scal(h, 0, tide_value(h, h->t))))) return rc;
     if ((rc = launch_elem<2, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, RL(0.0), RL(1.0), 1, false, false))) return rc;
+  } else {
+    if ((rc = launch_edge<3>(h, h->W[0], scal(h, 0, tide_value(h, h->t))))) return rc;
+    if ((rc = launch_elem<3, MODE_RHS>(h, h->W[0], h->W[0], rbuf, 0.0, RL(0.0), RL(1.0), 1, false, false))) return rc;
   }
   k_tiled_to_rows<<<dim3(grid_for(h->ne, 256), 3 * h->ndof), 256, 0, h->stream>>>(h->stage_buf, h->ld, rbuf, h->inv_e, (int)h->ne, 3 * h->ndof);
   CKL("k_tiled_to_rows");
@@ -1433,7 +1491,8 @@ int api_get_flux(Handle* h, double* flux) {
   if (h->fused && h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a stage-granular step is in progress");
   CK(cudaSetDevice(h->prm.device));
   if (h->fused) {   // the element-centric stage kernel keeps no flux buffer: evaluate A1 on the current state
-    int rc = h->prm.p == 1 ? launch_edge<1>(h, h->W[0], scal(h, 0, tide_value(h, h->t))) : launch_edge<2>(h, h->W[0], scal(h, 0, tide_value(h, h->t)));
+    int rc = h->prm.p == 1 ? launch_edge<1>(h, h->W[0], scal(h, 0, tide_value(h, h->t))) : h->prm.p == 2 ? launch_edge<2>(h, h->W[0], scal(h, 0, tide_value(h, h->t)))
+                           : launch_edge<3>(h, h->W[0], scal(h, 0, tide_value(h, h->t)));
     if (rc) return rc;
   }
   // internal edge order and working precision -> caller's order, binary64
@@ -1491,6 +1550,7 @@ int api_get_nodal(Handle* h, double* zn, double* qxn, double* qyn) {
   double* out = h->stage_buf;   // [3][ldn] (3 * ldn <= the state-sized staging buffer: n_nodes < n_elem + 3 for any triangulation with a boundary)
   if ((size_t)3 * h->ldn * sizeof(double) > h->stage_bytes) return h->fail(DGSWEM_E_ARG, "nodal output needs n_nodes <= ndof * n_elem");
   if (h->prm.p == 1) k_nodal<1><<<grid_for(h->nn, 256), 256, 0, h->stream>>>(out, h->ldn, h->W[0], h->node_ptr, h->node_ev, (int)h->nn);
+  else if (h->prm.p == 3) k_nodal<3><<<grid_for(h->nn, 256), 256, 0, h->stream>>>(out, h->ldn, h->W[0], h->node_ptr, h->node_ev, (int)h->nn);
   else k_nodal<2><<<grid_for(h->nn, 256), 256, 0, h->stream>>>(out, h->ldn, h->W[0], h->node_ptr, h->node_ev, (int)h->nn);
   CKL("k_nodal");
   double* dst[3] = {zn, qxn, qyn};

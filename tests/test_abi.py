@@ -100,7 +100,7 @@ def test_create_validates_arguments_and_mesh_on_the_host(lib):
     from workloads import c1
     w = c1(nq=4)
     m = w.mesh
-    for key, val in (("p", 3), ("rk_order", 4), ("rk_stages", 5), ("rk_stages", 1), ("reorder", 3), ("h0_dry", 0.0), ("h0_dry", 1e-200), ("g", -9.81), ("cf", -1.0)):
+    for key, val in (("p", 4), ("p", 0), ("rk_order", 4), ("rk_stages", 5), ("rk_stages", 1), ("reorder", 3), ("h0_dry", 0.0), ("h0_dry", 1e-200), ("g", -9.81), ("cf", -1.0)):
         bad = dict(w.params); bad[key] = val
         rc, msg = _raw_create(lib, w, params=bad)
         assert rc == -1, (key, val, rc, msg)

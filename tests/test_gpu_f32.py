@@ -47,6 +47,8 @@ RECIPES = {
     "c1": lambda: c1(),
     "c2p1": lambda: perturbed(c2(nq=40, p=1, state="hump", nsteps=30), amp_z=0.2),
     "c2p2": lambda: perturbed(c2(nq=40, p=2, state="hump", nsteps=30), amp_z=0.2),
+    "c2p3": lambda: perturbed(c2(nq=40, p=3, state="hump", nsteps=30), amp_z=0.2),
+    "c5p3-ssp43": lambda: _with_params(c5(nn=40, nsteps=30, p=3), rk_stages=4),
     "c2rest": lambda: c2(nq=40, p=1, state="rest", nsteps=30),
     "c3": lambda: perturbed(c3(nn=60, nsteps=40)),
     "c4": lambda: c4(nqx=64, nqy=32, nsteps=80),
