@@ -428,7 +428,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             from oracle import oracle as orc
         orc.build()
         o = orc.Oracle.from_workload(w)
-        nsamp = max(1, min(args.steps, int(round(12.0 / (w.mesh.n_elem * w.n_stage * 0.28e-6 + 1e-3)))))
+        nsamp = max(1, min(args.steps, int(round(45.0 / (w.mesh.n_elem * w.n_stage * 0.28e-6 + 1e-3)))))   # about 10-15 s on 16 cores
         o.step(1, w.dt)
         t0 = time.perf_counter()
         o.step(nsamp, w.dt)

@@ -105,3 +105,10 @@ def test_c2_full_size(O, G, p):
     w = c2(p=p)
     assert w.mesh.n_elem == 524_288
     full_size_case(O, G, w, 4)
+
+
+def test_c2_full_size_p3(O, G):
+    """The C2 mesh at p = 3, all ten modes populated."""
+    w = perturbed(c2(p=3), amp_z=0.2)
+    assert w.mesh.n_elem == 524_288 and np.abs(w.ze[6:]).max() > 1e-3
+    full_size_case(O, G, w, 2)
