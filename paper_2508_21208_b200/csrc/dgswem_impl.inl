@@ -600,18 +600,20 @@ int launch_stage(Handle* h, const real* win, const real* w0, real* wout, double 
   }
   prof_begin(h, PK_ELEM);
   const int grid = grid_for(h->ne, DGK_STAGE_THREADS);
+  constexpr int PFV = (P == 1) ? 1 : 0;          // the prefetching kernels exist for p = 1 (where this form is the default)
+  const bool pf = PFV != 0 && h->pf_dist > 0;
   if (h->prm.flux == 1) {   // Roe: the generic-flag kernel only
     k_stage<P, MODE, -1, 1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A);
   } else if constexpr (MODE == MODE_UPDATE) {
     // specialised on (first stage, wind): no w^n registers in stage 1, no wind registers without wind
     switch (stage_variant(h, first)) {
-      case 0: k_stage<P, MODE, 0><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      case 1: k_stage<P, MODE, 1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      case 2: k_stage<P, MODE, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      case 3: k_stage<P, MODE, 3><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      case 6: k_stage<P, MODE, 6><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      case 7: k_stage<P, MODE, 7><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
-      default: k_stage<P, MODE, -1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      case 0: if (pf) k_stage<P, MODE, 0, 0, 0, PFV><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); else k_stage<P, MODE, 0><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      case 1: if (pf) k_stage<P, MODE, 1, 0, 0, PFV><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); else k_stage<P, MODE, 1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      case 2: if (pf) k_stage<P, MODE, 2, 0, 0, PFV><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); else k_stage<P, MODE, 2><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      case 3: if (pf) k_stage<P, MODE, 3, 0, 0, PFV><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); else k_stage<P, MODE, 3><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      case 6: if (pf) k_stage<P, MODE, 6, 0, 0, PFV><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); else k_stage<P, MODE, 6><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      case 7: if (pf) k_stage<P, MODE, 7, 0, 0, PFV><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); else k_stage<P, MODE, 7><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
+      default: if (pf) k_stage<P, MODE, -1, 0, 0, PFV><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); else k_stage<P, MODE, -1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A); break;
     }
   } else {
     k_stage<P, MODE, -1><<<grid, DGK_STAGE_THREADS, 0, h->stream>>>(A);
@@ -914,12 +916,13 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
 
   auto body = [&]() -> int {
     // ---- tables to constant memory (both degrees; identical for every handle)
-    Tables T1, T2;
-    Tables T3;
+    Tables T1, T2, T3;
     make_tables(1, T1); make_tables(2, T2); make_tables(3, T3);
-    CK(cudaMemcpyToSymbolAsync(c_tab3, &T3, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
-    CK(cudaMemcpyToSymbolAsync(c_tab1, &T1, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
-    CK(cudaMemcpyToSymbolAsync(c_tab2, &T2, sizeof(Tables), 0, cudaMemcpyHostToDevice, h->stream));
+    static TablesT<1> C1; static TablesT<2> C2;      // (static: the asynchronous copies below read them)
+    copy_tables<1>(T1, C1); copy_tables<2>(T2, C2);
+    CK(cudaMemcpyToSymbolAsync(c_tab1, &C1, sizeof(C1), 0, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaMemcpyToSymbolAsync(c_tab2, &C2, sizeof(C2), 0, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaMemcpyToSymbolAsync(c_tab3, &T3, sizeof(T3), 0, cudaMemcpyHostToDevice, h->stream));
     CK(cudaStreamSynchronize(h->stream));
 
     h->res_edge[0] = resident_ctas(k_edge_pipe<1>, DGK_EDGE_THREADS, 0, prm->device);
