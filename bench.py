@@ -213,7 +213,9 @@ def workload_config(w) -> dict:
     """What names the workload: the SAME dict on both arms (the driver compares them); how an arm ran it is in `run`."""
     return {"workload": w.name, "n_elem": w.mesh.n_elem, "n_edge": w.mesh.n_edge, "n_nodes": w.mesh.n_nodes, "p": w.params["p"],
             "rk_order": w.params["rk_order"], "dt": w.dt, "limiter": w.params["limiter"], "wetdry": w.params["wetdry"],
-            "flux": w.params.get("flux", 0), "wind": w.holland is not None, "tide": w.tide is not None}
+            "flux": w.params.get("flux", 0), "wind": w.holland is not None, "tide": w.tide is not None,
+            # timing hygiene: no L2 flush between iterations where one stage buffer alone exceeds the 126 MB L2
+            "l2": "inputs larger than L2 (no flush)" if 3 * w.ndof * w.mesh.n_elem * 8 > 130e6 else "working set fits L2, not flushed between steps"}
 
 
 def run_reference(args, rank: int):
@@ -395,6 +397,16 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             byts = (alg_bytes(w, k, True, fused, rb) * nfirst + alg_bytes(w, k, False, fused, rb) * (cnt - nfirst)) / cnt
             per_kind[k] = {"launches": cnt, "avg_ms": tms / cnt, "alg_bytes_per_launch": byts,
                            "achieved_gbs": byts / (tms / cnt * 1e-3) / 1e9, "share_of_step": tms / ms_prof}
+    # DRAM bytes per launch from the committed `ncu --set full` captures (profiles/traffic.csv), where one exists: for a
+    # kernel whose writes depend on the data (the write-if-changed limiter pass) this is the honest numerator
+    tfile = ROOT / "profiles" / "traffic.csv"
+    if tfile.exists():
+        for ln in tfile.read_text().splitlines()[1:]:
+            f = ln.split(",")
+            kk = "elem" if (len(f) >= 3 and f[1] == "stage") else (f[1] if len(f) >= 3 else None)
+            if len(f) >= 3 and f[0] == args.workload and kk in per_kind and (f[1] != "stage" or fused) and (f[1] != "elem" or not fused):
+                per_kind[kk]["ncu_dram_bytes_per_launch"] = float(f[2])
+                per_kind[kk]["frac_of_peak_by_ncu_dram_bytes"] = float(f[2]) / (per_kind[kk]["avg_ms"] * 1e-3) / 1e9 / peak
     dom = max(per_kind, key=lambda k: per_kind[k]["avg_ms"] * per_kind[k]["launches"])
     d = per_kind[dom]
     # DRAM bytes per launch of that kernel from the committed `ncu --set full` capture (profiles/traffic.csv)

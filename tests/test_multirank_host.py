@@ -81,6 +81,6 @@ def test_both_arms_name_the_workload_with_the_same_config_keys():
     import bench
     w = bench.make_workload("C1")
     cfg = bench.workload_config(w)
-    assert set(cfg) == {"workload", "n_elem", "n_edge", "n_nodes", "p", "rk_order", "dt", "limiter", "wetdry", "flux", "wind", "tide"}
+    assert set(cfg) == {"workload", "n_elem", "n_edge", "n_nodes", "p", "rk_order", "dt", "limiter", "wetdry", "flux", "wind", "tide", "l2"}
     src = (ROOT / "bench.py").read_text()
     assert src.count('"config": workload_config(w)') + src.count('"config": cfg') >= 2
