@@ -272,7 +272,7 @@ def run_decomp(args, rank: int, world: int, local_rank: int):
     pd = PartitionedDgswem(w.params, m.xy, w.bathy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, n_parts,
                            tide=w.tide, holland=w.holland, reorder=args.reorder, device=local_rank,
                            parts=[rank] if world > 1 else None, transport=DistTransport() if world > 1 else None,
-                           overlap=None if args.decomp_overlap < 0 else bool(args.decomp_overlap))
+                           overlap=None if args.decomp_overlap < 0 else bool(args.decomp_overlap), graph=bool(args.decomp_graph) and world == 1)
     pd.set_state(0.0, w.ze, w.qx, w.qy)
 
     def barrier():
@@ -300,7 +300,7 @@ def run_decomp(args, rank: int, world: int, local_rank: int):
             "data": "synthetic",
             "config": {"workload": w.name, "n_elem": m.n_elem, "p": w.params["p"], "rk_order": w.params["rk_order"], "dt": w.dt,
                        "parallelism": f"domain decomposition: {n_parts} partitions on {world} GPU(s), halo exchange every RK stage",
-                       "ghost_elements": int(ghosts), "overlap": bool(pd.overlap), "transport": "NCCL isend/irecv" if world > 1 else "device copies (one GPU)"},
+                       "ghost_elements": int(ghosts), "overlap": bool(pd.overlap), "one_graph_per_step": bool(pd.graph), "transport": "NCCL isend/irecv" if world > 1 else "device copies (one GPU)"},
             "gpu_launches": int(launches), "e2e": None, "roofline": None, "cpu_baseline": None}
     print(json.dumps(line), flush=True)
     pd.close()
@@ -485,6 +485,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--decomp", type=int, default=0, help="domain decomposition instead of replicas: one partition per rank "
                     "(N > 1), or this many partitions on the one GPU (N = 1)")
+    ap.add_argument("--decomp-graph", type=int, default=0, help="--decomp on one GPU: record the whole decomposed step into one CUDA graph and replay it")
     ap.add_argument("--decomp-overlap", type=int, default=-1, help="--decomp: 1 = every stage first on the send-list elements, whose "
                     "exchange then overlaps the interior elements; 0 = unsplit; -1 = on when there is one partition per rank")
     args = ap.parse_args()

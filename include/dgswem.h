@@ -130,6 +130,17 @@ int dgswem_stage_rhs(dgswem_t*, int s);
 int dgswem_stage_rhs_part(dgswem_t*, int s, int part);
 int dgswem_stage_limit(dgswem_t*, int s);
 int dgswem_end_step(dgswem_t*);
+/* Recording a stage-granular step into the CALLER's CUDA graph (a decomposed run: every partition's kernels and the
+ * exchange between them in one graph per step).  Kernel arguments are frozen in
+ * a graph, so while capture mode is on the per-stage scalars (tidal elevation, storm centre) are passed as references
+ * into the handle's device table, row = a device step counter, and dgswem_end_step records the counter's increment
+ * instead of advancing the handle's time: the caller brackets ONE begin_step ... end_step sequence (and its
+ * halo_pack / halo_unpack calls with device buffers) with dgswem_capture_mode(1) ... (0) while its own stream capture
+ * is active on streams that include this handle's.  Before replaying the graph n <= 4096 times the caller calls
+ * dgswem_graph_steps(n, dt) -- dt as recorded --: it tabulates the scalars of the next n steps, uploads them on the
+ * handle's stream, resets the counter and advances the handle's time by n dt.  Same bits as the unrecorded calls. */
+int dgswem_capture_mode(dgswem_t*, int on);
+int dgswem_graph_steps(dgswem_t*, int64_t nsteps, double dt);
 int dgswem_set_halo(dgswem_t*, int64_t n_send, const int32_t* send_ids, int64_t n_recv, const int32_t* recv_ids);
 int dgswem_halo_pack(dgswem_t*, int what, double* buf, int buf_on_device);
 int dgswem_halo_unpack(dgswem_t*, int what, const double* buf, int buf_on_device);

@@ -44,7 +44,7 @@ class DgswemError(RuntimeError):
 
 EXPORTS = ["dgswem_create", "dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_set_wind_forcing", "dgswem_set_rain", "dgswem_get_pressure", "dgswem_step",
            "dgswem_eval_rhs", "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_nodal", "dgswem_get_wind",
-           "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_rhs_part", "dgswem_stage_limit", "dgswem_end_step", "dgswem_set_halo",
+           "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_rhs_part", "dgswem_stage_limit", "dgswem_end_step", "dgswem_capture_mode", "dgswem_graph_steps", "dgswem_set_halo",
            "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_fp64_peak", "dgswem_stage_form", "dgswem_precision", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
 
 _lib = None
@@ -83,6 +83,8 @@ def load_library():
     L.dgswem_stage_rhs_part.argtypes = [VP, C.c_int, C.c_int]
     L.dgswem_stage_limit.argtypes = [VP, C.c_int]
     L.dgswem_end_step.argtypes = [VP]
+    L.dgswem_capture_mode.argtypes = [VP, C.c_int]
+    L.dgswem_graph_steps.argtypes = [VP, I64, D]
     L.dgswem_set_halo.argtypes = [VP, I64, PI32, I64, PI32]
     L.dgswem_halo_pack.argtypes = [VP, C.c_int, C.c_void_p, C.c_int]
     L.dgswem_halo_unpack.argtypes = [VP, C.c_int, C.c_void_p, C.c_int]
@@ -98,7 +100,7 @@ def load_library():
     for name in ("dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_set_wind_forcing", "dgswem_set_rain",
                  "dgswem_get_pressure", "dgswem_step", "dgswem_eval_rhs",
                  "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_wind", "dgswem_sync",
-                 "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_rhs_part", "dgswem_stage_limit", "dgswem_end_step", "dgswem_set_halo",
+                 "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_rhs_part", "dgswem_stage_limit", "dgswem_end_step", "dgswem_capture_mode", "dgswem_graph_steps", "dgswem_set_halo",
                  "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_get_nodal"):
         getattr(L, name).restype = C.c_int
     _lib = L
@@ -266,6 +268,12 @@ class Dgswem:
             self._check(self.L.dgswem_stage_rhs_part(self.h, int(s), int(part)))
         else:
             self._check(self.L.dgswem_stage_rhs(self.h, int(s)))
+
+    def capture_mode(self, on):
+        self._check(self.L.dgswem_capture_mode(self.h, int(bool(on))))
+
+    def graph_steps(self, nsteps, dt):
+        self._check(self.L.dgswem_graph_steps(self.h, int(nsteps), float(dt)))
 
     def stage_limit(self, s):
         self._check(self.L.dgswem_stage_limit(self.h, int(s)))

@@ -79,6 +79,8 @@ int dgswem_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhook
 void dgswem_destroy(dgswem_t* h) { if (h) DISPATCH(h, api_destroy); }
 
 int dgswem_end_step(dgswem_t* h) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_end_step); }
+int dgswem_capture_mode(dgswem_t* h, int on) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_capture_mode, on); }
+int dgswem_graph_steps(dgswem_t* h, int64_t nsteps, double dt) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_graph_steps, nsteps, dt); }
 int dgswem_sync(dgswem_t* h) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_sync); }
 int dgswem_set_state(dgswem_t* h, double t, const double* ze, const double* qx, const double* qy) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_set_state, t, ze, qx, qy); }
 int dgswem_set_tide(dgswem_t* h, double amp, double omega, double phase) { if (!h) return DGSWEM_E_ARG; return DISPATCH(h, api_set_tide, amp, omega, phase); }

@@ -777,9 +777,48 @@ int capture_steps(Handle* h, int steps, double dt, bool need_tab, Handle::StepGr
   return 0;
 }
 
+// The per-step scalars of a replayed graph (tidal elevation of every stage, storm centre): device table + pinned staging
+// copy + the event that guards the staging copy, created once per handle
+constexpr long long kScalRows = 4096;   // steps per table upload (256 KiB); longer calls go in chunks
+int ensure_scalar_table(Handle* h) {
+  if (h->scal_cap != 0) return 0;
+  // all three resources first, then published together: a failure leaves the handle as it was (scal_cap == 0)
+  double* tab = (double*)h->dalloc((size_t)kScalRows * kScalStride * sizeof(double));
+  if (!tab) return h->fail(DGSWEM_E_CUDA, "device allocation failed");
+  double* host = nullptr;
+  cudaEvent_t ev = nullptr;
+  cudaError_t e = cudaMallocHost((void**)&host, (size_t)kScalRows * kScalStride * sizeof(double));
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+  if (e != cudaSuccess) {
+    if (host) cudaFreeHost(host);
+    h->dfree(tab);
+    return h->cuda_fail(e, "scalar table setup");
+  }
+  h->scal_tab = tab; h->scal_host = host; h->scal_ev = ev; h->scal_cap = kScalRows;
+  return 0;
+}
+// rows for the `chunk` steps that start at h->t, tabulated on the host exactly as the stream path computes them, uploaded on
+// the handle's stream; the device step counter goes back to row 0
+int upload_scalar_rows(Handle* h, long long chunk, double dt) {
+  const double* c = h->rk.c;
+  CK(cudaEventSynchronize(h->scal_ev));   // the previous upload has left the pinned staging copy
+  double t = h->t;
+  for (long long n = 0; n < chunk; ++n) {
+    double* row = h->scal_host + (size_t)n * kScalStride;
+    for (int i = 0; i < kScalStride; ++i) row[i] = 0.0;
+    for (int st = 0; st < h->nstage; ++st) row[st] = tide_value(h, t + c[st] * dt);
+    row[4] = h->hol.x0 + h->hol.vx * t; row[5] = h->hol.y0 + h->hol.vy * t;
+    t = t + dt;
+  }
+  // stream order keeps earlier replays' reads of the device table ahead of this overwrite
+  CK(cudaMemcpyAsync(h->scal_tab, h->scal_host, (size_t)chunk * kScalStride * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  CK(cudaEventRecord(h->scal_ev, h->stream));
+  CK(cudaMemsetAsync(h->step_ctr, 0, sizeof(int), h->stream));
+  return 0;
+}
+
 template <int P>
 int run_steps(Handle* h, long long nsteps, double dt) {
-  const double* c = h->rk.c;
   if (!h->graphs_on || h->profiling || nsteps == 0) {
     for (long long n = 0; n < nsteps; ++n) {
       int rc = enqueue_step<P>(h, dt, h->t);
@@ -794,22 +833,7 @@ int run_steps(Handle* h, long long nsteps, double dt) {
   const bool tide_on = h->tide_amp != 0.0;
   const bool need_tab = tide_on || h->wind_on;
   if (h->graph_one.exec && (h->graph_dt != dt || h->graph_wind != h->wind_on || h->graph_tide != tide_on)) drop_graphs(h);
-  constexpr long long kScalRows = 4096;   // steps per table upload (256 KiB); longer calls go in chunks
-  if (need_tab && h->scal_cap == 0) {
-    // all three resources first, then published together: a failure leaves the handle as it was (scal_cap == 0)
-    double* tab = (double*)h->dalloc((size_t)kScalRows * kScalStride * sizeof(double));
-    if (!tab) return h->fail(DGSWEM_E_CUDA, "device allocation failed");
-    double* host = nullptr;
-    cudaEvent_t ev = nullptr;
-    cudaError_t e = cudaMallocHost((void**)&host, (size_t)kScalRows * kScalStride * sizeof(double));
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
-    if (e != cudaSuccess) {
-      if (host) cudaFreeHost(host);
-      h->dfree(tab);
-      return h->cuda_fail(e, "scalar table setup");
-    }
-    h->scal_tab = tab; h->scal_host = host; h->scal_ev = ev; h->scal_cap = kScalRows;
-  }
+  if (need_tab) { int rc = ensure_scalar_table(h); if (rc) return rc; }
   const int many = h->ne < 65536 ? 8 : (h->ne < 1000000 ? 2 : 1);
   if (!h->graph_one.exec) {
     int rc = capture_steps<P>(h, 1, dt, need_tab, h->graph_one);
@@ -820,21 +844,7 @@ int run_steps(Handle* h, long long nsteps, double dt) {
   long long done = 0;
   while (done < nsteps) {
     const long long chunk = need_tab ? std::min(nsteps - done, h->scal_cap) : nsteps - done;
-    if (need_tab) {
-      CK(cudaEventSynchronize(h->scal_ev));   // the previous upload has left the pinned staging copy
-      double t = h->t;
-      for (long long n = 0; n < chunk; ++n) {
-        double* row = h->scal_host + (size_t)n * kScalStride;
-        for (int i = 0; i < kScalStride; ++i) row[i] = 0.0;
-        for (int st = 0; st < h->nstage; ++st) row[st] = tide_value(h, t + c[st] * dt);
-        row[4] = h->hol.x0 + h->hol.vx * t; row[5] = h->hol.y0 + h->hol.vy * t;
-        t = t + dt;
-      }
-      // stream order keeps earlier replays' reads of the device table ahead of this overwrite
-      CK(cudaMemcpyAsync(h->scal_tab, h->scal_host, (size_t)chunk * kScalStride * sizeof(double), cudaMemcpyHostToDevice, h->stream));
-      CK(cudaEventRecord(h->scal_ev, h->stream));
-      CK(cudaMemsetAsync(h->step_ctr, 0, sizeof(int), h->stream));
-    }
+    if (need_tab) { int rc = upload_scalar_rows(h, chunk, dt); if (rc) return rc; }
     long long left = chunk;
     while (left > 0) {
       Handle::StepGraph& g = (h->graph_many.exec && left >= h->graph_many.steps) ? h->graph_many : h->graph_one;
@@ -1363,9 +1373,36 @@ int api_stage_limit(Handle* h, int s) {
 int api_end_step(Handle* h) {
   if (!h) return DGSWEM_E_ARG;
   if (h->step_dt == 0.0) return h->fail(DGSWEM_E_ARG, "no step in progress (dgswem_begin_step)");
-  h->t = h->t + h->step_dt;
+  if (h->capturing) {
+    // being recorded into the caller's graph, not run: time does not move; the replayed step ends by moving to the next table row
+    k_advance<<<1, 1, 0, h->stream>>>(h->step_ctr);
+    CKL("k_advance");
+  } else {
+    h->t = h->t + h->step_dt;
+  }
   h->step_dt = 0.0;
   h->last_out = h->W[0];
+  return DGSWEM_OK;
+}
+
+// ---- a stage-granular step recorded into the CALLER's CUDA graph (a decomposed run's whole step: all partitions + the exchange)
+int api_capture_mode(Handle* h, int on) {
+  if (!h) return DGSWEM_E_ARG;
+  if (h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a stage-granular step is in progress");
+  if (on) { CK(cudaSetDevice(h->prm.device)); int rc = ensure_scalar_table(h); if (rc) return rc; }
+  h->capturing = on != 0;
+  return DGSWEM_OK;
+}
+int api_graph_steps(Handle* h, int64_t nsteps, double dt) {
+  if (!h) return DGSWEM_E_ARG;
+  if (nsteps < 0 || !(dt > 0.0)) return h->fail(DGSWEM_E_ARG, "need nsteps >= 0 and dt > 0");
+  if (h->capturing || h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "not while a step is being recorded or is in progress");
+  CK(cudaSetDevice(h->prm.device));
+  int rc = ensure_scalar_table(h);
+  if (rc) return rc;
+  if (nsteps > h->scal_cap) return h->fail(DGSWEM_E_ARG, "at most 4096 steps per call");
+  if ((rc = upload_scalar_rows(h, nsteps, dt))) return rc;
+  for (int64_t n = 0; n < nsteps; ++n) h->t = h->t + dt;
   return DGSWEM_OK;
 }
 

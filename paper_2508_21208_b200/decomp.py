@@ -82,7 +82,7 @@ class PartitionedDgswem:
     only and `transport` must be a DistTransport whose ranks are the part ids."""
 
     def __init__(self, params, xy, bathy, tri, edge_elem, edge_local, edge_bc, elem_edge, n_parts, *, tide=None, holland=None,
-                 reorder=1, device=0, parts=None, transport=None, part_of_element=None, overlap=None):
+                 reorder=1, device=0, parts=None, transport=None, part_of_element=None, overlap=None, graph=False):
         import torch
         from .binding import Dgswem
         if int(params["limiter"]) == 2:
@@ -96,6 +96,11 @@ class PartitionedDgswem:
         # rank); with every partition on one GPU the split only adds launches (C3, 4 partitions: 91.7 against 102.8 G DOF-updates/s)
         self.overlap = (transport is not None and not isinstance(transport, LocalTransport)) if overlap is None else bool(overlap)
         self.comm = torch.cuda.Stream(device=device)      # the transport's stream: runs beside the partitions' streams
+        self.cap = torch.cuda.Stream(device=device)       # the stream a whole step is recorded on and replayed from (graph=True)
+        self.graph = bool(graph)
+        self._graph, self._graph_dt = None, None
+        if self.graph and transport is not None and not isinstance(transport, LocalTransport):
+            raise ValueError("graph=True records device copies between partitions of one process: LocalTransport only")
         self.n_elem = int(np.asarray(tri).shape[0])
         self.limiter = bool(params["limiter"])
         self.n_stage = int(params.get("rk_stages", 0)) or int(params["rk_order"])
@@ -159,6 +164,7 @@ class PartitionedDgswem:
     def join(self):
         """Make torch's current stream wait for everything enqueued on the partitions' streams (for timing with events)."""
         cur = self.torch.cuda.current_stream()
+        ev = self.torch.cuda.Event(); ev.record(self.cap); cur.wait_event(ev)
         for g in self.handles:
             ev = self.torch.cuda.Event()
             ev.record(g.stream)
@@ -169,32 +175,77 @@ class PartitionedDgswem:
             gid = self.subs[p].elem_gid
             g.set_state(t, np.ascontiguousarray(ze[:, gid]), np.ascontiguousarray(qx[:, gid]), np.ascontiguousarray(qy[:, gid]))
 
+    def _one_step(self, dt):
+        for g in self.handles:
+            g.begin_step(dt)
+        for s in range(self.n_stage):
+            first_what = 1 if self.limiter else 0           # what the stage's first exchange carries
+            if self.overlap:
+                for g in self.handles:
+                    g.stage_rhs(s, part=1)
+                pending = self._exchange_begin(first_what)
+                for g in self.handles:
+                    g.stage_rhs(s, part=2)
+                self._exchange_end(first_what, pending)
+            else:
+                for g in self.handles:
+                    g.stage_rhs(s)
+                self._exchange(first_what)
+            if self.limiter:
+                for g in self.handles:
+                    g.stage_limit(s)
+                self._exchange(0)
+        for g in self.handles:
+            g.end_step()
+
     def step(self, nsteps, dt):
-        """overlap (default): every stage first runs on the elements other partitions wait for (dgswem_stage_rhs_part 1),
-        packs them and starts the transport on the communication stream, and only then runs on the interior elements, so
-        that the exchange travels while they are computed; the unpack waits for both.  Same bits either way."""
-        for _ in range(int(nsteps)):
+        """overlap: every stage first runs on the elements other partitions wait for (dgswem_stage_rhs_part 1), packs them and
+        starts the transport on the communication stream, and only then runs on the interior elements, so that the exchange
+        travels while they are computed; the unpack waits for both.
+        graph (LocalTransport only): the whole step -- every partition's kernels, packs, copies, unpacks, with their event
+        dependencies -- is recorded once into ONE CUDA graph (dgswem_capture_mode) and replayed; per-step scalars come
+        from each handle's device table (dgswem_graph_steps).  Same bits in every mode."""
+        nsteps = int(nsteps)
+        if not self.graph:
+            for _ in range(nsteps):
+                self._one_step(dt)
+            return
+        torch = self.torch
+        if self._graph is None or self._graph_dt != dt:
+            self._capture(dt)
+        done = 0
+        while done < nsteps:
+            n = min(nsteps - done, 4096)
+            for g in self.handles:                       # scalar rows of the next n steps, on each handle's stream
+                g.graph_steps(n, dt)
+                ev = torch.cuda.Event(); ev.record(g.stream); self.cap.wait_event(ev)
+            with torch.cuda.stream(self.cap):
+                for _ in range(n):
+                    self._graph.replay()
+                fin = torch.cuda.Event(); fin.record(self.cap)
+            for g in self.handles:                       # the next upload / any later call on a handle comes after the replays
+                g.stream.wait_event(fin)
+            done += n
+
+    def _capture(self, dt):
+        torch = self.torch
+        torch.cuda.synchronize()
+        for g in self.handles:
+            g.capture_mode(True)
+        try:
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=self.cap, capture_error_mode="relaxed"):
+                fork = torch.cuda.Event(); fork.record(self.cap)
+                for g in self.handles:                   # the handles' streams join the capture
+                    g.stream.wait_event(fork)
+                self.comm.wait_event(fork)
+                self._one_step(dt)
+                for st in [g.stream for g in self.handles] + [self.comm]:
+                    ev = torch.cuda.Event(); ev.record(st); self.cap.wait_event(ev)
+        finally:
             for g in self.handles:
-                g.begin_step(dt)
-            for s in range(self.n_stage):
-                first_what = 1 if self.limiter else 0           # what the stage's first exchange carries
-                if self.overlap:
-                    for g in self.handles:
-                        g.stage_rhs(s, part=1)
-                    pending = self._exchange_begin(first_what)
-                    for g in self.handles:
-                        g.stage_rhs(s, part=2)
-                    self._exchange_end(first_what, pending)
-                else:
-                    for g in self.handles:
-                        g.stage_rhs(s)
-                    self._exchange(first_what)
-                if self.limiter:
-                    for g in self.handles:
-                        g.stage_limit(s)
-                    self._exchange(0)
-            for g in self.handles:
-                g.end_step()
+                g.capture_mode(False)
+        self._graph, self._graph_dt = graph, dt
 
     def get_state(self):
         """(t, ze, qx, qy) of the elements this process owns, scattered into global-size arrays (others stay NaN)."""

@@ -71,6 +71,35 @@ def test_partitioned_run_equals_undivided_run(O, G, monkeypatch, case, n_parts, 
     pd.close()
 
 
+@pytest.mark.parametrize("overlap", [False, True], ids=["unsplit", "overlap"])
+@pytest.mark.parametrize("case", ["c3-tide-wetdry", "c4-limiter-wind", "c5-p2-rk3-all"])
+def test_partitioned_step_recorded_as_one_cuda_graph(O, G, case, overlap):
+    """graph=True: one CUDA graph holds a whole decomposed step (three partitions' kernels, packs, copies, unpacks and
+    their dependencies; dgswem_capture_mode), replayed for every step with the tide / storm-centre scalars read from the
+    handles' device tables (dgswem_graph_steps), in two calls so that the tables are refilled at a later time.  Same bits
+    as the oracle's undivided run."""
+    from paper_2508_21208_b200.decomp import PartitionedDgswem
+    w = CASES[case]()
+    m = w.mesh
+    o = O.Oracle.from_workload(w)
+    o.step(w.nsteps, w.dt)
+    t_orc, *s_orc = o.get_state()
+    pd = PartitionedDgswem(w.params, m.xy, w.bathy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, 3,
+                           tide=w.tide, holland=w.holland, overlap=overlap, graph=True)
+    pd.set_state(0.0, w.ze, w.qx, w.qy)
+    l0 = sum(g.launch_count() for g in pd.handles)
+    first = w.nsteps // 3
+    pd.step(first, w.dt)
+    pd.step(w.nsteps - first, w.dt)
+    t, *s = pd.get_state()
+    assert t == t_orc
+    for c in range(3):
+        assert np.array_equal(s[c], s_orc[c])
+    assert np.array_equal(pd.get_wetdry(), o.get_wetdry())
+    assert pd._graph is not None
+    pd.close()
+
+
 def test_stage_api_equals_dgswem_step_and_rejects_misuse(G):
     """begin_step / stage_rhs / stage_limit / end_step on an undivided mesh (no halo) is dgswem_step; misuse is an error."""
     w = c4(nqx=32, nqy=16, nsteps=15)
