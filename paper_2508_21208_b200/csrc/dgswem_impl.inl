@@ -1329,6 +1329,7 @@ int api_step(Handle* h, int64_t nsteps, double dt) {
   if (!h) return DGSWEM_E_ARG;
   if (nsteps < 0 || !(dt > 0.0)) return h->fail(DGSWEM_E_ARG, "need nsteps >= 0 and dt > 0");
   if (h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a stage-granular step is in progress (dgswem_end_step)");
+  if (h->capturing) return h->fail(DGSWEM_E_ARG, "capture mode is on (dgswem_capture_mode(0) first)");
   CK(cudaSetDevice(h->prm.device));
   return h->prm.p == 1 ? run_steps<1>(h, nsteps, dt) : h->prm.p == 2 ? run_steps<2>(h, nsteps, dt) : run_steps<3>(h, nsteps, dt);
 }
@@ -1389,6 +1390,7 @@ int api_end_step(Handle* h) {
 int api_capture_mode(Handle* h, int on) {
   if (!h) return DGSWEM_E_ARG;
   if (h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a stage-granular step is in progress");
+  if (on && h->profiling) return h->fail(DGSWEM_E_ARG, "per-launch profiling events cannot be recorded into a graph (dgswem_profile(0) first)");
   if (on) { CK(cudaSetDevice(h->prm.device)); int rc = ensure_scalar_table(h); if (rc) return rc; }
   h->capturing = on != 0;
   return DGSWEM_OK;
@@ -1673,6 +1675,7 @@ int64_t api_launch_count(const Handle* h) { return h ? h->launches : 0; }
 
 int api_profile(Handle* h, int enable) {
   if (!h) return DGSWEM_E_ARG;
+  if (enable && h->capturing) return h->fail(DGSWEM_E_ARG, "capture mode is on: profiling events cannot be recorded into a graph");
   h->profiling = enable != 0;
   return DGSWEM_OK;
 }

@@ -122,5 +122,15 @@ def test_stage_api_equals_dgswem_step_and_rejects_misuse(G):
         b.stage_rhs(7)
     with pytest.raises(G.DgswemError):
         b.stage_rhs(0, part=3)
+    with pytest.raises(G.DgswemError):
+        b.capture_mode(True)                # not inside a step
     b.end_step()
+    b.capture_mode(True)
+    with pytest.raises(G.DgswemError):
+        b.step(1, w.dt)                     # dgswem_step while the handle records for the caller's graph
+    with pytest.raises(G.DgswemError):
+        b.graph_steps(1, w.dt)
+    b.capture_mode(False)
+    with pytest.raises(G.DgswemError):
+        b.graph_steps(5000, w.dt)           # more rows than the scalar table holds
     a.close(); b.close()
