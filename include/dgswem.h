@@ -17,8 +17,9 @@
  *   - calls on one handle must not be concurrent.  Work is enqueued on the handle's stream;
  *     get_* calls synchronise it.
  *   - environment, read by dgswem_create (tuning / test knobs; every setting gives the same bits):
- *     DGSWEM_FUSED=0/1 form of the RK stage (see dgswem_stage_form), DGSWEM_GRAPH=0 plain stream launches instead of
- *     CUDA-graph replay in dgswem_step, DGSWEM_PERSISTENT_CTAS=n cap (0: off) on the persistent kernels' grids.
+ *     DGSWEM_FUSED=0..3 form of the RK stage (see dgswem_stage_form), DGSWEM_GRAPH=0 plain stream launches instead of
+ *     CUDA-graph replay in dgswem_step, DGSWEM_PERSISTENT_CTAS=n cap (0: off) on the persistent kernels' grids,
+ *     DGSWEM_PF_DIST=n tiles ahead that the stage kernel pulls into L2 (0: off; default on for meshes larger than L2).
  */
 #ifndef DGSWEM_H
 #define DGSWEM_H
@@ -183,9 +184,10 @@ int dgswem_test_math(dgswem_t*, int64_t n, const double* x, double* out);
  * (x 2 = flop/s).  Synchronises. */
 int dgswem_fp64_peak(dgswem_t*, double* dfma_per_s);
 
-/* Which form of the RK stage this handle runs: 0 = edge kernel + element kernel with the per-edge flux
- * buffer, 1 = element-centric stage kernel without it (default for p = 1; DGSWEM_FUSED=0/1 in the environment of
- * dgswem_create overrides).  Both give the same bits. */
+/* Which form of the RK stage this handle runs (DGSWEM_FUSED=0..3 in the environment of dgswem_create overrides the
+ * default): 0 = edge kernel + element kernel with the per-edge flux buffer (default for p = 2; the only form at p = 3),
+ * 1 = element-centric stage kernel without it (default for p = 1), 2 = the same with a shared-memory edge tile (each
+ * tile-interior flux evaluated once), 3 = the same with TMA-staged operands.  All give the same bits. */
 int dgswem_stage_form(const dgswem_t*);
 
 /* Working precision of the handle: 64 or 32 (dgswem_params.precision). */
