@@ -167,6 +167,34 @@ int dgswem_get_wetdry(dgswem_t*, uint8_t* wet);
  * evaluated at that node (summed in ascending caller element id); zn, qxn, qyn: [n_nodes] each, host.  Synchronises. */
 int dgswem_get_nodal(dgswem_t*, double* zn, double* qxn, double* qyn);
 
+/* ---- Nodal output without any allocation (csrc/dgswem_static.cu).
+ * For callers that cannot allocate device memory at the moment they want nodal fields, and so can neither create a handle
+ * nor let one grow: code running while a stream capture is open (cudaMalloc is forbidden there and breaks the capture),
+ * a solver living inside an application whose memory pool already holds the whole GPU (cudaMalloc fails), a time loop
+ * that must not stall (cudaMalloc / cudaFree synchronise the device).  Same result, bit for bit, as dgswem_get_nodal
+ * on a binary64 handle holding the same mesh and state: per node the mean, over the elements touching it in ascending
+ * element id, of the element's polynomial at that node; a node no element touches gets 0.
+ *   ALL pointers are DEVICE memory on `device`, owned by the caller, in the caller's numbering: tri [n_elem][3] node ids
+ *   (an entry outside [0, n_nodes) is left out of the averages -- it is not reported); ze, qx, qy [ndof][n_elem],
+ *   ndof = (p+1)(p+2)/2, p = 1, 2 or 3; outputs zn, qxn, qyn [n_nodes].  stream: a cudaStream_t cast to void*
+ *   (NULL = the default stream).  The call only enqueues kernels on that stream; it does not synchronise.
+ *   Limits: n_elem <= DGSWEM_STATIC_MAX_ELEM and n_nodes <= DGSWEM_STATIC_MAX_NODES, else DGSWEM_E_ARG (nothing is
+ *   launched).  The node -> element table is rebuilt on every call in one file-scope device array of
+ *   DGSWEM_STATIC_SCRATCH_BYTES (20 MiB), which every GPU that loads this library holds until the process exits.
+ *   The call uses no cudaMalloc, cudaFree or allocating library routine.
+ *   The FIRST call on each device looks up that device's address of the array (cudaGetSymbolAddress); make that first
+ *   call before starting any stream capture.  All calls share the one array: it keeps the previous call's contents (the
+ *   parts that must start at zero are cleared by each call), and two calls whose kernels can overlap on the same GPU
+ *   -- different streams or host threads without an ordering between them -- race on it and give wrong results.
+ *   Errors: 0, DGSWEM_E_ARG or DGSWEM_E_CUDA; text from dgswem_nodal_static_error (per host thread, valid until that
+ *   thread's next call). */
+#define DGSWEM_STATIC_MAX_ELEM      524288      /* 2^19: BASELINE configs[1]'s mesh just fits */
+#define DGSWEM_STATIC_MAX_NODES     524288
+#define DGSWEM_STATIC_SCRATCH_BYTES 20971520    /* 2^21 sort keys of 8 bytes + 2 x 2^19 int32 */
+int dgswem_nodal_static(int device, void* stream, int p, int64_t n_nodes, int64_t n_elem, const int32_t* tri,
+                        const double* ze, const double* qx, const double* qy, double* zn, double* qxn, double* qyn);
+const char* dgswem_nodal_static_error(void);
+
 /* Nodal kinematic wind stress tau_s/rho_0 of the last WIND evaluation, [2][n_nodes] (test hook). */
 int dgswem_get_wind(dgswem_t*, double* tau);
 

@@ -4,4 +4,4 @@
 sm_100a fp64 CUDA kernels do all the work.  Build the library in-tree with
 `python -m paper_2508_21208_b200.build`.
 """
-from .binding import Dgswem, DgswemError, load_library, LIB_PATH, EXPORTS  # noqa: F401
+from .binding import Dgswem, DgswemError, load_library, LIB_PATH, EXPORTS, nodal_static  # noqa: F401

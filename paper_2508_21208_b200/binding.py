@@ -45,7 +45,8 @@ class DgswemError(RuntimeError):
 EXPORTS = ["dgswem_create", "dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_set_wind_forcing", "dgswem_set_rain", "dgswem_get_pressure", "dgswem_step",
            "dgswem_eval_rhs", "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_nodal", "dgswem_get_wind",
            "dgswem_begin_step", "dgswem_stage_rhs", "dgswem_stage_rhs_part", "dgswem_stage_limit", "dgswem_end_step", "dgswem_capture_mode", "dgswem_graph_steps", "dgswem_set_halo",
-           "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_fp64_peak", "dgswem_stage_form", "dgswem_precision", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy"]
+           "dgswem_halo_pack", "dgswem_halo_unpack", "dgswem_test_math", "dgswem_fp64_peak", "dgswem_stage_form", "dgswem_precision", "dgswem_launch_count", "dgswem_profile", "dgswem_profile_read", "dgswem_sync", "dgswem_last_error", "dgswem_destroy",
+           "dgswem_nodal_static", "dgswem_nodal_static_error"]
 
 _lib = None
 
@@ -97,6 +98,8 @@ def load_library():
     L.dgswem_sync.argtypes = [VP]
     L.dgswem_last_error.argtypes = [VP]; L.dgswem_last_error.restype = C.c_char_p
     L.dgswem_destroy.argtypes = [VP]; L.dgswem_destroy.restype = None
+    L.dgswem_nodal_static.argtypes = [C.c_int, VP, C.c_int, I64, I64, VP, VP, VP, VP, VP, VP, VP]; L.dgswem_nodal_static.restype = C.c_int
+    L.dgswem_nodal_static_error.argtypes = []; L.dgswem_nodal_static_error.restype = C.c_char_p
     for name in ("dgswem_set_state", "dgswem_set_tide", "dgswem_set_wind_holland", "dgswem_set_wind_forcing", "dgswem_set_rain",
                  "dgswem_get_pressure", "dgswem_step", "dgswem_eval_rhs",
                  "dgswem_get_flux", "dgswem_get_state", "dgswem_get_wetdry", "dgswem_get_wind", "dgswem_sync",
@@ -109,6 +112,44 @@ def load_library():
 
 def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+STATIC_MAX_ELEM = 524288     # DGSWEM_STATIC_MAX_ELEM / DGSWEM_STATIC_MAX_NODES of include/dgswem.h
+STATIC_MAX_NODES = 524288
+
+
+def nodal_static(p, tri, ze, qx, qy, zn, qxn, qyn, *, n_nodes=None, n_elem=None):
+    """dgswem_nodal_static: element-averaged nodal values of a modal state, for callers that cannot
+    allocate device memory when they need them (a stream capture is open, a memory pool owns the GPU, the time loop
+    must not stall on cudaMalloc): no handle, no allocation -- the node -> element table is rebuilt per call in the
+    library's fixed 20 MiB device array, hence the limits STATIC_MAX_ELEM / STATIC_MAX_NODES (DgswemError beyond them).
+
+    Every argument is a contiguous torch CUDA tensor owned by the caller, all on one device: tri int32 [n_elem, 3];
+    ze, qx, qy float64 [ndof, n_elem]; outputs zn, qxn, qyn float64 [n_nodes], overwritten.  Kernels are enqueued on
+    torch's current stream of that device; nothing is synchronised.  Same bits as Dgswem.get_nodal for the same mesh
+    and state.  Make the first call on a device outside any stream capture, and do not let two calls overlap on one GPU
+    (they share the array).  n_nodes / n_elem override the sizes taken from the tensor shapes (tests of the limits)."""
+    import torch
+    ts = (tri, ze, qx, qy, zn, qxn, qyn)
+    dev = tri.device
+    if dev.type != "cuda" or any(t.device != dev for t in ts):
+        raise ValueError("nodal_static takes CUDA tensors on one device (there is no CPU fallback)")
+    if any(not t.is_contiguous() for t in ts):
+        raise ValueError("nodal_static takes contiguous tensors")
+    if tri.dtype != torch.int32 or any(t.dtype != torch.float64 for t in ts[1:]):
+        raise ValueError("tri must be int32, all other tensors float64")
+    ndof = (int(p) + 1) * (int(p) + 2) // 2
+    ne = tri.shape[0] if n_elem is None else int(n_elem)
+    nn = zn.shape[0] if n_nodes is None else int(n_nodes)
+    if n_elem is None and n_nodes is None:
+        if tri.shape != (ne, 3) or any(t.shape != (ndof, ne) for t in (ze, qx, qy)) or any(t.shape != (nn,) for t in (zn, qxn, qyn)):
+            raise ValueError("shapes: tri [n_elem, 3]; ze, qx, qy [ndof, n_elem]; zn, qxn, qyn [n_nodes]")
+    L = load_library()
+    idx = dev.index if dev.index is not None else torch.cuda.current_device()
+    rc = L.dgswem_nodal_static(idx, torch.cuda.current_stream(dev).cuda_stream, int(p), nn, ne,
+                               *(t.data_ptr() for t in ts))
+    if rc != 0:
+        raise DgswemError(rc, (L.dgswem_nodal_static_error() or b"").decode())
 
 
 class Dgswem:

@@ -2,7 +2,8 @@
 
 Flags that matter: -fmad=false and host -ffp-contract=off (the compilers contract nothing by
 themselves -- fused multiply-adds are the explicit fma() calls of the canonical arithmetic -- so results are reproducible bit
-for bit against the specification), -lineinfo (ncu source page).  csrc/dgswem.cu compiles kernels and host code twice (fp64, fp32)."""
+for bit against the specification), -lineinfo (ncu source page).  csrc/dgswem.cu compiles kernels and host code twice (fp64, fp32);
+csrc/dgswem_static.cu (the allocation-free nodal output) is linked into the same library."""
 from __future__ import annotations
 
 import os
@@ -13,7 +14,8 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 SRC = PKG / "csrc" / "dgswem.cu"
-DEPS = [SRC, PKG / "csrc" / "dgswem_kernels.cuh", PKG / "csrc" / "dgswem_impl.inl", ROOT / "include" / "dgswem.h"]
+SRC_STATIC = PKG / "csrc" / "dgswem_static.cu"   # dgswem_nodal_static: own translation unit, own file-scope scratch
+DEPS = [SRC, SRC_STATIC, PKG / "csrc" / "dgswem_kernels.cuh", PKG / "csrc" / "dgswem_impl.inl", ROOT / "include" / "dgswem.h"]
 LIB = PKG / "libdgswem.so"
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false", "-split-compile", "0",
@@ -32,7 +34,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         return LIB
     tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
     extra = os.environ.get("DGSWEM_NVCC_EXTRA", "").split()   # tuning sweeps: e.g. -DDGK_STAGE_MINB=4
-    cmd = [nvcc(), *NVCC_FLAGS, *extra, "-I", str(ROOT / "include"), "-I", str(PKG / "csrc"), "-o", str(tmp), str(SRC)]
+    cmd = [nvcc(), *NVCC_FLAGS, *extra, "-I", str(ROOT / "include"), "-I", str(PKG / "csrc"), "-o", str(tmp), str(SRC), str(SRC_STATIC)]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd))
