@@ -139,7 +139,10 @@ int dgswem_end_step(dgswem_t*);
  * halo_pack / halo_unpack calls with device buffers) with dgswem_capture_mode(1) ... (0) while its own stream capture
  * is active on streams that include this handle's.  Before replaying the graph n <= 4096 times the caller calls
  * dgswem_graph_steps(n, dt) -- dt as recorded --: it tabulates the scalars of the next n steps, uploads them on the
- * handle's stream, resets the counter and advances the handle's time by n dt.  Same bits as the unrecorded calls. */
+ * handle's stream, resets the counter and advances the handle's time by n dt.  Same bits as the unrecorded calls.
+ * While capture mode is on, dgswem_step and every call that synchronises the handle's stream (set_state, eval_rhs, all
+ * get_* calls, sync, profile_read, test_math, fp64_peak, halo_pack / halo_unpack with host buffers) return
+ * DGSWEM_E_ARG: a synchronisation inside a stream capture would invalidate the capture. */
 int dgswem_capture_mode(dgswem_t*, int on);
 int dgswem_graph_steps(dgswem_t*, int64_t nsteps, double dt);
 int dgswem_set_halo(dgswem_t*, int64_t n_send, const int32_t* send_ids, int64_t n_recv, const int32_t* recv_ids);

@@ -320,6 +320,8 @@ struct Handle : ::dgswem {
 };
 
 #define CK(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return h->cuda_fail(e__, #call); } while (0)
+// entry points that synchronise the handle's stream: a synchronisation inside a stream capture invalidates the capture
+#define NO_CAPTURE() do { if (h->capturing) return h->fail(DGSWEM_E_ARG, "capture mode is on and this call synchronises the stream, which would invalidate the capture (dgswem_capture_mode(0) first)"); } while (0)
 #define CKL(name) do { cudaError_t e__ = cudaGetLastError(); if (e__ != cudaSuccess) return h->cuda_fail(e__, name); h->launches++; } while (0)
 
 enum ProfKind { PK_WIND = 0, PK_EDGE = 1, PK_ELEM = 2, PK_LIMWD = 3, PK_COUNT = 4 };
@@ -634,7 +636,7 @@ int launch_limwd(Handle* h, real* w) {
   const int grid = std::max(1, std::min(ntiles, h->res_limwd > 0 ? h->res_limwd : ntiles));
   if (h->prm.limiter == 2) {   // vertex neighbourhood: extrema of the means around every node first
     k_node_minmax<<<grid_for(h->nn, 256), 256, 0, h->stream>>>(h->nmm, h->ldn, h->mean, h->node_ptr, h->node_ev, (int)h->nn);
-    if (cudaGetLastError() == cudaSuccess) h->launches++;
+    CKL("k_node_minmax");   // a failed launch must not let the limiter run on stale node extrema
     k_limwd_tma<P, 2><<<grid, 128, LimTile<P>::kSmem, h->stream>>>(A, ntiles);
   } else {
     k_limwd_tma<P, 1><<<grid, 128, LimTile<P>::kSmem, h->stream>>>(A, ntiles);
@@ -1265,6 +1267,7 @@ int api_create(dgswem_t** out, const dgswem_params* prm, const dgswem_devhooks* 
 
 int api_set_state(Handle* h, double t, const double* ze, const double* qx, const double* qy) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   if (!ze || !qx || !qy) return h->fail(DGSWEM_E_ARG, "NULL state pointer");
   CK(cudaSetDevice(h->prm.device));
   const double* src[3] = {ze, qx, qy};
@@ -1376,6 +1379,7 @@ int api_end_step(Handle* h) {
   if (h->step_dt == 0.0) return h->fail(DGSWEM_E_ARG, "no step in progress (dgswem_begin_step)");
   if (h->capturing) {
     // being recorded into the caller's graph, not run: time does not move; the replayed step ends by moving to the next table row
+    CK(cudaSetDevice(h->prm.device));
     k_advance<<<1, 1, 0, h->stream>>>(h->step_ctr);
     CKL("k_advance");
   } else {
@@ -1460,6 +1464,7 @@ static int halo_rows(const Handle* h, int what) { return what == 0 ? 3 * h->ndof
 int api_halo_pack(Handle* h, int what, double* buf, int buf_on_device) {
   if (!h) return DGSWEM_E_ARG;
   if ((what != 0 && what != 1) || (!buf && h->n_send > 0)) return h->fail(DGSWEM_E_ARG, "bad halo_pack arguments");
+  if (!buf_on_device) NO_CAPTURE();   // the host-buffer form copies back and synchronises
   if (h->n_send == 0) return DGSWEM_OK;
   CK(cudaSetDevice(h->prm.device));
   const int rows = halo_rows(h, what);
@@ -1477,6 +1482,7 @@ int api_halo_pack(Handle* h, int what, double* buf, int buf_on_device) {
 int api_halo_unpack(Handle* h, int what, const double* buf, int buf_on_device) {
   if (!h) return DGSWEM_E_ARG;
   if ((what != 0 && what != 1) || (!buf && h->n_recv > 0)) return h->fail(DGSWEM_E_ARG, "bad halo_unpack arguments");
+  if (!buf_on_device) NO_CAPTURE();   // the host-buffer form synchronises
   if (h->n_recv == 0) return DGSWEM_OK;
   CK(cudaSetDevice(h->prm.device));
   const int rows = halo_rows(h, what);
@@ -1495,6 +1501,7 @@ int api_halo_unpack(Handle* h, int what, const double* buf, int buf_on_device) {
 
 int api_eval_rhs(Handle* h, double* rze, double* rqx, double* rqy) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   if (!rze || !rqx || !rqy) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
   if (h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a stage-granular step is in progress: its stage buffer is the scratch of dgswem_eval_rhs");
   CK(cudaSetDevice(h->prm.device));
@@ -1529,6 +1536,7 @@ int api_eval_rhs(Handle* h, double* rze, double* rqx, double* rqy) {
 
 int api_get_flux(Handle* h, double* flux) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   if (!flux) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
   if (h->fused && h->step_dt != 0.0) return h->fail(DGSWEM_E_ARG, "a stage-granular step is in progress");
   CK(cudaSetDevice(h->prm.device));
@@ -1549,6 +1557,7 @@ int api_get_flux(Handle* h, double* flux) {
 
 int api_get_state(Handle* h, double* t, double* ze, double* qx, double* qy) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   if (!ze || !qx || !qy) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
   CK(cudaSetDevice(h->prm.device));
   k_tiled_to_rows<<<dim3(grid_for(h->ne, 256), 3 * h->ndof), 256, 0, h->stream>>>(h->stage_buf, h->ld, h->W[0], h->inv_e, (int)h->ne, 3 * h->ndof);
@@ -1572,6 +1581,7 @@ int api_get_state(Handle* h, double* t, double* ze, double* qx, double* qy) {
 
 int api_get_wetdry(Handle* h, uint8_t* wet) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   if (!wet) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
   CK(cudaSetDevice(h->prm.device));
   const unsigned char* src = h->wet;
@@ -1587,6 +1597,7 @@ int api_get_wetdry(Handle* h, uint8_t* wet) {
 
 int api_get_nodal(Handle* h, double* zn, double* qxn, double* qyn) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   if (!zn || !qxn || !qyn) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
   CK(cudaSetDevice(h->prm.device));
   double* out = h->stage_buf;   // [3][ldn] (3 * ldn <= the state-sized staging buffer: n_nodes < n_elem + 3 for any triangulation with a boundary)
@@ -1604,6 +1615,7 @@ int api_get_nodal(Handle* h, double* zn, double* qxn, double* qyn) {
 
 int api_get_wind(Handle* h, double* tau) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   if (!tau) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
   CK(cudaSetDevice(h->prm.device));
   k_gather_rows<<<dim3(grid_for(h->nn, 256), 2), 256, 0, h->stream>>>(h->stage_buf, h->ldn, h->tau, h->ldn, nullptr, (int)h->nn, 2);
@@ -1616,6 +1628,7 @@ int api_get_wind(Handle* h, double* tau) {
 
 int api_get_pressure(Handle* h, double* etap) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   if (!etap) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
   CK(cudaSetDevice(h->prm.device));
   k_gather_rows<<<dim3(grid_for(h->nn, 256), 1), 256, 0, h->stream>>>(h->stage_buf, h->ldn, h->etap, h->ldn, nullptr, (int)h->nn, 1);
@@ -1627,6 +1640,7 @@ int api_get_pressure(Handle* h, double* etap) {
 
 int api_test_math(Handle* h, int64_t n, const double* x, double* out) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   if (n < 1 || !x || !out) return h->fail(DGSWEM_E_ARG, "need n >= 1 and non-NULL pointers");
   CK(cudaSetDevice(h->prm.device));
   double* dx = (double*)h->dalloc((size_t)n * sizeof(double));
@@ -1645,6 +1659,7 @@ int api_test_math(Handle* h, int64_t n, const double* x, double* out) {
 
 int api_fp64_peak(Handle* h, double* dfma_per_s) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   if (!dfma_per_s) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
   CK(cudaSetDevice(h->prm.device));
   int sms = 0;
@@ -1682,6 +1697,7 @@ int api_profile(Handle* h, int enable) {
 
 int api_profile_read(Handle* h, double* ms, int64_t* count) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   if (!ms || !count) return h->fail(DGSWEM_E_ARG, "NULL output pointer");
   CK(cudaSetDevice(h->prm.device));
   CK(cudaStreamSynchronize(h->stream));
@@ -1697,6 +1713,7 @@ int api_profile_read(Handle* h, double* ms, int64_t* count) {
 
 int api_sync(Handle* h) {
   if (!h) return DGSWEM_E_ARG;
+  NO_CAPTURE();
   CK(cudaSetDevice(h->prm.device));
   CK(cudaStreamSynchronize(h->stream));
   return DGSWEM_OK;

@@ -82,6 +82,7 @@ class PartitionedDgswem:
     only and `transport` must be a DistTransport whose ranks are the part ids."""
 
     def __init__(self, params, xy, bathy, tri, edge_elem, edge_local, edge_bc, elem_edge, n_parts, *, tide=None, holland=None,
+                 pressure=False, rain=0.0, precision=64,
                  reorder=1, device=0, parts=None, transport=None, part_of_element=None, overlap=None, graph=False):
         import torch
         from .binding import Dgswem
@@ -109,11 +110,17 @@ class PartitionedDgswem:
         for p in self.mine:
             sm = self.subs[p]
             g = Dgswem(params, sm.xy, bathy[sm.node_gid], sm.tri, sm.edge_elem, sm.edge_local, sm.edge_bc, sm.elem_edge,
-                       reorder=reorder, device=device)
+                       reorder=reorder, device=device, precision=precision)
             if tide is not None:
                 g.set_tide(*tide)
             if holland is not None:
                 g.set_wind_holland(holland)
+                if pressure:                               # surface-pressure gradient of the vortex (R-15)
+                    g.set_wind_forcing(True, True)
+            elif pressure:
+                raise ValueError("pressure=True needs a Holland vortex (holland=...)")
+            if rain:
+                g.set_rain(float(rain))                    # uniform mass source (R-16)
             plan = HaloPlan(sm)
             g.set_halo(plan.send_ids, plan.recv_ids)
             rows = g.halo_rows(0)
@@ -126,6 +133,16 @@ class PartitionedDgswem:
         # LocalTransport indexes plans by part id: only valid when this process drives all parts
         if parts is not None and isinstance(self.transport, LocalTransport):
             raise ValueError("driving a subset of the partitions needs a DistTransport")
+
+    @classmethod
+    def from_workload(cls, w, n_parts, **kw):
+        """Every forcing the workload carries (tide, vortex, and the pressure / rain notes of workloads.with_forcing), as
+        Dgswem.from_workload applies them to an undivided run, and the initial state."""
+        m = w.mesh
+        pd = cls(w.params, m.xy, w.bathy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, n_parts, tide=w.tide,
+                 holland=w.holland, pressure=bool(w.notes.get("pressure")), rain=float(w.notes.get("rain") or 0.0), **kw)
+        pd.set_state(0.0, w.ze, w.qx, w.qy)
+        return pd
 
     # ------------------------------------------------------------------
     def _exchange_begin(self, what):

@@ -134,3 +134,64 @@ def test_stage_api_equals_dgswem_step_and_rejects_misuse(G):
     with pytest.raises(G.DgswemError):
         b.graph_steps(5000, w.dt)           # more rows than the scalar table holds
     a.close(); b.close()
+
+
+def test_capture_mode_refuses_calls_that_synchronise(G):
+    """While a stage-granular step is being recorded into the caller's graph (dgswem_capture_mode(1)) a call that
+    synchronises the handle's stream would invalidate the capture: such calls are refused with DGSWEM_E_ARG and work
+    again once capture mode is off."""
+    w = c3(nn=20, nsteps=2)
+    g = G.Dgswem.from_workload(w)
+    g.capture_mode(True)
+    for call in (g.get_state, g.get_wetdry, g.get_nodal, g.eval_rhs, g.get_flux, g.sync, lambda: g.step(1, w.dt),
+                 lambda: g.set_state(0.0, w.ze, w.qx, w.qy)):
+        with pytest.raises(G.DgswemError, match="capture mode") as ei:
+            call()
+        assert ei.value.code == -1
+    g.capture_mode(False)
+    g.step(2, w.dt)
+    t, *_ = g.get_state()
+    assert t == 2 * w.dt
+    g.close()
+
+
+def _with_params(w, **kw):
+    from workloads.configs import Workload
+    prm = dict(w.params); prm.update(kw)
+    return Workload(w.name, w.mesh, w.bathy, prm, w.ze, w.qx, w.qy, w.dt, w.nsteps, tide=w.tide, holland=w.holland, notes=w.notes)
+
+
+VARIANTS = {
+    "roe": lambda: _with_params(c4(nqx=48, nqy=24, nsteps=30), flux=1),
+    "ssp43": lambda: _with_params(c5(nn=30, nsteps=16), rk_stages=4),
+    "ssp42-p1": lambda: _with_params(perturbed(c3(nn=40, nsteps=20)), rk_stages=4),
+    "p3": lambda: perturbed(c5(nn=30, nsteps=12, p=3), amp_z=0.2),
+    "pressure-rain": lambda: __import__("workloads").with_forcing(c5(nn=30, nsteps=16, p=1, rk_order=2), pressure=True, rain=2.5e-5),
+    "f32": lambda: c4(nqx=48, nqy=24, nsteps=30),
+}
+
+
+@pytest.mark.parametrize("graph", [False, True], ids=["stream", "graph"])
+@pytest.mark.parametrize("variant", sorted(VARIANTS))
+def test_partitioned_run_of_the_method_variants(O, G, variant, graph):
+    """Roe flux, many-stage SSP-RK, p = 3, pressure-gradient + rain forcing and binary32 working precision in a
+    decomposed run (three partitions, PartitionedDgswem.from_workload, which hands every forcing of the workload to
+    every handle): owned elements bit-equal to the oracle's undivided run (the binary32 oracle for precision 32)."""
+    from paper_2508_21208_b200.decomp import PartitionedDgswem
+    w = VARIANTS[variant]()
+    if variant == "f32":
+        from oracle import oracle32
+        oracle32.build()
+        o = oracle32.Oracle.from_workload(w)
+    else:
+        o = O.Oracle.from_workload(w)
+    o.step(w.nsteps, w.dt)
+    t_orc, *s_orc = o.get_state()
+    pd = PartitionedDgswem.from_workload(w, 3, graph=graph, precision=32 if variant == "f32" else 64)
+    pd.step(w.nsteps, w.dt)
+    t, *s = pd.get_state()
+    assert t == t_orc
+    for c in range(3):
+        assert np.isfinite(s_orc[c]).all() and np.array_equal(s[c], np.asarray(s_orc[c], dtype=np.float64))
+    assert np.array_equal(pd.get_wetdry(), o.get_wetdry())
+    pd.close()
