@@ -116,6 +116,8 @@ int dgswem_step(dgswem_t*, int64_t nsteps, double dt);
  * exchange what=0 };  end_step  -- where "exchange" = halo_pack on the owner, transport, halo_unpack on the ghost side.
  * The ghost elements' own results are meaningless and are overwritten by every exchange; owned elements then get the
  * same bits as in an undivided run.  dgswem_step must not be called between begin_step and end_step.
+ * With the vertex-neighbourhood limiter (limiter = 2) the ghost layer must hold every foreign element that shares a NODE
+ * with an owned element (the limiter takes the extrema of the means around each vertex), not only the edge-neighbours.
  *   dgswem_set_halo: element ids (caller numbering of this handle) to pack (owned elements that are ghosts elsewhere)
  *   and to unpack (this handle's ghosts); copied.  what = 0: the stage buffer written last (3*ndof rows; the current
  *   state between steps), what = 1: the RK-updated means (3 rows).  buf: [rows][n_send] resp. [rows][n_recv] doubles,

@@ -1414,8 +1414,6 @@ int api_graph_steps(Handle* h, int64_t nsteps, double dt) {
 
 int api_set_halo(Handle* h, int64_t n_send, const int32_t* send_ids, int64_t n_recv, const int32_t* recv_ids) {
   if (!h) return DGSWEM_E_ARG;
-  if (h->prm.limiter == 2)
-    return h->fail(DGSWEM_E_ARG, "the vertex-neighbourhood limiter needs the elements around every vertex: one layer of edge-neighbour ghosts is not enough");
   if (n_send < 0 || n_recv < 0 || (n_send > 0 && !send_ids) || (n_recv > 0 && !recv_ids)) return h->fail(DGSWEM_E_ARG, "bad halo lists");
   CK(cudaSetDevice(h->prm.device));
   // caller numbering -> internal numbering (host copy of inv_e)

@@ -86,11 +86,11 @@ class PartitionedDgswem:
                  reorder=1, device=0, parts=None, transport=None, part_of_element=None, overlap=None, graph=False):
         import torch
         from .binding import Dgswem
-        if int(params["limiter"]) == 2:
-            raise ValueError("the vertex-neighbourhood limiter (limiter = 2) needs every element around a vertex; the "
-                             "partitions carry one layer of edge-neighbour ghosts only: use limiter 0 or 1")
         self.torch = torch
-        self.subs = partition(xy, tri, edge_elem, edge_local, edge_bc, elem_edge, n_parts, part=part_of_element)
+        # the vertex-neighbourhood limiter bounds an element by the means of every element around its vertices: its
+        # partitions carry all foreign elements that share a node with an owned one, not only the edge-neighbours
+        self.subs = partition(xy, tri, edge_elem, edge_local, edge_bc, elem_edge, n_parts, part=part_of_element,
+                              ghost="vertex" if int(params["limiter"]) == 2 else "edge")
         self.mine = list(range(n_parts)) if parts is None else list(parts)
         self.transport = transport if transport is not None else LocalTransport()
         # overlap of the exchange with the interior elements: on by default where there is a wire to hide (one partition per
@@ -100,6 +100,7 @@ class PartitionedDgswem:
         self.cap = torch.cuda.Stream(device=device)       # the stream a whole step is recorded on and replayed from (graph=True)
         self.graph = bool(graph)
         self._graph, self._graph_dt = None, None
+        self.launches_per_graph_step = 0
         if self.graph and transport is not None and not isinstance(transport, LocalTransport):
             raise ValueError("graph=True records device copies between partitions of one process: LocalTransport only")
         self.n_elem = int(np.asarray(tri).shape[0])
@@ -247,6 +248,7 @@ class PartitionedDgswem:
     def _capture(self, dt):
         torch = self.torch
         torch.cuda.synchronize()
+        l0 = sum(g.launch_count() for g in self.handles)
         for g in self.handles:
             g.capture_mode(True)
         try:
@@ -263,6 +265,8 @@ class PartitionedDgswem:
             for g in self.handles:
                 g.capture_mode(False)
         self._graph, self._graph_dt = graph, dt
+        # kernels of the library recorded into one step of the graph (the library counts launches, recorded ones included)
+        self.launches_per_graph_step = sum(g.launch_count() for g in self.handles) - l0
 
     def get_state(self):
         """(t, ze, qx, qy) of the elements this process owns, scattered into global-size arrays (others stay NaN)."""

@@ -6,7 +6,9 @@ their centroids and returns, for every part, a self-contained local mesh in the 
 
   * local elements = the part's OWNED elements (in ascending global id) followed by its GHOST elements: the
     edge-neighbours of owned elements that belong to other parts (one layer: all the stage needs of a neighbour is its
-    state, and all the limiter needs is its mean);
+    state, and all the edge-neighbour limiter needs is its mean) -- or, with ghost="vertex", every foreign element that
+    shares a NODE with an owned element: the vertex-neighbourhood limiter (limiter = 2, R-18) bounds an
+    element by the means of all elements around its three vertices;
   * an edge with both elements local keeps its global orientation (e+, e-); an edge whose other element is not local --
     the outer edges of ghost elements -- is closed as a land edge of the local element (its result is never used: ghost
     elements are overwritten by every exchange); true boundary edges keep their code;
@@ -76,8 +78,12 @@ def element_parts(xy, tri, n_parts: int) -> np.ndarray:
     return part
 
 
-def partition(xy, tri, edge_elem, edge_local, edge_bc, elem_edge, n_parts: int, part: np.ndarray | None = None):
-    """Split the mesh into `n_parts` SubMesh objects (see the module docstring).  `part` overrides the element -> part map."""
+def partition(xy, tri, edge_elem, edge_local, edge_bc, elem_edge, n_parts: int, part: np.ndarray | None = None,
+              ghost: str = "edge"):
+    """Split the mesh into `n_parts` SubMesh objects (see the module docstring).  `part` overrides the element -> part map;
+    ghost = "edge" (edge-neighbours of owned elements) or "vertex" (every foreign element around a node of an owned one)."""
+    if ghost not in ("edge", "vertex"):
+        raise ValueError("ghost must be 'edge' or 'vertex'")
     xy = np.asarray(xy, dtype=np.float64)
     tri = np.asarray(tri, dtype=np.int32)
     edge_elem = np.asarray(edge_elem, dtype=np.int32)
@@ -102,6 +108,10 @@ def partition(xy, tri, edge_elem, edge_local, edge_bc, elem_edge, n_parts: int, 
         in_p, in_m = part_p == p, part_m == p
         cut = interior & (in_p != in_m)
         ghosts = np.unique(np.where(in_p[cut], em[cut], ep[cut]))
+        if ghost == "vertex":
+            touched = np.zeros(xy.shape[0], dtype=bool)
+            touched[tri[owned].ravel()] = True
+            ghosts = np.flatnonzero(touched[tri].any(axis=1) & (part != p))      # ascending global id; contains the edge-neighbours
         elem_gid = np.concatenate([owned, ghosts]).astype(np.int64)
         g2l = np.full(ne, -1, dtype=np.int64)
         g2l[elem_gid] = np.arange(elem_gid.size)

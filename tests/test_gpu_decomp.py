@@ -168,6 +168,9 @@ VARIANTS = {
     "p3": lambda: perturbed(c5(nn=30, nsteps=12, p=3), amp_z=0.2),
     "pressure-rain": lambda: __import__("workloads").with_forcing(c5(nn=30, nsteps=16, p=1, rk_order=2), pressure=True, rain=2.5e-5),
     "f32": lambda: c4(nqx=48, nqy=24, nsteps=30),
+    # vertex-neighbourhood limiter: partitions with a vertex ghost layer (every foreign element around an owned node)
+    "vertexlim-c4": lambda: _with_params(perturbed(c4(nqx=48, nqy=24, nsteps=30), amp_z=0.2), limiter=2),
+    "vertexlim-c5p2": lambda: _with_params(perturbed(c5(nn=30, nsteps=16), amp_z=0.2), limiter=2),
 }
 
 

@@ -53,6 +53,38 @@ def test_partition_invariants(n_parts):
         assert sum(v.size for v in s.recv.values()) == s.n_local - s.n_owned
 
 
+@pytest.mark.parametrize("n_parts", [2, 5])
+def test_vertex_ghost_layer_for_the_vertex_limiter(n_parts):
+    """ghost="vertex" (what PartitionedDgswem uses with limiter = 2): the ghosts of a part are exactly the foreign elements
+    that share a node with one of its owned elements -- so every node of an owned element has, locally, the same set of
+    incident elements as in the whole mesh (what the node extrema of DESIGN.md R-18 are taken over) -- the
+    edge-neighbour layer is contained in it, and the halo lists still pair up element by element."""
+    from paper_2508_21208_b200.partition import partition
+    w = _mesh(); m = w.mesh
+    edge_subs = partition(m.xy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, n_parts)
+    subs = partition(m.xy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, n_parts, ghost="vertex")
+    around = [set() for _ in range(m.n_nodes)]
+    for e, t in enumerate(m.tri):
+        for n in t:
+            around[n].add(e)
+    for s, se in zip(subs, edge_subs):
+        own = set(s.elem_gid[:s.n_owned].tolist())
+        ghosts = set(s.elem_gid[s.n_owned:].tolist())
+        want = set().union(*[around[n] for e in own for n in m.tri[e]]) - own
+        assert ghosts == want and ghosts >= set(se.elem_gid[se.n_owned:].tolist()) and len(ghosts) > se.n_local - se.n_owned
+        local = set(s.elem_gid.tolist())
+        for e in own:
+            for n in m.tri[e]:
+                assert around[n] <= local
+        assert np.array_equal(m.tri[s.elem_gid], s.node_gid[s.tri])
+        for q, ids in s.recv.items():
+            assert np.array_equal(s.elem_gid[ids], subs[q].elem_gid[subs[q].send[s.part]])
+            assert (ids >= s.n_owned).all() and (subs[q].send[s.part] < subs[q].n_owned).all()
+        assert sum(v.size for v in s.recv.values()) == s.n_local - s.n_owned
+    with pytest.raises(ValueError):
+        partition(m.xy, m.tri, m.edge_elem, m.edge_local, m.edge_bc, m.elem_edge, 2, ghost="node")
+
+
 def test_local_meshes_pass_the_library_validation():
     """dgswem_create validates tables on the host before touching CUDA: every local mesh must get past it."""
     import ctypes as C
