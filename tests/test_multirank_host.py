@@ -84,3 +84,25 @@ def test_both_arms_name_the_workload_with_the_same_config_keys():
     assert set(cfg) == {"workload", "n_elem", "n_edge", "n_nodes", "p", "rk_order", "dt", "limiter", "wetdry", "flux", "wind", "tide", "l2"}
     src = (ROOT / "bench.py").read_text()
     assert src.count('"config": workload_config(w)') + src.count('"config": cfg') >= 2
+
+
+def test_bench_bookkeeping_plain_stages_and_traffic_table():
+    """Roofline bookkeeping of bench.py: the number of stages that do not read w^n follows the scheme (1 for SSP(2,2) and
+    SSP(3,3), s-1 for SSP(s,2), 3 for SSP(4,3)), and profiles/traffic.csv parses into per-(workload, kernel) records that
+    name their ncu capture."""
+    import bench
+    from workloads import c1
+    from workloads.configs import Workload
+
+    def with_rk(order, stages):
+        w = c1(nq=4)
+        prm = dict(w.params); prm.update(rk_order=order, rk_stages=stages)
+        return Workload(w.name, w.mesh, w.bathy, prm, w.ze, w.qx, w.qy, w.dt, w.nsteps)
+
+    assert [bench.plain_stages(with_rk(o, s)) for o, s in ((2, 0), (3, 0), (2, 3), (2, 4), (3, 4))] == [1, 1, 2, 3, 3]
+    tr = bench.read_traffic()
+    rec = tr[("C3", "stage")]
+    assert rec["dram_bytes"] > 1e9 and rec["source"] and rec["fp64_inst_per_elem"] > 100
+    assert all(v["source"] for v in tr.values())
+    w = bench.make_workload("C1+perturbed")
+    assert w.name.endswith("+perturbed") and abs(w.qx).max() > 0
